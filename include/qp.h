@@ -1,0 +1,128 @@
+/*
+ * qp.h -- C ABI of libqp.so: B200-native (sm_100a) all-pairs posterior stage of QuickProbs 2.
+ *
+ * What it computes (Methods, stage I): "Posterior probability matrices are calculated for all
+ * sequence pairs on the basis of hidden Markov model and partition function. The matrices are further employed
+ * to establish maximum expected accuracy alignments. Alignment scores are used to estimate pairwise distances".
+ * The matrices are kept "in a sparse form" (footnote). The paper prints no recurrence or constant;
+ * the exact definitions are the readings of SURVEY.md section 8(c) (c-1 model, c-2 combine/threshold/MEA/distance),
+ * restated in DESIGN.md. Every step (schedule, forward, backward, combine, sparsify, expected accuracy) runs in
+ * CUDA kernels; there is no CPU fallback.
+ *
+ * Conventions
+ *  - "d_" pointers are DEVICE pointers owned by the caller (e.g. torch tensors); "h_"/struct pointers are HOST.
+ *  - The library allocates no device memory: scratch comes from the caller's workspace.
+ *  - Work is enqueued on `cuda_stream` (a cudaStream_t passed as void*). With QP_FLAG_SYNC_STATUS the call
+ *    synchronises the stream once at the end, reads the device status word and returns it; without it the call
+ *    returns after enqueueing and device-detected errors are only visible in qp_output.status.
+ *  - Return value: 0 (QP_OK) or a negative QP_ERR_* code. No exception or abort crosses the ABI.
+ *  - Rows of pair p's matrix = residues of the FIRST index of d_pairs[p]; columns = residues of the second.
+ */
+#ifndef QP_H_
+#define QP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define QP_MAX_INS 2
+#define QP_MAX_ALPHABET 31 /* residue codes 0..alphabet-1; code 31 is reserved internally */
+#define QP_MAX_LEN 65535   /* longest supported sequence (CSR scratch packs a column offset in 16 bits) */
+
+enum {
+    QP_OK = 0,
+    QP_ERR_INVALID_ARG = -1,        /* NULL pointer, bad alphabet / n_ins / threshold / precision, P or k < 0  */
+    QP_ERR_BAD_RESIDUE = -2,        /* a residue code >= alphabet                (device-detected)              */
+    QP_ERR_EMPTY_SEQUENCE = -3,     /* a listed sequence has length 0 or > QP_MAX_LEN (device-detected)         */
+    QP_ERR_BAD_PAIR = -4,           /* pair index out of [0,k) or x == y          (device-detected)              */
+    QP_ERR_WORKSPACE_TOO_SMALL = -5,/* workspace cannot hold the fixed arrays + one scratch slot per class     */
+    QP_ERR_NNZ_CAPACITY = -6,       /* CSR needs more than nnz_capacity entries; pair_nnz_base[P] = required   */
+    QP_ERR_CUDA = -7,               /* a CUDA runtime call failed                                              */
+    QP_ERR_RANGE = -8               /* model weights outside the dynamic range the kernels renormalise for     */
+};
+
+enum { QP_FP32 = 0, QP_FP64 = 1 };
+
+enum {
+    QP_FLAG_SYNC_STATUS = 1,        /* synchronise the stream at the end and return the device status          */
+    QP_FLAG_NO_REFINE = 2           /* QP_FP32 only: skip the fp64 re-evaluation of near-identical pairs        */
+};
+
+/*
+ * One weighted pair automaton, natural-log weights. States M, X_1..X_G, Y_1..Y_G;
+ * X/Y symmetric by construction; no X<->Y transition. -INFINITY is a legal weight (probability 0).
+ *   HMM instance: log_match = ln e(a,b), log_ins = ln q(a), t_MI = ln delta_g, t_II = ln eps_g,
+ *                 t_IM = ln(1-eps_g), t_MM = ln(1-2 sum delta), init/end = ln pi.
+ *   PF instance (substitution matrix, gap penalties, temperature), passed already divided by T:
+ *                 log_match = s(a,b)/T, log_ins = 0, t_MM = t_IM = 0, t_MI = init_I = -g_open/T, t_II = -g_ext/T,
+ *                 init_M = end = 0.
+ */
+typedef struct {
+    int32_t n_ins;           /* G: 1 or 2                                                   */
+    int32_t alphabet;        /* A: 2..QP_MAX_ALPHABET, the same for both models             */
+    const double* log_match; /* host, A*A row-major, must be symmetric                      */
+    const double* log_ins;   /* host, A                                                     */
+    double t_MM, t_MI[QP_MAX_INS], t_II[QP_MAX_INS], t_IM[QP_MAX_INS];
+    double init_M, init_I[QP_MAX_INS], end_M, end_I[QP_MAX_INS];
+} qp_model;
+
+typedef struct {
+    qp_model hmm, pf;
+    double threshold;        /* tau > 0: CSR keeps P(i,j) >= tau (value from BASELINE.json)        */
+    int32_t precision;       /* QP_FP32 | QP_FP64: arithmetic of the DP kernels                                */
+    int32_t flags;           /* QP_FLAG_*                                                                      */
+    double refine_below;     /* QP_FP32: pairs whose fp32 distance is below this are re-evaluated in fp64
+                                (distance only). <= 0 selects the default 0.25. See DESIGN.md "Precision".      */
+} qp_params;
+
+/* Outputs. All device memory, caller-allocated. Optional members may be NULL. */
+typedef struct {
+    int64_t* pair_row_base;  /* [P+1] exclusive prefix of (n_p+1): pair p's row_ptr starts here                 */
+    int64_t* pair_nnz_base;  /* [P+1] exclusive prefix of nnz_p:   pair p's col_idx/val start here              */
+    int32_t* row_ptr;        /* [sum(n_p+1)] offsets local to the pair (0..nnz_p)                               */
+    int32_t* col_idx;        /* [nnz_capacity] 0-based column (residue of the second sequence), ascending/row  */
+    float* val;              /* [nnz_capacity] combined posterior P(i,j) >= tau                                 */
+    int64_t nnz_capacity;
+    float* dist;             /* [k*k] row-major; (x,y) and (y,x) are written for listed pairs only              */
+    float* dense_P;          /* optional: concatenated dense n_p*m_p row-major matrices, pair order (tests)    */
+    double* logZ;            /* optional [P][4]: ln Z of hmm fwd, hmm bwd, pf fwd, pf bwd                        */
+    int32_t* status;         /* [4] device status word: {code, pair index or -1, detail, refined pair count}    */
+} qp_output;
+
+/*
+ * Host-only query (no device access): bytes of workspace that let every scheduling class run with its full
+ * complement of resident warps, capped at budget_bytes (0 = no cap). Never less than the minimum that
+ * qp_posteriors accepts for this input. h_offsets [k+1], h_pairs [P][2] are host copies of the device inputs.
+ * Errors: QP_ERR_INVALID_ARG, QP_ERR_BAD_PAIR, QP_ERR_EMPTY_SEQUENCE, QP_ERR_WORKSPACE_TOO_SMALL (budget below
+ * the minimum; *out_bytes then holds the minimum).
+ */
+int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int32_t* h_pairs, int64_t P,
+                       const qp_params* params, int64_t nnz_capacity, int want_dense, size_t budget_bytes,
+                       size_t* out_bytes);
+
+/*
+ * The hot path. d_seqs: packed residue codes (uint8); d_offsets [k+1]: sequence s is
+ * d_seqs[d_offsets[s] .. d_offsets[s+1]); d_pairs [P][2] int32. Steps, all on the device:
+ *   a0 schedule (class by stripe width, longest-first order, scratch slots)
+ *   a1-a4 pair-HMM and partition-function forward and backward
+ *   a5 combine P = sqrt((P_hmm^2+P_pf^2)/2), a6 threshold + CSR compaction
+ *   a7 expected-accuracy (MEA) max-plus DP and d = 1 - A(n,m)/min(n,m)
+ * d_workspace must be 256-byte aligned. Outputs for pairs after an error are unspecified.
+ */
+int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, const int32_t* d_pairs, int64_t P,
+                  const qp_params* params, void* d_workspace, size_t workspace_bytes, const qp_output* out,
+                  void* cuda_stream);
+
+/* Number of kernels the last qp_posteriors call on this thread launched (bench.py's gpu_launches). */
+int qp_last_launch_count(void);
+
+const char* qp_status_string(int status);
+const char* qp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* QP_H_ */

@@ -1,0 +1,651 @@
+// qp_api.cu -- host side of the C ABI (include/qp.h) plus the small device-side scheduling kernels.
+//
+// Schedule ("redesigning graphics processor calculations to handle sequences of
+// any length ... more efficient memory allocation model"): everything below runs on the device, the host never
+// sees a sequence length.
+//   classify : per pair -> (rows n, cols m, stripe class C, scratch bytes -> size bin); histogram per class/bin
+//   bins     : per class, bins ordered largest first -> start position of every bin
+//   scatter  : counting sort of the pair indices into order[] (class-major, largest scratch first)
+//   slots    : grant W_c resident warps per class under the workspace budget; warp w's scratch slot is sized for
+//              the w-th largest pair of its class, which bounds every pair that warp will pull later
+//   scans    : pair_row_base (CSR row_ptr placement), dense offsets, and after the pair kernels pair_nnz_base
+//   copy     : staging pool (completion order) -> caller's col_idx/val in pair order
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+#include <algorithm>
+
+#include "qp.h"
+#include "qp_internal.h"
+
+namespace qp {
+
+template <typename R, int GP, int C> cudaError_t launch_pair(const KArgs<R>& ka, int grid, cudaStream_t st);
+#define QP_DECL_F32(C)                                                                          \
+    extern template cudaError_t launch_pair<float, 1, C>(const KArgs<float>&, int, cudaStream_t); \
+    extern template cudaError_t launch_pair<float, 2, C>(const KArgs<float>&, int, cudaStream_t);
+#define QP_DECL_F64(C) \
+    extern template cudaError_t launch_pair<double, 2, C>(const KArgs<double>&, int, cudaStream_t);
+QP_DECL_F32(2) QP_DECL_F32(4) QP_DECL_F32(6) QP_DECL_F32(8) QP_DECL_F32(10) QP_DECL_F32(12) QP_DECL_F32(14) QP_DECL_F32(16)
+QP_DECL_F64(2) QP_DECL_F64(4) QP_DECL_F64(6) QP_DECL_F64(8)
+
+constexpr uint32_t kMaskF32 = 0xff;   // C = 2..16
+constexpr uint32_t kMaskF64 = 0x0f;   // C = 2..8
+
+// ------------------------------------------------------------------------------------------------------------
+// device-side scheduling kernels
+// ------------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void set_status(SchedHeader* h, int code, int where) {
+    if (atomicCAS(&h->status[0], 0, code) == 0) h->status[1] = where;
+}
+
+__global__ void k_check_residues(const uint8_t* __restrict__ seqs, const int64_t* __restrict__ offs, int k, int A,
+                                 SchedHeader* h) {
+    const int64_t lo = offs[0], hi = offs[k];
+    for (int64_t q = lo + blockIdx.x * (int64_t)blockDim.x + threadIdx.x; q < hi; q += (int64_t)gridDim.x * blockDim.x)
+        if (seqs[q] >= A) set_status(h, QP_ERR_BAD_RESIDUE, -1);
+}
+
+__global__ void k_classify(const int64_t* __restrict__ offs, int k, const int32_t* __restrict__ pairs, int64_t P,
+                           uint32_t cmask, int real_bytes, PairInfo* __restrict__ info, int32_t* __restrict__ rows1,
+                           int64_t* __restrict__ cells, SchedHeader* h) {
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    const int x = pairs[2 * p], y = pairs[2 * p + 1];
+    PairInfo pi;
+    pi.xoff = pi.yoff = 0;
+    pi.n = pi.m = 0;
+    pi.cls = -1;
+    pi.nb = 0;
+    pi.bin = 0;
+    if (x < 0 || y < 0 || x >= k || y >= k || x == y) {
+        set_status(h, QP_ERR_BAD_PAIR, (int)p);
+    } else {
+        const int64_t n = offs[x + 1] - offs[x], m = offs[y + 1] - offs[y];
+        if (n < 1 || m < 1 || n > QP_MAX_LEN || m > QP_MAX_LEN) {
+            set_status(h, QP_ERR_EMPTY_SEQUENCE, (int)p);
+        } else {
+            pi.xoff = offs[x];
+            pi.yoff = offs[y];
+            pi.n = (int)n;
+            pi.m = (int)m;
+            int nb;
+            const int c = choose_class((int)m + 1, cmask, &nb);
+            pi.cls = (int16_t)c;
+            pi.nb = (int16_t)nb;
+            pi.bin = bin_of((uint64_t)slot_bytes((int)n, 2 * (c + 1), nb, real_bytes));
+            atomicAdd(&h->hist[c][pi.bin], 1u);
+        }
+    }
+    info[p] = pi;
+    rows1[p] = pi.n + 1;
+    if (cells) cells[p] = (int64_t)pi.n * pi.m;
+}
+
+__global__ void k_bins(SchedHeader* h) {
+    __shared__ int cnt[kNumClasses];
+    const int c = threadIdx.x;
+    if (c < kNumClasses) {
+        uint32_t run = 0;
+        for (int b = kNumBins - 1; b >= 0; --b) {
+            h->bin_start[c][b] = run;
+            run += h->hist[c][b];
+        }
+        cnt[c] = (int)run;
+        h->cls_count[c] = (int)run;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int s = 0;
+        for (int q = 0; q < kNumClasses; ++q) {
+            h->cls_start[q] = s;
+            s += cnt[q];
+        }
+    }
+}
+
+__global__ void k_scatter(const PairInfo* __restrict__ info, int64_t P, int32_t* __restrict__ order, SchedHeader* h) {
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= P) return;
+    const int c = info[p].cls;
+    if (c < 0) return;
+    const int b = info[p].bin;
+    const uint32_t pos = h->cls_start[c] + h->bin_start[c][b] + atomicAdd(&h->bin_fill[c][b], 1u);
+    order[pos] = (int32_t)p;
+}
+
+// block-wide exclusive scan of one value per thread (1024 threads), returns the exclusive prefix; total in *tot
+__device__ int64_t block_excl_scan(int64_t v, int64_t* sh, int64_t* tot) {
+    const int t = threadIdx.x;
+    sh[t] = v;
+    __syncthreads();
+    for (int o = 1; o < (int)blockDim.x; o <<= 1) {
+        int64_t a = (t >= o) ? sh[t - o] : 0;
+        __syncthreads();
+        sh[t] += a;
+        __syncthreads();
+    }
+    int64_t incl = sh[t];
+    *tot = sh[blockDim.x - 1];
+    __syncthreads();
+    return incl - v;
+}
+
+struct MaxW {
+    int w[kNumClasses];
+};
+
+// grant resident warps per class under the slot budget, then lay the slots out
+__global__ void k_slots(const PairInfo* __restrict__ info, const int32_t* __restrict__ order, MaxW maxw,
+                        int64_t avail, int64_t* __restrict__ slot_off, SchedHeader* h) {
+    __shared__ int64_t sh[1024];
+    __shared__ int W[kNumClasses], W0[kNumClasses + 1];
+    __shared__ int done, fail;
+    const int t = threadIdx.x;
+    for (int shift = 0;; ++shift) {
+        if (t == 0) {
+            int s = 0, all1 = 1;
+            for (int c = 0; c < kNumClasses; ++c) {
+                int cnt = h->cls_count[c];
+                int w = cnt ? max(1, min(cnt, maxw.w[c] >> shift)) : 0;
+                if (w > 1) all1 = 0;
+                W[c] = w;
+                W0[c] = s;
+                s += w;
+            }
+            W0[kNumClasses] = s;
+            done = all1;
+        }
+        __syncthreads();
+        const int N = W0[kNumClasses];
+        const int per = (N + blockDim.x - 1) / blockDim.x;
+        int64_t loc = 0;
+        for (int q = t * per; q < min(N, (t + 1) * per); ++q) {
+            int c = 0;
+            while (q >= W0[c + 1]) ++c;
+            loc += (int64_t)bin_ub(info[order[h->cls_start[c] + (q - W0[c])]].bin);
+        }
+        int64_t tot;
+        int64_t ex = block_excl_scan(loc, sh, &tot);
+        if (tot <= avail) {
+            for (int q = t * per; q < min(N, (t + 1) * per); ++q) {
+                int c = 0;
+                while (q >= W0[c + 1]) ++c;
+                slot_off[q] = ex;
+                ex += (int64_t)bin_ub(info[order[h->cls_start[c] + (q - W0[c])]].bin);
+            }
+            if (t == 0) fail = 0;
+            break;
+        }
+        if (done) {
+            if (t == 0) fail = 1;
+            break;
+        }
+        __syncthreads();
+    }
+    __syncthreads();
+    if (t < kNumClasses) {
+        h->cls_W[t] = fail ? 0 : W[t];
+        h->cls_slot0[t] = W0[t];
+        h->cls_cursor[t] = W[t];
+    }
+    if (t == 0 && fail) set_status(h, QP_ERR_WORKSPACE_TOO_SMALL, -1);
+}
+
+// out[0..P] = exclusive prefix of in[0..P-1]; single block
+template <typename T> __global__ void k_scan(const T* __restrict__ in, int64_t P, int64_t* __restrict__ out) {
+    __shared__ int64_t sh[1024];
+    const int t = threadIdx.x;
+    const int64_t per = (P + blockDim.x - 1) / blockDim.x;
+    const int64_t lo = min(P, t * per), hi = min(P, (t + 1) * per);
+    int64_t loc = 0;
+    for (int64_t q = lo; q < hi; ++q) loc += (int64_t)in[q];
+    int64_t tot;
+    int64_t ex = block_excl_scan(loc, sh, &tot);
+    for (int64_t q = lo; q < hi; ++q) {
+        out[q] = ex;
+        ex += (int64_t)in[q];
+    }
+    if (t == 0) out[P] = tot;
+}
+
+__global__ void k_copy_pool(const int32_t* __restrict__ nnz, const int64_t* __restrict__ pool_off,
+                            const int64_t* __restrict__ base, int64_t P, const int32_t* __restrict__ pool_col,
+                            const float* __restrict__ pool_val, int64_t cap, int32_t* __restrict__ col,
+                            float* __restrict__ val) {
+    const int64_t p = blockIdx.x * (int64_t)(blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (p >= P) return;
+    const int lane = threadIdx.x & 31;
+    const int64_t cnt = nnz[p], src = pool_off[p], dst = base[p];
+    if (src + cnt > cap || dst + cnt > cap) return;
+    for (int64_t q = lane; q < cnt; q += 32) {
+        col[dst + q] = pool_col[src + q];
+        val[dst + q] = pool_val[src + q];
+    }
+}
+
+struct MaxW64 {
+    int w[kNumClasses];
+};
+__global__ void k_refine_plan(MaxW64 maxw, int64_t avail, SchedHeader* h) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    unsigned long long used = 0;
+    int total = 0;
+    for (int c = 0; c < kNumClasses; ++c) {
+        const int cnt = h->refine_count[c];
+        int W = 0;
+        if (cnt > 0) {
+            const unsigned long long sb = h->refine_slot_bytes[c];
+            const long long fit = (long long)(((unsigned long long)avail - used) / sb);
+            W = (int)min((long long)min(cnt, maxw.w[c]), fit);
+            if (W <= 0) {
+                W = 0;
+                set_status(h, QP_ERR_WORKSPACE_TOO_SMALL, -1);
+            }
+            h->refine_slot0[c] = used;
+            used += (unsigned long long)W * sb;
+            total += cnt;
+        }
+        h->refine_W[c] = W;
+        h->refine_cursor[c] = W;
+    }
+    h->status[3] = total;
+}
+
+__global__ void k_finish(const SchedHeader* h, int32_t* status) {
+    if (threadIdx.x < 4) status[threadIdx.x] = h->status[threadIdx.x];
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// host
+// ------------------------------------------------------------------------------------------------------------
+static thread_local int g_launches = 0;
+
+struct Ctx {   // lazily created side streams so that the per-class kernels overlap their tails
+    bool ok = false;
+    int dev = -1, sms = kSmAssumed;
+    cudaStream_t st[kNumClasses];
+    cudaEvent_t fork, join[kNumClasses];
+};
+static thread_local Ctx g_ctx;
+
+static bool ctx_init() {
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    if (g_ctx.ok && g_ctx.dev == dev) return true;
+    g_ctx.dev = dev;
+    if (cudaDeviceGetAttribute(&g_ctx.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return false;
+    for (int c = 0; c < kNumClasses; ++c) {
+        if (cudaStreamCreateWithFlags(&g_ctx.st[c], cudaStreamNonBlocking) != cudaSuccess) return false;
+        if (cudaEventCreateWithFlags(&g_ctx.join[c], cudaEventDisableTiming) != cudaSuccess) return false;
+    }
+    if (cudaEventCreateWithFlags(&g_ctx.fork, cudaEventDisableTiming) != cudaSuccess) return false;
+    g_ctx.ok = true;
+    return true;
+}
+
+static inline int64_t align256(int64_t v) { return (v + 255) & ~(int64_t)255; }
+
+struct Layout {   // byte offsets inside the workspace
+    int64_t hdr, info, order, rows1, cells, nnz, pool_off, dense_off, slot_off, refine_list, pool_col, pool_val, slots;
+    int64_t fixed;   // everything before the slots
+};
+
+static Layout make_layout(int64_t P, int64_t nnz_cap, bool dense, int64_t max_slots) {
+    Layout L;
+    int64_t o = 0;
+    auto take = [&](int64_t bytes) {
+        int64_t r = o;
+        o += align256(bytes);
+        return r;
+    };
+    L.hdr = take(sizeof(SchedHeader));
+    L.info = take(P * (int64_t)sizeof(PairInfo));
+    L.order = take(P * 4);
+    L.rows1 = take(P * 4);
+    L.cells = take(dense ? P * 8 : 0);
+    L.nnz = take(P * 4);
+    L.pool_off = take(P * 8);
+    L.dense_off = take(dense ? (P + 1) * 8 : 0);
+    L.slot_off = take(max_slots * 8);
+    L.refine_list = take((int64_t)kNumClasses * P * 4);
+    L.pool_col = take(nnz_cap * 4);
+    L.pool_val = take(nnz_cap * 4);
+    L.slots = o;
+    L.fixed = o;
+    return L;
+}
+
+static int max_warps(int cls, bool fp64, int sms) { return sms * ctas_per_sm(2 * (cls + 1), fp64) * kWarpsPerCta; }
+static int64_t total_max_slots(int sms) {
+    int64_t s = 0;
+    for (int c = 0; c < kNumClasses; ++c) s += max_warps(c, false, sms);
+    return s;
+}
+
+static int check_model(const qp_model& m) {
+    if (m.n_ins < 1 || m.n_ins > QP_MAX_INS) return QP_ERR_INVALID_ARG;
+    if (m.alphabet < 2 || m.alphabet > QP_MAX_ALPHABET) return QP_ERR_INVALID_ARG;
+    if (!m.log_match || !m.log_ins) return QP_ERR_INVALID_ARG;
+    return QP_OK;
+}
+static int check_params(const qp_params* p) {
+    if (!p) return QP_ERR_INVALID_ARG;
+    int r = check_model(p->hmm);
+    if (r) return r;
+    r = check_model(p->pf);
+    if (r) return r;
+    if (p->hmm.alphabet != p->pf.alphabet) return QP_ERR_INVALID_ARG;
+    if (!(p->threshold > 0.0) || !(p->threshold <= 1.0)) return QP_ERR_INVALID_ARG;
+    if (p->precision != QP_FP32 && p->precision != QP_FP64) return QP_ERR_INVALID_ARG;
+    return QP_OK;
+}
+
+// linear-space weights after the background normalisation (posterior-invariant, SURVEY.md 8(c) pin 8):
+// em(a,b) = exp(lm[a][b] - lx[a] - lx[b]), insert emissions 1. Returns log2 of the largest per-row growth.
+template <typename R> static double prep_model(const qp_model& m, Weights<R>& w, double* em /*32x32*/, double* lx) {
+    const int A = m.alphabet;
+    auto ex = [](double v) { return v == -INFINITY ? 0.0 : std::exp(v); };
+    double emax = 0.0;
+    for (int a = 0; a < kTabDim; ++a) {
+        lx[a] = a < A ? m.log_ins[a] : 0.0;
+        for (int b = 0; b < kTabDim; ++b) {
+            double v = 0.0;
+            if (a < A && b < A) v = ex(m.log_match[a * A + b] - m.log_ins[a] - m.log_ins[b]);
+            em[a * kTabDim + b] = v;
+            emax = std::max(emax, v);
+        }
+    }
+    w.wMM = (R)ex(m.t_MM);
+    w.initM = (R)ex(m.init_M);
+    w.endM = (R)ex(m.end_M);
+    double wsum = ex(m.t_MM);
+    for (int g = 0; g < kMaxIns; ++g) {
+        const bool on = g < m.n_ins;
+        w.wMI[g] = on ? (R)ex(m.t_MI[g]) : R(0);
+        w.wII[g] = on ? (R)ex(m.t_II[g]) : R(0);
+        w.wIM[g] = on ? (R)ex(m.t_IM[g]) : R(0);
+        w.initI[g] = on ? (R)ex(m.init_I[g]) : R(0);
+        w.endI[g] = on ? (R)ex(m.end_I[g]) : R(0);
+        if (on) wsum += 2.0 * ex(m.t_IM[g]) + ex(m.t_II[g]) + ex(m.t_MI[g]);
+    }
+    return std::log2(std::max(1.0, emax) * std::max(1.0, wsum));
+}
+
+template <typename R> static int fill_kargs(const qp_params* prm, KArgs<R>& ka) {
+    double eh[kTabDim * kTabDim], ep[kTabDim * kTabDim];
+    const double gh = prep_model<R>(prm->hmm, ka.wh, eh, ka.lx_h);
+    const double gp = prep_model<R>(prm->pf, ka.wp, ep, ka.lx_p);
+    for (int q = 0; q < kTabDim * kTabDim; ++q) {
+        ka.tab[q].x = (R)eh[q];
+        ka.tab[q].y = (R)ep[q];
+        if (!std::isfinite((double)ka.tab[q].x) || !std::isfinite((double)ka.tab[q].y)) return QP_ERR_RANGE;
+    }
+    // renormalise often enough that values cannot leave the exponent range between two renormalisations
+    const double g = std::max(gh, gp), room = sizeof(R) == 4 ? 56.0 : 500.0;
+    int every = 8;
+    while (every > 1 && every * g > room) every >>= 1;
+    if (every * g > room) return QP_ERR_RANGE;
+    ka.rescale_mask = every - 1;
+    ka.tau = (R)prm->threshold;
+    return QP_OK;
+}
+
+static int launch_class_f32(int gp, int cls, const KArgs<float>& ka, int grid, cudaStream_t st) {
+    cudaError_t e = cudaErrorInvalidValue;
+#define QP_CASE(C)                                                                      \
+    case C / 2 - 1:                                                                     \
+        e = gp == 1 ? launch_pair<float, 1, C>(ka, grid, st) : launch_pair<float, 2, C>(ka, grid, st); \
+        break;
+    switch (cls) { QP_CASE(2) QP_CASE(4) QP_CASE(6) QP_CASE(8) QP_CASE(10) QP_CASE(12) QP_CASE(14) QP_CASE(16) }
+#undef QP_CASE
+    ++g_launches;
+    return e == cudaSuccess ? QP_OK : QP_ERR_CUDA;
+}
+static int launch_class_f64(int cls, const KArgs<double>& ka, int grid, cudaStream_t st) {
+    cudaError_t e = cudaErrorInvalidValue;
+    switch (cls) {
+        case 0: e = launch_pair<double, 2, 2>(ka, grid, st); break;
+        case 1: e = launch_pair<double, 2, 4>(ka, grid, st); break;
+        case 2: e = launch_pair<double, 2, 6>(ka, grid, st); break;
+        case 3: e = launch_pair<double, 2, 8>(ka, grid, st); break;
+    }
+    ++g_launches;
+    return e == cudaSuccess ? QP_OK : QP_ERR_CUDA;
+}
+
+template <typename R> static void fill_common(KArgs<R>& ka, const uint8_t* d_seqs, const int32_t* d_pairs, int32_t k,
+                                              char* ws, const Layout& L, const qp_output* out, int64_t P) {
+    ka.k = k;
+    ka.seqs = d_seqs;
+    ka.pairs = d_pairs;
+    ka.info = (const PairInfo*)(ws + L.info);
+    ka.order = (const int32_t*)(ws + L.order);
+    ka.hdr = (SchedHeader*)(ws + L.hdr);
+    ka.slot_off = (const int64_t*)(ws + L.slot_off);
+    ka.slots = ws + L.slots;
+    ka.refine_list = (int32_t*)(ws + L.refine_list);
+    ka.refine_stride = P;
+    ka.refine_cmask = kMaskF64;
+    ka.pair_row_base = out->pair_row_base;
+    ka.row_ptr = out->row_ptr;
+    ka.pool_col = (int32_t*)(ws + L.pool_col);
+    ka.pool_val = (float*)(ws + L.pool_val);
+    ka.pool_cap = out->nnz_capacity;
+    ka.nnz = (int32_t*)(ws + L.nnz);
+    ka.pool_off = (int64_t*)(ws + L.pool_off);
+    ka.dist = out->dist;
+    ka.dense_P = out->dense_P;
+    ka.dense_off = (const int64_t*)(ws + L.dense_off);
+    ka.logZ = out->logZ;
+}
+
+#define QP_CUDA(x)                                  \
+    do {                                            \
+        if ((x) != cudaSuccess) return QP_ERR_CUDA; \
+    } while (0)
+
+}  // namespace qp
+
+using namespace qp;
+
+extern "C" int qp_last_launch_count(void) { return g_launches; }
+
+extern "C" const char* qp_version(void) { return "qp-b200 0.1 (sm_100a)"; }
+
+extern "C" const char* qp_status_string(int s) {
+    switch (s) {
+        case QP_OK: return "ok";
+        case QP_ERR_INVALID_ARG: return "invalid argument";
+        case QP_ERR_BAD_RESIDUE: return "residue code >= alphabet";
+        case QP_ERR_EMPTY_SEQUENCE: return "empty or over-long sequence";
+        case QP_ERR_BAD_PAIR: return "pair index out of range or x == y";
+        case QP_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+        case QP_ERR_NNZ_CAPACITY: return "nnz capacity exceeded";
+        case QP_ERR_CUDA: return "CUDA runtime error";
+        case QP_ERR_RANGE: return "model weights outside the supported dynamic range";
+        default: return "unknown status";
+    }
+}
+
+extern "C" int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int32_t* h_pairs, int64_t P,
+                                  const qp_params* params, int64_t nnz_capacity, int want_dense, size_t budget_bytes,
+                                  size_t* out_bytes) {
+    if (!h_offsets || (!h_pairs && P > 0) || !out_bytes || k < 0 || P < 0 || nnz_capacity < 0) return QP_ERR_INVALID_ARG;
+    int r = check_params(params);
+    if (r) return r;
+    const bool fp64 = params->precision == QP_FP64;
+    const uint32_t cmask = fp64 ? kMaskF64 : kMaskF32;
+    const int rb = fp64 ? 8 : 4;
+    int sms = kSmAssumed;
+    {
+        int dev;
+        if (cudaGetDevice(&dev) == cudaSuccess) {
+            int v;
+            if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0) sms = v;
+        } else {
+            (void)cudaGetLastError();
+        }
+    }
+    const Layout L = make_layout(P, nnz_capacity, want_dense != 0, total_max_slots(sms));
+    std::vector<std::vector<uint64_t>> sz(kNumClasses);
+    std::vector<uint64_t> sz64;   // fp64 slots of the pairs a refinement pass could see
+    for (int64_t p = 0; p < P; ++p) {
+        const int x = h_pairs[2 * p], y = h_pairs[2 * p + 1];
+        if (x < 0 || y < 0 || x >= k || y >= k || x == y) return QP_ERR_BAD_PAIR;
+        const int64_t n = h_offsets[x + 1] - h_offsets[x], m = h_offsets[y + 1] - h_offsets[y];
+        if (n < 1 || m < 1 || n > QP_MAX_LEN || m > QP_MAX_LEN) return QP_ERR_EMPTY_SEQUENCE;
+        int nb;
+        const int c = choose_class((int)m + 1, cmask, &nb);
+        sz[c].push_back(bin_ub(bin_of((uint64_t)slot_bytes((int)n, 2 * (c + 1), nb, rb))));
+        if (!fp64) {
+            const int c2 = choose_class((int)m + 1, kMaskF64, &nb);
+            sz64.push_back((uint64_t)slot_bytes((int)n, 2 * (c2 + 1), nb, 8));
+        }
+    }
+    uint64_t full = 0, minimum = 0;
+    for (int c = 0; c < kNumClasses; ++c) {
+        std::sort(sz[c].begin(), sz[c].end(), std::greater<uint64_t>());
+        const size_t W = std::min<size_t>(sz[c].size(), (size_t)max_warps(c, fp64, sms));
+        for (size_t w = 0; w < W; ++w) full += sz[c][w];
+        if (!sz[c].empty()) minimum += sz[c][0];
+    }
+    // the refinement pass reuses the slot region: make sure its largest slot fits at least once
+    uint64_t ref_min = 0;
+    for (uint64_t v : sz64) ref_min = std::max(ref_min, v);
+    minimum = std::max(minimum, ref_min);
+    full = std::max(full, minimum);
+    const uint64_t need_min = (uint64_t)L.fixed + minimum, need_full = (uint64_t)L.fixed + full;
+    if (budget_bytes != 0 && budget_bytes < need_min) {
+        *out_bytes = (size_t)need_min;
+        return QP_ERR_WORKSPACE_TOO_SMALL;
+    }
+    *out_bytes = (size_t)((budget_bytes != 0 && budget_bytes < need_full) ? budget_bytes : need_full);
+    return QP_OK;
+}
+
+extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, const int32_t* d_pairs,
+                             int64_t P, const qp_params* params, void* d_workspace, size_t workspace_bytes,
+                             const qp_output* out, void* cuda_stream) {
+    g_launches = 0;
+    if (!out || k < 0 || P < 0 || P > 0x7fffffff) return QP_ERR_INVALID_ARG;
+    int r = check_params(params);
+    if (r) return r;
+    if (!out->pair_row_base || !out->pair_nnz_base || !out->status) return QP_ERR_INVALID_ARG;
+    if (P > 0 && (!d_seqs || !d_offsets || !d_pairs || !d_workspace || !out->row_ptr || !out->dist)) return QP_ERR_INVALID_ARG;
+    if (out->nnz_capacity < 0 || (out->nnz_capacity > 0 && (!out->col_idx || !out->val))) return QP_ERR_INVALID_ARG;
+    if (((uintptr_t)d_workspace & 255) != 0) return QP_ERR_INVALID_ARG;
+    if (!ctx_init()) return QP_ERR_CUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const bool fp64 = params->precision == QP_FP64;
+    const bool dense = out->dense_P != nullptr;
+    const int sms = g_ctx.sms;
+    const Layout L = make_layout(P, out->nnz_capacity, dense, total_max_slots(sms));
+    if ((int64_t)workspace_bytes < L.fixed + 256) return QP_ERR_WORKSPACE_TOO_SMALL;
+    char* ws = (char*)d_workspace;
+    SchedHeader* hdr = (SchedHeader*)(ws + L.hdr);
+    const int64_t avail = (int64_t)workspace_bytes - L.slots;
+
+    QP_CUDA(cudaMemsetAsync(hdr, 0, sizeof(SchedHeader), st));
+    if (P == 0) {
+        QP_CUDA(cudaMemsetAsync(out->pair_row_base, 0, 8, st));
+        QP_CUDA(cudaMemsetAsync(out->pair_nnz_base, 0, 8, st));
+        QP_CUDA(cudaMemsetAsync(out->status, 0, 16, st));
+        if (params->flags & QP_FLAG_SYNC_STATUS) QP_CUDA(cudaStreamSynchronize(st));
+        return QP_OK;
+    }
+    QP_CUDA(cudaMemsetAsync(ws + L.nnz, 0, (size_t)P * 4, st));
+
+    // ---- a0: schedule, entirely on the device --------------------------------------------------------------
+    const uint32_t cmask = fp64 ? kMaskF64 : kMaskF32;
+    const int rb = fp64 ? 8 : 4;
+    const int pb = (int)((P + 255) / 256);
+    k_check_residues<<<2 * sms, 256, 0, st>>>(d_seqs, d_offsets, k, params->hmm.alphabet, hdr);
+    k_classify<<<pb, 256, 0, st>>>(d_offsets, k, d_pairs, P, cmask, rb, (PairInfo*)(ws + L.info),
+                                   (int32_t*)(ws + L.rows1), dense ? (int64_t*)(ws + L.cells) : nullptr, hdr);
+    k_bins<<<1, 32, 0, st>>>(hdr);
+    k_scatter<<<pb, 256, 0, st>>>((const PairInfo*)(ws + L.info), P, (int32_t*)(ws + L.order), hdr);
+    MaxW mw;
+    for (int c = 0; c < kNumClasses; ++c) mw.w[c] = ((cmask >> c) & 1) ? max_warps(c, fp64, sms) : 0;
+    k_slots<<<1, 1024, 0, st>>>((const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), mw, avail,
+                                (int64_t*)(ws + L.slot_off), hdr);
+    k_scan<int32_t><<<1, 1024, 0, st>>>((const int32_t*)(ws + L.rows1), P, out->pair_row_base);
+    g_launches += 6;
+    if (dense) {
+        k_scan<int64_t><<<1, 1024, 0, st>>>((const int64_t*)(ws + L.cells), P, (int64_t*)(ws + L.dense_off));
+        ++g_launches;
+    }
+    QP_CUDA(cudaGetLastError());
+
+    // ---- a1..a7: one persistent kernel per stripe class, forked onto side streams ---------------------------
+    KArgs<float>* ka32 = nullptr;
+    KArgs<double>* ka64 = nullptr;
+    std::vector<char> buf32(sizeof(KArgs<float>)), buf64(sizeof(KArgs<double>));
+    ka32 = new (buf32.data()) KArgs<float>();
+    ka64 = new (buf64.data()) KArgs<double>();
+    const bool refine = !fp64 && !(params->flags & QP_FLAG_NO_REFINE);
+    if (!fp64) {
+        r = fill_kargs<float>(params, *ka32);
+        if (r) return r;
+        fill_common(*ka32, d_seqs, d_pairs, k, ws, L, out, P);
+        ka32->refine_pass = 0;
+        ka32->refine_below = refine ? (float)(params->refine_below > 0.0 ? params->refine_below : 0.25) : -1.0f;
+    }
+    if (fp64 || refine) {
+        r = fill_kargs<double>(params, *ka64);
+        if (r) return r;
+        fill_common(*ka64, d_seqs, d_pairs, k, ws, L, out, P);
+        ka64->refine_pass = fp64 ? 0 : 1;
+        ka64->refine_below = -1.0f;
+    }
+    QP_CUDA(cudaEventRecord(g_ctx.fork, st));
+    for (int c = 0; c < kNumClasses; ++c) {
+        if (!((cmask >> c) & 1)) continue;
+        QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
+        const int grid = sms * ctas_per_sm(2 * (c + 1), fp64);
+        r = fp64 ? launch_class_f64(c, *ka64, grid, g_ctx.st[c])
+                 : launch_class_f32(params->pf.n_ins, c, *ka32, grid, g_ctx.st[c]);
+        if (r) return r;
+        QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
+        QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));
+    }
+
+    // ---- fp64 re-evaluation of the distance of near-identical pairs ----------------
+    if (refine) {
+        MaxW64 mw64;
+        for (int c = 0; c < kNumClasses; ++c) mw64.w[c] = ((kMaskF64 >> c) & 1) ? max_warps(c, true, sms) : 0;
+        k_refine_plan<<<1, 32, 0, st>>>(mw64, avail, hdr);
+        ++g_launches;
+        QP_CUDA(cudaEventRecord(g_ctx.fork, st));
+        for (int c = 0; c < kNumClasses; ++c) {
+            if (!((kMaskF64 >> c) & 1)) continue;
+            QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
+            r = launch_class_f64(c, *ka64, sms * ctas_per_sm(2 * (c + 1), true), g_ctx.st[c]);
+            if (r) return r;
+            QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
+            QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));
+        }
+    }
+
+    // ---- CSR placement in pair order ---------------------------------------------------------------------------
+    k_scan<int32_t><<<1, 1024, 0, st>>>((const int32_t*)(ws + L.nnz), P, out->pair_nnz_base);
+    if (out->nnz_capacity > 0)
+        k_copy_pool<<<(int)((P + 3) / 4), 128, 0, st>>>((const int32_t*)(ws + L.nnz), (const int64_t*)(ws + L.pool_off),
+                                                        out->pair_nnz_base, P, (const int32_t*)(ws + L.pool_col),
+                                                        (const float*)(ws + L.pool_val), out->nnz_capacity,
+                                                        out->col_idx, out->val);
+    k_finish<<<1, 32, 0, st>>>(hdr, out->status);
+    g_launches += 3;
+    QP_CUDA(cudaGetLastError());
+
+    if (params->flags & QP_FLAG_SYNC_STATUS) {
+        int32_t hs[4] = {0, 0, 0, 0};
+        QP_CUDA(cudaMemcpyAsync(hs, out->status, sizeof hs, cudaMemcpyDeviceToHost, st));
+        QP_CUDA(cudaStreamSynchronize(st));
+        return hs[0];
+    }
+    return QP_OK;
+}

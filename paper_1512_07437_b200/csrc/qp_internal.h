@@ -1,0 +1,132 @@
+// qp_internal.h -- data layout shared by the scheduler kernels, the pair kernels and the host API.
+#pragma once
+#include <stdint.h>
+
+#include "qp_lane.h"
+
+namespace qp {
+
+constexpr int kNumClasses = 8;        // stripe widths C = 2,4,...,16 (class c <-> C = 2(c+1))
+constexpr int kWarpsPerCta = 4;
+constexpr int kNumBins = 384;         // size bins: 8 per octave of scratch bytes
+constexpr int kSmAssumed = 148;       // used by the host-only workspace query when no device is visible
+
+#if defined(__CUDACC__)
+#define QP_HD2 __host__ __device__ inline
+#else
+#define QP_HD2 inline
+#endif
+
+// resident CTAs per SM the pair kernels are compiled for (register budget via __launch_bounds__)
+constexpr int ctas_per_sm(int C, bool fp64) {
+    return fp64 ? (C <= 4 ? 3 : 2) : (C <= 8 ? 4 : (C <= 12 ? 3 : 2));
+}
+
+struct alignas(16) PairInfo {
+    int64_t xoff, yoff;   // start of the row / column sequence in d_seqs
+    int32_t n, m;         // rows (first sequence), columns (second sequence)
+    int16_t cls;          // class index, -1 = skipped (invalid pair)
+    int16_t nb;           // column blocks of 32*C columns
+    int32_t bin;          // size bin of its scratch slot
+};
+
+// ---- per-pair scratch slot ---------------------------------------------------------------------------------
+// block b, step t:  [C][32] vec2 (F_hmm, F_pf) | [32] int2 exponents | [32] uint8 kept-entry counts (+pad)
+// after the backward pass consumed the vec2 slots of a (t, lane) they are reused for the kept CSR entries.
+QP_HD2 int64_t step_stride(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes + 256 + 64; }
+QP_HD2 int64_t exps_offset(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes; }
+QP_HD2 int64_t cnts_offset(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes + 256; }
+QP_HD2 int num_steps(int n) { return n + 32; }
+QP_HD2 int64_t bnd_rec_bytes(int real_bytes) { return 12 * (int64_t)real_bytes + 16; }   // see BndRec in qp_pair.cuh
+QP_HD2 int64_t slot_bytes(int n, int C, int nb, int real_bytes) {
+    int64_t b = (int64_t)nb * num_steps(n) * step_stride(C, real_bytes);
+    if (nb > 1) b += 2 * (int64_t)(n + 1) * bnd_rec_bytes(real_bytes);
+    return (b + 255) & ~(int64_t)255;
+}
+
+// choose (C, nb) for m+1 columns among the allowed stripe widths (bit c set <-> C = 2(c+1) available):
+// minimal padded width nb*32*C, ties -> fewer blocks. Returns class index.
+QP_HD2 int choose_class(int cols, uint32_t cmask, int* nb_out) {
+    int best = -1, best_nb = 0;
+    int64_t best_w = 0;
+    for (int c = 0; c < kNumClasses; ++c) {
+        if (!((cmask >> c) & 1)) continue;
+        int C = 2 * (c + 1);
+        int nb = (cols + 32 * C - 1) / (32 * C);
+        int64_t w = (int64_t)nb * 32 * C;
+        if (best < 0 || w < best_w || (w == best_w && nb < best_nb)) {
+            best = c;
+            best_nb = nb;
+            best_w = w;
+        }
+    }
+    *nb_out = best_nb;
+    return best;
+}
+
+// size bins: 8 per octave. bin_of(v) for v >= 16; bin_ub = exclusive upper bound of the bin's range.
+QP_HD2 int bin_of(uint64_t v) {
+    int e = 63;
+    while (e > 3 && !((v >> e) & 1)) --e;
+    int mant = (int)((v >> (e - 3)) & 7);
+    int b = (e - 3) * 8 + mant;
+    return b < kNumBins ? b : kNumBins - 1;
+}
+QP_HD2 uint64_t bin_ub(int b) {
+    int e = b / 8 + 3, mant = b % 8;
+    return (uint64_t)(8 + mant + 1) << (e - 3);
+}
+
+struct SchedHeader {
+    int32_t status[4];                       // mirrors qp_output.status
+    unsigned long long pool_cursor;          // CSR staging pool bump pointer (entries)
+    int32_t cls_count[kNumClasses];          // pairs per class
+    int32_t cls_start[kNumClasses];          // start of the class in order[]
+    int32_t cls_W[kNumClasses];              // resident warps (= scratch slots) granted to the class
+    int32_t cls_slot0[kNumClasses];          // first entry of the class in slot_off[]
+    int32_t cls_cursor[kNumClasses];         // next position in the class's order list
+    int32_t refine_count[kNumClasses];       // pairs queued for fp64 re-evaluation, per fp64 class
+    int32_t refine_cursor[kNumClasses];
+    int32_t refine_W[kNumClasses];
+    unsigned long long refine_slot_bytes[kNumClasses];   // largest fp64 scratch slot among the queued pairs
+    unsigned long long refine_slot0[kNumClasses];        // byte offset of the class's first slot
+    uint32_t hist[kNumClasses][kNumBins];    // pairs per (class, size bin)
+    uint32_t bin_start[kNumClasses][kNumBins];   // position of the bin inside the class, largest bins first
+    uint32_t bin_fill[kNumClasses][kNumBins];
+};
+
+// kernel argument block (passed by value, __grid_constant__)
+template <typename R> struct KArgs {
+    typename Traits<R>::vec2 tab[kTabDim * kTabDim];   // (em_hmm, em_pf)[x*32+y], sentinel row/col zero
+    Weights<R> wh, wp;
+    R tau;
+    int rescale_mask;            // renormalise every (mask+1) steps
+    int32_t k;                   // number of sequences (dist is k x k)
+    int32_t refine_pass;         // 1: process the refine list, write distances only
+    float refine_below;          // fp32 pass: queue pairs whose distance is below this (<=0: never)
+    double lx_h[kTabDim], lx_p[kTabDim];   // insert log-weights (for the logZ constant)
+    const uint8_t* seqs;
+    const int32_t* pairs;        // [P][2]
+    const PairInfo* info;
+    const int32_t* order;
+    SchedHeader* hdr;
+    const int64_t* slot_off;     // byte offset of each slot inside slots
+    char* slots;
+    int32_t* refine_list;        // [kNumClasses][refine_stride] pair indices queued for fp64 re-evaluation
+    int64_t refine_stride;
+    uint32_t refine_cmask;       // stripe widths the fp64 kernels exist for
+    // outputs
+    const int64_t* pair_row_base;
+    int32_t* row_ptr;
+    int32_t* pool_col;
+    float* pool_val;
+    int64_t pool_cap;
+    int32_t* nnz;                // per pair
+    int64_t* pool_off;           // per pair
+    float* dist;
+    float* dense_P;
+    const int64_t* dense_off;
+    double* logZ;
+};
+
+}  // namespace qp

@@ -1,0 +1,6 @@
+// fp32 pair kernels, stripe width C=16 (GP = insert-state pairs of the partition-function model)
+#include "qp_kernel.cuh"
+namespace qp {
+template cudaError_t launch_pair<float, 1, 16>(const KArgs<float>&, int, cudaStream_t);
+template cudaError_t launch_pair<float, 2, 16>(const KArgs<float>&, int, cudaStream_t);
+}

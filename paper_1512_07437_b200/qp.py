@@ -1,0 +1,216 @@
+"""Thin ctypes binding over libqp.so (include/qp.h). Argument marshalling only: every step of the hot path
+(schedule, forward, backward, combine, sparsify, expected accuracy) runs in the CUDA kernels of csrc/.
+
+PyTorch is used for device memory and streams only. There is no CPU fallback: importing this module raises if
+libqp.so has not been built (python -m paper_1512_07437_b200.build), and calling it without a CUDA device fails.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libqp.so")
+
+QP_OK = 0
+ERR = {"INVALID_ARG": -1, "BAD_RESIDUE": -2, "EMPTY_SEQUENCE": -3, "BAD_PAIR": -4, "WORKSPACE_TOO_SMALL": -5,
+       "NNZ_CAPACITY": -6, "CUDA": -7, "RANGE": -8}
+QP_FP32, QP_FP64 = 0, 1
+FLAG_SYNC_STATUS, FLAG_NO_REFINE = 1, 2
+
+EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_last_launch_count", "qp_status_string", "qp_version"]
+
+
+class QpError(RuntimeError):
+    def __init__(self, code, msg=""):
+        self.code = code
+        super().__init__(f"libqp: {status_string(code)} ({code}) {msg}")
+
+
+class _Model(C.Structure):
+    _fields_ = [("n_ins", C.c_int32), ("alphabet", C.c_int32),
+                ("log_match", C.POINTER(C.c_double)), ("log_ins", C.POINTER(C.c_double)),
+                ("t_MM", C.c_double), ("t_MI", C.c_double * 2), ("t_II", C.c_double * 2), ("t_IM", C.c_double * 2),
+                ("init_M", C.c_double), ("init_I", C.c_double * 2), ("end_M", C.c_double), ("end_I", C.c_double * 2)]
+
+
+class _Params(C.Structure):
+    _fields_ = [("hmm", _Model), ("pf", _Model), ("threshold", C.c_double), ("precision", C.c_int32),
+                ("flags", C.c_int32), ("refine_below", C.c_double)]
+
+
+class _Output(C.Structure):
+    _fields_ = [("pair_row_base", C.c_void_p), ("pair_nnz_base", C.c_void_p), ("row_ptr", C.c_void_p),
+                ("col_idx", C.c_void_p), ("val", C.c_void_p), ("nnz_capacity", C.c_int64), ("dist", C.c_void_p),
+                ("dense_P", C.c_void_p), ("logZ", C.c_void_p), ("status", C.c_void_p)]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1512_07437_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    L.qp_workspace_bytes.restype = C.c_int
+    L.qp_workspace_bytes.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.POINTER(_Params), C.c_int64,
+                                     C.c_int, C.c_size_t, C.POINTER(C.c_size_t)]
+    L.qp_posteriors.restype = C.c_int
+    L.qp_posteriors.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.POINTER(_Params),
+                                C.c_void_p, C.c_size_t, C.POINTER(_Output), C.c_void_p]
+    L.qp_last_launch_count.restype = C.c_int
+    L.qp_status_string.restype = C.c_char_p
+    L.qp_status_string.argtypes = [C.c_int]
+    L.qp_version.restype = C.c_char_p
+    return L
+
+
+_lib = _load()
+
+
+def status_string(code: int) -> str:
+    return _lib.qp_status_string(int(code)).decode()
+
+
+def version() -> str:
+    return _lib.qp_version().decode()
+
+
+def last_launch_count() -> int:
+    return int(_lib.qp_last_launch_count())
+
+
+class CParams:
+    """qp_params built from paper_1512_07437_b200.inputs.Params; keeps the host tables alive."""
+
+    def __init__(self, params, precision="fp32", flags=FLAG_SYNC_STATUS, refine_below=0.0):
+        self._keep = []
+        s = _Params()
+        for name in ("hmm", "pf"):
+            m = getattr(params, name)
+            lm = np.ascontiguousarray(m.log_match, dtype=np.float64)
+            li = np.ascontiguousarray(m.log_ins, dtype=np.float64)
+            self._keep += [lm, li]
+            cm = getattr(s, name)
+            cm.n_ins, cm.alphabet = int(m.n_ins), int(m.alphabet)
+            cm.log_match = lm.ctypes.data_as(C.POINTER(C.c_double))
+            cm.log_ins = li.ctypes.data_as(C.POINTER(C.c_double))
+            cm.t_MM, cm.init_M, cm.end_M = float(m.t_MM), float(m.init_M), float(m.end_M)
+            for f in ("t_MI", "t_II", "t_IM", "init_I", "end_I"):
+                arr = getattr(cm, f)
+                for g, v in enumerate(m.padded(f)):
+                    arr[g] = v
+        s.threshold = float(params.threshold)
+        s.precision = QP_FP64 if precision in ("fp64", QP_FP64) else QP_FP32
+        s.flags = int(flags)
+        s.refine_below = float(refine_below)
+        self.s = s
+
+    @property
+    def ref(self):
+        return C.byref(self.s)
+
+
+def workspace_bytes(h_offsets, k, h_pairs, cparams: CParams, nnz_capacity: int, want_dense=False, budget=0) -> int:
+    """qp_workspace_bytes: host-only query (numpy int64 offsets [k+1], int32 pairs [P,2])."""
+    h_offsets = np.ascontiguousarray(h_offsets, dtype=np.int64)
+    h_pairs = np.ascontiguousarray(h_pairs, dtype=np.int32).reshape(-1, 2)
+    out = C.c_size_t(0)
+    r = _lib.qp_workspace_bytes(h_offsets.ctypes.data, int(k), h_pairs.ctypes.data, len(h_pairs), cparams.ref,
+                                int(nnz_capacity), int(bool(want_dense)), int(budget), C.byref(out))
+    if r != QP_OK:
+        raise QpError(r, f"(minimum workspace {out.value} bytes)" if r == ERR["WORKSPACE_TOO_SMALL"] else "")
+    return int(out.value)
+
+
+@dataclass
+class Result:
+    """Device tensors written by qp_posteriors (layout: include/qp.h `qp_output`)."""
+    pair_row_base: object
+    pair_nnz_base: object
+    row_ptr: object
+    col_idx: object
+    val: object
+    dist: object
+    dense_P: object
+    dense_off: object  # host numpy int64 [P+1] (only with want_dense)
+    logZ: object
+    status: object
+    code: int
+    launches: int
+
+    def csr(self, p):
+        """(row_ptr, col, val) of pair p as numpy arrays."""
+        rb = self.pair_row_base[p:p + 2].tolist()
+        nb = self.pair_nnz_base[p:p + 2].tolist()
+        return (self.row_ptr[rb[0]:rb[1]].cpu().numpy(), self.col_idx[nb[0]:nb[1]].cpu().numpy(),
+                self.val[nb[0]:nb[1]].cpu().numpy())
+
+
+def posteriors(d_seqs, d_offsets, k, d_pairs, cparams: CParams, workspace, *, nnz_capacity, h_rows_total,
+               want_dense_cells=0, want_logZ=False, dist=None, stream=None, check=True) -> Result:
+    """qp_posteriors on torch CUDA tensors. `h_rows_total` = sum over pairs of (n_p + 1) (sizes row_ptr);
+    `want_dense_cells` = sum n_p*m_p to also get the dense matrices (tests), 0 otherwise."""
+    import torch
+
+    dev = d_seqs.device
+    P = int(d_pairs.shape[0])
+    i64, i32, f32 = torch.int64, torch.int32, torch.float32
+    o = _Output()
+    t = dict(
+        pair_row_base=torch.empty(P + 1, dtype=i64, device=dev),
+        pair_nnz_base=torch.empty(P + 1, dtype=i64, device=dev),
+        row_ptr=torch.empty(max(int(h_rows_total), 1), dtype=i32, device=dev),
+        col_idx=torch.empty(max(int(nnz_capacity), 1), dtype=i32, device=dev),
+        val=torch.empty(max(int(nnz_capacity), 1), dtype=f32, device=dev),
+        dist=dist if dist is not None else torch.zeros((k, k), dtype=f32, device=dev),
+        dense_P=torch.empty(int(want_dense_cells), dtype=f32, device=dev) if want_dense_cells else None,
+        logZ=torch.empty((P, 4), dtype=torch.float64, device=dev) if want_logZ else None,
+        status=torch.zeros(4, dtype=i32, device=dev),
+    )
+    for name, v in t.items():
+        setattr(o, name, v.data_ptr() if v is not None else None)
+    o.nnz_capacity = int(nnz_capacity)
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    with torch.cuda.device(dev):
+        code = _lib.qp_posteriors(d_seqs.data_ptr(), d_offsets.data_ptr(), int(k), d_pairs.data_ptr(), P,
+                                  cparams.ref, workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                  C.byref(o), C.c_void_p(st.cuda_stream))
+    res = Result(dense_off=None, code=int(code), launches=last_launch_count(), **t)
+    if check and code != QP_OK:
+        raise QpError(code)
+    return res
+
+
+def run_family(family, pairs, params, *, precision="fp32", want_dense=False, want_logZ=False, nnz_capacity=None,
+               refine_below=0.0, flags=FLAG_SYNC_STATUS, device="cuda:0", budget=0, beta_guess=0.08) -> Result:
+    """Convenience: host numpy family + pair list -> upload, size the workspace, call qp_posteriors, and retry
+    once with the exact capacity if the CSR did not fit. Returns device tensors."""
+    import torch
+
+    pairs = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
+    L = family.lengths
+    n, m = L[pairs[:, 0]], L[pairs[:, 1]]
+    cells = int((n * m).sum()) if len(pairs) else 0
+    rows_total = int((n + 1).sum()) if len(pairs) else 0
+    cp = CParams(params, precision=precision, flags=flags, refine_below=refine_below)
+    dev = torch.device(device)
+    d_seqs = torch.from_numpy(np.ascontiguousarray(family.seqs)).to(dev)
+    d_offs = torch.from_numpy(np.ascontiguousarray(family.offsets, dtype=np.int64)).to(dev)
+    d_pairs = torch.from_numpy(pairs).to(dev)
+    cap = int(nnz_capacity) if nnz_capacity is not None else int(beta_guess * cells) + 1024
+    for attempt in range(2):
+        wsb = workspace_bytes(family.offsets, family.k, pairs, cp, cap, want_dense, budget)
+        ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+        res = posteriors(d_seqs, d_offs, family.k, d_pairs, cp, ws, nnz_capacity=cap, h_rows_total=rows_total,
+                         want_dense_cells=cells if want_dense else 0, want_logZ=want_logZ, check=False)
+        if res.code == ERR["NNZ_CAPACITY"] and attempt == 0 and nnz_capacity is None:
+            cap = int(res.pair_nnz_base[-1].item())
+            continue
+        if res.code != QP_OK:
+            raise QpError(res.code)
+        break
+    if want_dense:
+        res.dense_off = np.concatenate([[0], np.cumsum(n.astype(np.int64) * m.astype(np.int64))])
+    return res
