@@ -119,6 +119,17 @@ int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, co
 /* Number of kernels the last qp_posteriors call on this thread launched (bench.py's gpu_launches). */
 int qp_last_launch_count(void);
 
+/*
+ * Phase timing for bench.py's roofline line. qp_set_profile(1) makes later qp_posteriors calls on this thread
+ * record CUDA events on the caller's stream at the phase boundaries (no synchronisation is added). After the
+ * caller has synchronised the stream, qp_get_profile fills ms[0..3] with the device time of the last call:
+ *   ms[0] schedule (a0), ms[1] pair kernels (a1-a7, all stripe classes, fork to join),
+ *   ms[2] fp64 distance refinement, ms[3] CSR placement (scan + copy).
+ * Returns QP_OK, or QP_ERR_INVALID_ARG if no profiled call has completed.
+ */
+void qp_set_profile(int on);
+int qp_get_profile(float ms[4]);
+
 const char* qp_status_string(int status);
 const char* qp_version(void);
 

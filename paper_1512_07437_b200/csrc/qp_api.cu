@@ -263,6 +263,20 @@ __global__ void k_finish(const SchedHeader* h, int32_t* status) {
 // host
 // ------------------------------------------------------------------------------------------------------------
 static thread_local int g_launches = 0;
+static thread_local int g_profile = 0;
+static thread_local bool g_prof_valid = false;
+static thread_local cudaEvent_t g_pev[5];
+static thread_local bool g_pev_ok = false;
+
+static void prof_mark(int i, cudaStream_t st) {
+    if (!g_profile) return;
+    if (!g_pev_ok) {
+        for (int q = 0; q < 5; ++q) cudaEventCreate(&g_pev[q]);
+        g_pev_ok = true;
+    }
+    cudaEventRecord(g_pev[i], st);
+    if (i == 4) g_prof_valid = true;
+}
 
 struct Ctx {   // lazily created side streams so that the per-class kernels overlap their tails
     bool ok = false;
@@ -454,6 +468,18 @@ using namespace qp;
 
 extern "C" int qp_last_launch_count(void) { return g_launches; }
 
+extern "C" void qp_set_profile(int on) {
+    g_profile = on;
+    if (!on) g_prof_valid = false;
+}
+
+extern "C" int qp_get_profile(float ms[4]) {
+    if (!g_prof_valid || !ms) return QP_ERR_INVALID_ARG;
+    for (int q = 0; q < 4; ++q)
+        if (cudaEventElapsedTime(&ms[q], g_pev[q], g_pev[q + 1]) != cudaSuccess) return QP_ERR_CUDA;
+    return QP_OK;
+}
+
 extern "C" const char* qp_version(void) { return "qp-b200 0.1 (sm_100a)"; }
 
 extern "C" const char* qp_status_string(int s) {
@@ -537,12 +563,19 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
     if (!out->pair_row_base || !out->pair_nnz_base || !out->status) return QP_ERR_INVALID_ARG;
     if (P > 0 && (!d_seqs || !d_offsets || !d_pairs || !d_workspace || !out->row_ptr || !out->dist)) return QP_ERR_INVALID_ARG;
     if (out->nnz_capacity < 0 || (out->nnz_capacity > 0 && (!out->col_idx || !out->val))) return QP_ERR_INVALID_ARG;
-    if (((uintptr_t)d_workspace & 255) != 0) return QP_ERR_INVALID_ARG;
+    if (P > 0 && ((uintptr_t)d_workspace & 255) != 0) return QP_ERR_INVALID_ARG;
     if (!ctx_init()) return QP_ERR_CUDA;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const bool fp64 = params->precision == QP_FP64;
     const bool dense = out->dense_P != nullptr;
     const int sms = g_ctx.sms;
+    if (P == 0) {   // nothing to do: empty prefixes, status ok; the workspace is not touched
+        QP_CUDA(cudaMemsetAsync(out->pair_row_base, 0, 8, st));
+        QP_CUDA(cudaMemsetAsync(out->pair_nnz_base, 0, 8, st));
+        QP_CUDA(cudaMemsetAsync(out->status, 0, 16, st));
+        if (params->flags & QP_FLAG_SYNC_STATUS) QP_CUDA(cudaStreamSynchronize(st));
+        return QP_OK;
+    }
     const Layout L = make_layout(P, out->nnz_capacity, dense, total_max_slots(sms));
     if ((int64_t)workspace_bytes < L.fixed + 256) return QP_ERR_WORKSPACE_TOO_SMALL;
     char* ws = (char*)d_workspace;
@@ -550,13 +583,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
     const int64_t avail = (int64_t)workspace_bytes - L.slots;
 
     QP_CUDA(cudaMemsetAsync(hdr, 0, sizeof(SchedHeader), st));
-    if (P == 0) {
-        QP_CUDA(cudaMemsetAsync(out->pair_row_base, 0, 8, st));
-        QP_CUDA(cudaMemsetAsync(out->pair_nnz_base, 0, 8, st));
-        QP_CUDA(cudaMemsetAsync(out->status, 0, 16, st));
-        if (params->flags & QP_FLAG_SYNC_STATUS) QP_CUDA(cudaStreamSynchronize(st));
-        return QP_OK;
-    }
+    prof_mark(0, st);
     QP_CUDA(cudaMemsetAsync(ws + L.nnz, 0, (size_t)P * 4, st));
 
     // ---- a0: schedule, entirely on the device --------------------------------------------------------------
@@ -601,6 +628,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
         ka64->refine_pass = fp64 ? 0 : 1;
         ka64->refine_below = -1.0f;
     }
+    prof_mark(1, st);
     QP_CUDA(cudaEventRecord(g_ctx.fork, st));
     for (int c = 0; c < kNumClasses; ++c) {
         if (!((cmask >> c) & 1)) continue;
@@ -612,6 +640,8 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
         QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
         QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));
     }
+
+    prof_mark(2, st);
 
     // ---- fp64 re-evaluation of the distance of near-identical pairs ----------------
     if (refine) {
@@ -630,6 +660,8 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
         }
     }
 
+    prof_mark(3, st);
+
     // ---- CSR placement in pair order ---------------------------------------------------------------------------
     k_scan<int32_t><<<1, 1024, 0, st>>>((const int32_t*)(ws + L.nnz), P, out->pair_nnz_base);
     if (out->nnz_capacity > 0)
@@ -639,6 +671,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
                                                         out->col_idx, out->val);
     k_finish<<<1, 32, 0, st>>>(hdr, out->status);
     g_launches += 3;
+    prof_mark(4, st);
     QP_CUDA(cudaGetLastError());
 
     if (params->flags & QP_FLAG_SYNC_STATUS) {

@@ -19,7 +19,7 @@ constexpr int kSmAssumed = 148;       // used by the host-only workspace query w
 
 // resident CTAs per SM the pair kernels are compiled for (register budget via __launch_bounds__)
 constexpr int ctas_per_sm(int C, bool fp64) {
-    return fp64 ? (C <= 4 ? 3 : 2) : (C <= 8 ? 4 : (C <= 12 ? 3 : 2));
+    return fp64 ? (C <= 4 ? 3 : 2) : (C <= 6 ? 4 : (C <= 10 ? 3 : 2));
 }
 
 struct alignas(16) PairInfo {

