@@ -1,0 +1,395 @@
+#!/usr/bin/env python
+"""bench.py -- posterior DP cells/s of the all-pairs posterior stage (BASELINE.json `metric`) on N GPUs of one node.
+
+A "step" = one pass of the whole hot path (schedule, pair-HMM + partition-function forward/backward, combine,
+sparsify to CSR, expected-accuracy distance: SURVEY.md 8(a) a0-a7) over ALL pairs of one synthetic family.
+Default workload = BASELINE.json configs[3] (1,000 sequences, mean length 350, all 499,500 pairs), the largest
+single-GPU configuration and one of the two target configs; --config picks another.
+
+    python bench.py --gpus 1 --steps 5 --warmup 3
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+    python bench.py --impl reference ...     # the oracle (CPU, fp64) on a bounded sample: a baseline, not the target
+
+Prints ONE JSON line (rank 0). Inputs are seeded synthetic families (paper_1512_07437_b200.inputs); the paper's
+benchmark families are not available.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "posterior DP cells/sec (fwd+bwd, both models, combine+sparsify+MEA)"
+UNIT = "cells/s"
+ALGO_BYTES_PER_CELL = 16.0     # fp32 F_M of both models written in forward, read back in backward
+SFU_OPS_PER_CELL = 43.0        # canonical log-space transcendental count (context only)
+SFU_PEAK = 148 * 16 * 1.965e9  # SURVEY.md 8(d) nominal MUFU rate
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic(cfg):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture, if one exists for this config."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p)).get(f"cfg{cfg}")
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks + throttle reasons every 200 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                self.rows.append([c.strip() for c in out.strip().split(",")])
+            except Exception:
+                pass
+            time.sleep(0.2)
+
+    def summary(self):
+        sm = [int(r[0]) for r in self.rows if len(r) >= 6 and r[0].isdigit()]
+        mx = [int(r[1]) for r in self.rows if len(r) >= 6 and r[1].isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 6 for i in range(4) if r[2 + i].lower() == "active"})
+        return {"sm_mhz": int(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(sm)}
+
+
+def oracle_sample(fam, pairs, prm, target_cells, seed, threads=0):
+    """Oracle (as it stands) on a seeded sample of pairs holding about target_cells cells. Returns (cells, seconds, threads)."""
+    from oracle import qp_oracle as orc
+    L = fam.lengths
+    cells = L[pairs[:, 0]].astype(np.int64) * L[pairs[:, 1]].astype(np.int64)
+    order = np.random.default_rng(seed).permutation(len(pairs))
+    cum = np.cumsum(cells[order])
+    take = order[: max(1, int(np.searchsorted(cum, target_cells)) + 1)]
+    run = orc.Run(prm, fam, pairs[take], threads=threads)
+    return int(cells[take].sum()), float(run.seconds), int(run.threads), len(take)
+
+
+def run_reference(args):
+    """--impl reference: the fp64 CPU oracle on the same config/metric, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1512_07437_b200 import inputs
+    prm = inputs.default_params()
+    fam = inputs.config_family(args.config)
+    pairs = inputs.all_pairs(fam.k)
+    cores = os.cpu_count() or 1
+    budget_s = 90.0 / max(1, args.steps + args.warmup)              # whole run ~1.5 min of CPU time
+    target = 0.9e6 * cores * budget_s                                # ~0.9e6 cells/s/core measured for this oracle
+    for w in range(args.warmup):
+        oracle_sample(fam, pairs, prm, target, seed=1000 + w)
+    tot_cells, tot_s, threads, npairs = 0, 0.0, cores, 0
+    for s in range(args.steps):
+        c, sec, threads, npair = oracle_sample(fam, pairs, prm, target, seed=2000 + s)
+        tot_cells, tot_s, npairs = tot_cells + c, tot_s + sec, npairs + npair
+    val = tot_cells / tot_s
+    sample = f"{npairs // max(1, args.steps)} seeded random pairs per step (~{target:.2e} cells) of cfg{args.config}"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot_s / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config, fam, pairs), "note": "CPU oracle on a bounded sample per step"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg, fam, pairs):
+    L = fam.lengths
+    return (f"BASELINE.json configs[{cfg}]: {fam.k} synthetic proteins (seed {7437000 + cfg}), lengths "
+            f"{int(L.min())}-{int(L.max())} (mean {L.mean():.0f}), all {len(pairs)} pairs")
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as td
+    from paper_1512_07437_b200 import inputs, multi, qp
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        td.init_process_group("nccl", device_id=dev)
+
+    prm = inputs.default_params()
+    # N > 1, default ("weak"): the paper's bulk mode -- every rank takes one whole family of the
+    # same configuration (rank r: the same recipe with seed + 1000 r), independent problems, no collective.
+    # --shard-one-family ("strong"): ONE family, its pair list sharded over the ranks by balanced cell count,
+    # and the one real exchange of the path, the k x k distance matrix, all-reduced over NCCL every step.
+    shard = bool(args.shard_one_family) and world > 1
+    if world > 1 and not shard:
+        c = inputs._CONFIGS[args.config]
+        fam = inputs.gen_family(c["k"], c["law"], c["r_sub"], c["r_indel"], seed=inputs.SEED_BASE + args.config + 1000 * rank,
+                                tree=c["tree"], name=f"cfg{args.config}-rank{rank}")
+    else:
+        fam = inputs.config_family(args.config)
+    all_pairs = inputs.all_pairs(fam.k)
+    L = fam.lengths
+    mine = multi.shard_pairs(all_pairs, L, world, rank) if shard else np.arange(len(all_pairs))
+    pairs = np.ascontiguousarray(all_pairs[mine])
+    n, m = L[pairs[:, 0]].astype(np.int64), L[pairs[:, 1]].astype(np.int64)
+    my_cells, rows_total = int((n * m).sum()), int((n + 1).sum())
+    total_cells = my_cells
+    if world > 1:
+        t = torch.tensor([my_cells], dtype=torch.int64, device=dev)
+        td.all_reduce(t)
+        total_cells = int(t.item())
+
+    # ---- device-resident inputs, outputs and workspace (allocated once, reused every step) -------------------
+    d_seqs = torch.from_numpy(np.ascontiguousarray(fam.seqs)).to(dev)
+    d_offs = torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev)
+    d_pairs = torch.from_numpy(pairs).to(dev)
+    cp_async = qp.CParams(prm, flags=0)
+    cap = int(0.05 * my_cells) + 4096
+    dist = torch.zeros((fam.k, fam.k), dtype=torch.float32, device=dev)
+
+    def alloc(cap_):
+        wsb = qp.workspace_bytes(fam.offsets, fam.k, pairs, cp_async, cap_)
+        return torch.empty(wsb, dtype=torch.uint8, device=dev)
+
+    ws = alloc(cap)
+    res = qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp_async, ws, nnz_capacity=cap, h_rows_total=rows_total,
+                        dist=dist, check=False)
+    torch.cuda.synchronize()
+    code = int(res.status[0].item())
+    if code not in (0, qp.ERR["NNZ_CAPACITY"]):
+        raise qp.QpError(code)
+    # size the CSR exactly (plus slack) from the first pass: frees ~1/3 of the over-allocated memory
+    cap = int(res.pair_nnz_base[-1].item()) + 1024
+    del ws, res
+    torch.cuda.empty_cache()
+    ws = alloc(cap)
+    out_kw = dict(nnz_capacity=cap, h_rows_total=rows_total, dist=dist, check=False)
+
+    state = {"res": None}
+
+    def step():
+        r = qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp_async, ws, reuse=state["res"], **out_kw)
+        state["res"] = r
+        if shard:
+            # the one exchange of the path: every rank's distance entries (disjoint supports) summed over NCCL
+            # (on a copy: the next step rewrites this rank's own entries of `dist` in place)
+            multi.exchange_distances(r.dist.clone())
+        return r
+
+    for _ in range(max(args.warmup, 3)):
+        res = step()
+    torch.cuda.synchronize()
+    assert int(res.status[0].item()) == 0, qp.status_string(int(res.status[0].item()))
+    nnz = int(res.pair_nnz_base[-1].item())
+    launches_per_step = res.launches
+
+    # ---- timed region: K steps, CUDA events on the launching stream, barrier + sync on both sides -----------
+    sampler = ClockSampler(local)
+    qp.set_profile(True)
+    if world > 1:
+        td.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        res = step()
+    e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        td.barrier()
+    sampler.stop_flag = True
+    ms_total = e0.elapsed_time(e1)
+    prof = qp.get_profile()            # device ms of the phases of the LAST timed step (events recorded inside the region)
+    qp.set_profile(False)
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        td.all_reduce(t, op=td.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = total_cells / (ms_step * 1e-3)
+    sampler.join(timeout=2)
+    clocks = sampler.summary()
+
+    line = None
+    if rank == 0:
+        hbm_peak, peak_src = peaks()
+        kern_s = prof["pair_kernels"] * 1e-3
+        achieved = ALGO_BYTES_PER_CELL * my_cells / kern_s / 1e9
+        roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+                    "traffic": ncu_traffic(args.config), "peak_source": peak_src,
+                    "kernel": "qp::pair_kernel<float,1,C> (8 stripe-width instances, fork..join)",
+                    "kernel_ms": prof["pair_kernels"], "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
+                    "phases_ms": {k: round(v, 3) for k, v in prof.items()},
+                    "canonical_sfu_roofline": {"ops_per_cell": SFU_OPS_PER_CELL, "peak_ops_s": SFU_PEAK,
+                                               "frac": SFU_OPS_PER_CELL * my_cells / kern_s / SFU_PEAK,
+                                               "note": "north_star's log-space transcendental bound; this path is "
+                                                       "linear-space block floating point and issues 1 MUFU per cell"}}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+                "scaling": "strong" if shard else "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": workload_name(args.config, fam, all_pairs), "cells": total_cells,
+                           "threshold": prm.threshold, "nnz": nnz if world == 1 else None,
+                           "beta": nnz / my_cells, "all_pairs_wall_ms": ms_step,
+                           "l2": "per-step scratch traffic (16 B/cell) is far larger than the 126 MB L2",
+                           "parallelism": (f"one family, pairs sharded over {world} GPUs, one distance all-reduce per step"
+                                           if shard else f"{world} independent famil{'y' if world == 1 else 'ies'} (bulk mode), "
+                                           "one per GPU, no collective")},
+                "roofline": roofline, "clocks": clocks, "gpu_launches": launches_per_step * args.steps}
+
+    # ---- end to end through the public call with HOST buffers (pinned): H2D of the inputs, D2H of every output --
+    if world == 1 and not args.no_e2e:
+        e2e = run_e2e(args, fam, pairs, prm, qp, dev, my_cells)
+        line["e2e"] = e2e
+    elif rank == 0:
+        line["e2e"] = None
+
+    # ---- oracle beside it (rank 0, N=1): bounded sample on the host cores -------------------------------------
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cores = os.cpu_count() or 1
+        c, sec, threads, npair = oracle_sample(fam, all_pairs, prm, 0.9e6 * cores * 20.0, seed=7437)
+        line["cpu_baseline"] = {"value": c / sec, "unit": UNIT, "cores": threads, "kind": "oracle",
+                                "sample": f"{npair} seeded random pairs ({c:.3e} cells) of the same workload, {sec:.1f} s"}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        td.destroy_process_group()
+
+
+def run_e2e(args, fam, pairs, prm, qp, dev, my_cells):
+    """Same metric through qp_posteriors with host buffers: every step copies sequences/offsets/pairs from pinned
+    host memory, runs the call (synchronising status), and copies the distance matrix and the whole CSR back to
+    pinned host memory. Pairs are streamed in batches (BASELINE.json configs[3]: "memory-budgeted by streaming
+    pair batches") so that the pinned staging buffers stay bounded."""
+    import torch
+    L = fam.lengths
+    n, m = L[pairs[:, 0]].astype(np.int64), L[pairs[:, 1]].astype(np.int64)
+    cells = n * m
+    target = 6.0e9                                  # cells per batch -> ~2.5e8 nnz -> ~2 GB of CSR per batch
+    bounds = [0]
+    acc = 0
+    for p in range(len(pairs)):
+        acc += int(cells[p])
+        if acc >= target:
+            bounds.append(p + 1)
+            acc = 0
+    if bounds[-1] != len(pairs):
+        bounds.append(len(pairs))
+    nb = len(bounds) - 1
+    max_cells = max(int(cells[bounds[b]:bounds[b + 1]].sum()) for b in range(nb))
+    max_rows = max(int((n[bounds[b]:bounds[b + 1]] + 1).sum()) for b in range(nb))
+    max_pairs = max(bounds[b + 1] - bounds[b] for b in range(nb))
+    cap = int(0.05 * max_cells) + 4096
+    cp = qp.CParams(prm, flags=qp.FLAG_SYNC_STATUS)
+    h_seqs = torch.from_numpy(np.ascontiguousarray(fam.seqs)).pin_memory()
+    h_offs = torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).pin_memory()
+    h_pairs = torch.from_numpy(pairs).pin_memory()
+    # pinned result buffers (reused by every batch; a consumer would read them before the next batch lands)
+    h_col = torch.empty(cap, dtype=torch.int32).pin_memory()
+    h_val = torch.empty(cap, dtype=torch.float32).pin_memory()
+    h_rp = torch.empty(max_rows, dtype=torch.int32).pin_memory()
+    h_rb = torch.empty(max_pairs + 1, dtype=torch.int64).pin_memory()
+    h_nb = torch.empty(max_pairs + 1, dtype=torch.int64).pin_memory()
+    h_dist = torch.empty((fam.k, fam.k), dtype=torch.float32).pin_memory()
+    wsb = max(qp.workspace_bytes(fam.offsets, fam.k, pairs[bounds[b]:bounds[b + 1]], cp, cap) for b in range(nb))
+    ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+    dist = torch.zeros((fam.k, fam.k), dtype=torch.float32, device=dev)
+    h2d = d2h = 0
+
+    def one_step(count):
+        nonlocal h2d, d2h
+        d_seqs = h_seqs.to(dev, non_blocking=True)
+        d_offs = h_offs.to(dev, non_blocking=True)
+        if count:
+            h2d += h_seqs.numel() + 8 * h_offs.numel()
+        for b in range(nb):
+            lo, hi = bounds[b], bounds[b + 1]
+            d_pairs = h_pairs[lo:hi].to(dev, non_blocking=True)
+            rows = int((n[lo:hi] + 1).sum())
+            r = qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp, ws, nnz_capacity=cap, h_rows_total=rows, dist=dist,
+                              check=True)
+            h_nb[: hi - lo + 1].copy_(r.pair_nnz_base, non_blocking=True)
+            h_rb[: hi - lo + 1].copy_(r.pair_row_base, non_blocking=True)
+            h_rp[:rows].copy_(r.row_ptr[:rows], non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+            nz = int(h_nb[hi - lo].item())
+            h_col[:nz].copy_(r.col_idx[:nz], non_blocking=True)
+            h_val[:nz].copy_(r.val[:nz], non_blocking=True)
+            if count:
+                h2d += 8 * (hi - lo)
+                d2h += 16 * (hi - lo + 1) + 4 * rows + 8 * nz
+        h_dist.copy_(dist, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        if count:
+            d2h += 4 * fam.k * fam.k
+
+    one_step(False)   # warm-up
+    torch.cuda.synchronize()
+    steps = max(1, min(args.steps, 3))
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        one_step(True)
+    e1.record()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    return {"value": my_cells * steps / wall, "unit": UNIT, "h2d_bytes_per_step": h2d // steps,
+            "d2h_bytes_per_step": d2h // steps, "ms_per_step": 1e3 * wall / steps, "steps": steps, "batches": nb,
+            "note": "host wall clock around H2D + qp_posteriors(sync) + D2H of distances and the full CSR"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (0-4)")
+    ap.add_argument("--shard-one-family", action="store_true",
+                    help="N>1: shard ONE family's pair list over the ranks (strong scaling, NCCL all-reduce of distances)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -129,6 +129,9 @@ int qp_last_launch_count(void);
  */
 void qp_set_profile(int on);
 int qp_get_profile(float ms[4]);
+/* Per stripe class (C = 2(c+1)): start and stop of its pair kernel in ms after the end of the schedule phase,
+ * -1 for classes that did not run. Same preconditions as qp_get_profile. */
+int qp_get_profile_classes(float start_ms[8], float stop_ms[8]);
 
 const char* qp_status_string(int status);
 const char* qp_version(void);

@@ -266,12 +266,18 @@ static thread_local int g_launches = 0;
 static thread_local int g_profile = 0;
 static thread_local bool g_prof_valid = false;
 static thread_local cudaEvent_t g_pev[5];
+static thread_local cudaEvent_t g_cev[2 * kNumClasses];   // per stripe class: start / stop on its side stream
 static thread_local bool g_pev_ok = false;
+
+static void prof_class(int c, int which, cudaStream_t st) {
+    if (g_profile && g_pev_ok) cudaEventRecord(g_cev[2 * c + which], st);
+}
 
 static void prof_mark(int i, cudaStream_t st) {
     if (!g_profile) return;
     if (!g_pev_ok) {
         for (int q = 0; q < 5; ++q) cudaEventCreate(&g_pev[q]);
+        for (int q = 0; q < 2 * kNumClasses; ++q) cudaEventCreate(&g_cev[q]);
         g_pev_ok = true;
     }
     cudaEventRecord(g_pev[i], st);
@@ -473,6 +479,20 @@ extern "C" void qp_set_profile(int on) {
     if (!on) g_prof_valid = false;
 }
 
+extern "C" int qp_get_profile_classes(float start_ms[8], float stop_ms[8]) {
+    if (!g_prof_valid || !start_ms || !stop_ms) return QP_ERR_INVALID_ARG;
+    for (int c = 0; c < kNumClasses; ++c) {
+        start_ms[c] = stop_ms[c] = -1.0f;
+        if (cudaEventQuery(g_cev[2 * c]) != cudaSuccess) { (void)cudaGetLastError(); continue; }
+        if (cudaEventElapsedTime(&start_ms[c], g_pev[1], g_cev[2 * c]) != cudaSuccess ||
+            cudaEventElapsedTime(&stop_ms[c], g_pev[1], g_cev[2 * c + 1]) != cudaSuccess) {
+            (void)cudaGetLastError();
+            start_ms[c] = stop_ms[c] = -1.0f;
+        }
+    }
+    return QP_OK;
+}
+
 extern "C" int qp_get_profile(float ms[4]) {
     if (!g_prof_valid || !ms) return QP_ERR_INVALID_ARG;
     for (int q = 0; q < 4; ++q)
@@ -634,9 +654,11 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
         if (!((cmask >> c) & 1)) continue;
         QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
         const int grid = sms * ctas_per_sm(2 * (c + 1), fp64);
+        prof_class(c, 0, g_ctx.st[c]);
         r = fp64 ? launch_class_f64(c, *ka64, grid, g_ctx.st[c])
                  : launch_class_f32(params->pf.n_ins, c, *ka32, grid, g_ctx.st[c]);
         if (r) return r;
+        prof_class(c, 1, g_ctx.st[c]);
         QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
         QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));
     }

@@ -87,8 +87,8 @@ QP_HD int expo(double v) {
 }
 QP_HD float qfma(float a, float b, float c) { return fmaf(a, b, c); }
 QP_HD double qfma(double a, double b, double c) { return fma(a, b, c); }
-QP_HD float qmax(float a, float b) { return a > b ? a : b; }
-QP_HD double qmax(double a, double b) { return a > b ? a : b; }
+QP_HD float qmax(float a, float b) { return fmaxf(a, b); }
+QP_HD double qmax(double a, double b) { return fmax(a, b); }
 QP_HD int imax(int a, int b) { return a > b ? a : b; }
 
 // linear-space weights of one model; unused insert slots are 0
@@ -197,7 +197,7 @@ template <typename R, int G, int C> struct FwdModel {
 #pragma unroll
         for (int g = 0; g < G; ++g) {
             R X = Xn[g][k];
-            R Y = qfma(w.wMI[g], run.Ml, w.wII[g] * run.Yl[g]);
+            R Y = qfma(w.wII[g], run.Yl[g], w.wMI[g] * run.Ml);   // the row chain runs through one FMA only
             if (SPECIAL && sp.start && k == 1) Y = w.initI[g];      // Y_g(0,1) = init_I[g]
             R xy = X + Y;
             acc = g == 0 ? w.wIM[g] * xy : qfma(w.wIM[g], xy, acc);
@@ -321,7 +321,7 @@ template <typename R, int G, int C> struct BwdModel {
             acc = g == 0 ? w.wMI[g] * s : qfma(w.wMI[g], s, acc);
             if (SPECIAL) zacc = qfma(w.initI[g], s, zacc);
             BXn[g][k] = qfma(w.wIM[g], T, w.wII[g] * bx);
-            run.BYr[g] = qfma(w.wIM[g], T, w.wII[g] * run.BYr[g]);
+            run.BYr[g] = qfma(w.wII[g], run.BYr[g], w.wIM[g] * T);   // row chain: one FMA per cell
         }
         R BM = qfma(w.wMM, T, acc);
         if (SPECIAL && sp.end && k == sp.kz) {                        // cell (n,m): B_s(n,m) = end_s

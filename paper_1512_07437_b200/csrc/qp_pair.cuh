@@ -69,6 +69,15 @@ struct alignas(8) Entry {   // a kept posterior, parked in the consumed forward 
     int32_t k;              // column offset inside the lane's stripe
 };
 
+// park a kept entry without a branch (predicated 8-byte store)
+__device__ __forceinline__ void st_entry_if(void* ptr, float val, int k, bool keep) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %3, 0;\n\t@p st.global.v2.b32 [%0], {%1, %2};\n\t}"
+        :
+        : "l"(ptr), "r"(__float_as_int(val)), "r"(k), "r"((int)keep)
+        : "memory");
+}
+
 __device__ __forceinline__ int warp_sum(int v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(kFull, v, o);
@@ -273,21 +282,28 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         BwdBnd<R, GP>* bout = (BwdBnd<R, GP>*)((b & 1) ? bnd1 : bnd0);
         const int jbase = b * 32 * C + lane * C;
         int xnext = xcode_at(tstart - lane);
+        // F values and exponents of a step are loaded one step ahead (at the end of the previous iteration)
+        V2 Fv[C];
+        int2 eF;
+        auto load_step = [&](int t2) {
+            const int i2 = t2 - lane;
+            const bool act2 = (i2 >= 0) && (i2 <= n);
+            const char* stp2 = blk + (int64_t)t2 * stride;
+            const V2* in2 = (const V2*)stp2;
+#pragma unroll
+            for (int k = 0; k < C; ++k) {
+                if (act2) Fv[k] = in2[(C - 1 - k) * 32 + lane];
+                else { Fv[k].x = R(0); Fv[k].y = R(0); }
+            }
+            eF = act2 ? *(const int2*)(stp2 + exps_offset(C, RB) + lane * 8) : make_int2(0, 0);
+        };
+        load_step(tstart);
         for (int t = tstart; t >= 0; --t) {
             const int i = t - lane;
             const bool active = (i >= 0) && (i <= n);
             const int xcode = xnext;
             xnext = xcode_at(i - 1);
             char* stp = blk + (int64_t)t * stride;
-            const V2* in = (const V2*)stp;
-            V2 Fv[C];
-            int2 eF = make_int2(0, 0);
-#pragma unroll
-            for (int k = 0; k < C; ++k) {
-                if (active) Fv[k] = in[(C - 1 - k) * 32 + lane];
-                else { Fv[k].x = R(0); Fv[k].y = R(0); }
-            }
-            if (active) eF = *(const int2*)(stp + exps_offset(C, RB) + lane * 8);
             BwdEx<R, GH> rh = shfl_dn_ex(H.ex);
             BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex);
             Acc rA = shfl_dn1(exA);
@@ -312,14 +328,13 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             PScale<R> psh, psp;
             psh.set(eF.x + H.e - ez_h, invZh);
             psp.set(eF.y + Pm.e - ez_p, invZp);
-            Acc Adiag = Adin, Aright = rA;
-            int cnt = 0;
             const bool special = (last && t == tstart) || (b == 0 && t == 0);   // warp-uniform
             BwdSpecial sp;
             sp.end = special && (last && lane == lz && i == n);
             sp.capture = special && (b == 0 && lane == 0 && i == 0);
             sp.kz = kz;
-            auto body = [&](auto SPEC, int k) {
+            // loop 1: the two backward recurrences; F(i,j) is replaced in place by the model posteriors
+            auto rec_body = [&](auto SPEC, int k) {
                 constexpr bool S = decltype(SPEC)::value;
                 V2 em = row[ycode[k]];
                 R zh = R(0), zp = R(0);
@@ -331,10 +346,24 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     ezb_h = H.e;
                     ezb_p = Pm.e;
                 }
-                R ph = psh.apply(Fv[k].x, bmh);
-                R pp = psp.apply(Fv[k].y, bmp);
-                R P = combine_rms(ph, pp);
-                Acc q = quantise(P, mea_scale);
+                Fv[k].x = psh.apply(Fv[k].x, bmh);
+                Fv[k].y = psp.apply(Fv[k].y, bmp);
+            };
+            if (special) {
+#pragma unroll
+                for (int k = C - 1; k >= 0; --k) rec_body(std::true_type{}, k);
+            } else {
+#pragma unroll
+                for (int k = C - 1; k >= 0; --k) rec_body(std::false_type{}, k);
+            }
+            // loop 2: combine, expected-accuracy max-plus, threshold + parking of kept entries
+            Acc Adiag = Adin, Aright = rA;
+            int cnt = 0;
+            char* park = stp + (int64_t)lane * sizeof(V2);
+#pragma unroll
+            for (int k = C - 1; k >= 0; --k) {
+                const R P = combine_rms(Fv[k].x, Fv[k].y);
+                const Acc q = quantise(P, mea_scale);
                 Acc a = Adiag + q;
                 a = a > An[k] ? a : An[k];
                 a = a > Aright ? a : Aright;
@@ -342,24 +371,15 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                 An[k] = a;
                 Aright = a;
                 if (want_csr) {
-                    if (P >= ka.tau) {
-                        Entry en;
-                        en.val = (float)P;
-                        en.k = k;
-                        *(Entry*)(stp + ((int64_t)cnt * 32 + lane) * sizeof(V2)) = en;
-                        ++cnt;
-                    }
+                    const bool keep = P >= ka.tau;
+                    st_entry_if(park, (float)P, k, keep);
+                    park += keep ? 32 * (int)sizeof(V2) : 0;
+                    cnt += keep ? 1 : 0;
                     if (dense != nullptr && i >= 1 && i <= n && ((jvalid >> k) & 1))
                         dense[(int64_t)(i - 1) * m + (jbase + k - 1)] = (float)P;
                 }
-            };
-            if (special) {
-#pragma unroll
-                for (int k = C - 1; k >= 0; --k) body(std::true_type{}, k);
-            } else {
-#pragma unroll
-                for (int k = C - 1; k >= 0; --k) body(std::false_type{}, k);
             }
+            if (t > 0) load_step(t - 1);
             H.end(runH);
             Pm.end(runP);
             exA = An[0];
@@ -439,45 +459,91 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         int running = 0;
         // Segments (row i, block b) in row-major order, SEG at a time so that the loads of a batch are
         // independent: (1) the SEG count bytes, (2) SEG warp scans, (3) e-th entry of every segment, stores.
-        constexpr int SEG = 8;
-        const int nseg = n * nb;
+        constexpr int SEGM = 8;    // multi-block batch
         const int32_t colbase = lane * C - 1;
-        for (int s0 = 0; s0 < nseg; s0 += SEG) {
-            int cn[SEG], st[SEG];
-            const char* sp[SEG];
-            int32_t jb[SEG];
+        if (nb == 1) {
+            constexpr int SEG = 8;   // rows per batch (larger batches cost registers in the DP loops: measured slower)
+            const char* base = slot + (int64_t)(1 + lane) * stride;          // row 1
+            const char* cbase = base + cnts_offset(C, RB) + lane;
+            const bool lane_in = colbase < m;                                 // lane owns at least one real column
+            int cnx[SEG];   // counts of the NEXT batch, loaded while the current one is compacted
 #pragma unroll
-            for (int u = 0; u < SEG; ++u) {
-                const int sg = s0 + u;
-                const int i = 1 + sg / nb, b = sg - (i - 1) * nb;
-                jb[u] = b * 32 * C + colbase;
-                sp[u] = slot + (int64_t)b * blk_bytes + (int64_t)(i + lane) * stride;
-                cn[u] = (sg < nseg && jb[u] < m) ? (int)*(const uint8_t*)(sp[u] + cnts_offset(C, RB) + lane) : 0;
+            for (int u = 0; u < SEG; ++u) cnx[u] = (lane_in && u < n) ? (int)*(const uint8_t*)(cbase + (int64_t)u * stride) : 0;
+            for (int r0 = 0; r0 < n; r0 += SEG) {
+                int cn[SEG], st[SEG];
+#pragma unroll
+                for (int u = 0; u < SEG; ++u) {
+                    cn[u] = cnx[u];
+                    const int rn = r0 + SEG + u;
+                    cnx[u] = (lane_in && rn < n) ? (int)*(const uint8_t*)(cbase + (int64_t)rn * stride) : 0;
+                }
+                int maxc = 0;
+#pragma unroll
+                for (int u = 0; u < SEG; ++u) {
+                    if (lane == 0 && r0 + u < n) rp[r0 + u] = running;
+                    const int ex = warp_excl_scan(cn[u], lane);
+                    st[u] = running + ex + cn[u] - 1;   // destination of this lane's FIRST parked entry (highest column)
+                    running += __shfl_sync(kFull, ex + cn[u], 31);
+                    maxc = cn[u] > maxc ? cn[u] : maxc;
+                }
+                if (ok) {
+                    maxc = __reduce_max_sync(kFull, maxc);
+                    const char* eb = base + (int64_t)r0 * stride + (int64_t)lane * sizeof(V2);
+                    for (int e = 0; e < maxc; ++e) {
+                        Entry en[SEG];
+#pragma unroll
+                        for (int u = 0; u < SEG; ++u)
+                            if (e < cn[u]) en[u] = *(const Entry*)(eb + (int64_t)u * stride + (int64_t)e * 32 * sizeof(V2));
+#pragma unroll
+                        for (int u = 0; u < SEG; ++u)
+                            if (e < cn[u]) {
+                                const long long dst = (long long)poff + st[u] - e;
+                                ka.pool_col[dst] = colbase + en[u].k;
+                                ka.pool_val[dst] = en[u].val;
+                            }
+                    }
+                }
             }
-            int maxc = 0;
+        } else {
+            // segments (row i, block b) in row-major order
+            const int nseg = n * nb;
+            for (int s0 = 0; s0 < nseg; s0 += SEGM) {
+                int cn[SEGM], st[SEGM];
+                const char* sp[SEGM];
+                int32_t jb[SEGM];
 #pragma unroll
-            for (int u = 0; u < SEG; ++u) {
-                const int sg = s0 + u;
-                if (lane == 0 && sg < nseg && sg % nb == 0) rp[sg / nb] = running;
-                const int ex = warp_excl_scan(cn[u], lane);
-                st[u] = running + ex + cn[u] - 1;      // destination of this lane's FIRST parked entry (highest column)
-                running += __shfl_sync(kFull, ex + cn[u], 31);
-                maxc = cn[u] > maxc ? cn[u] : maxc;
-            }
-            if (ok) {
-                maxc = __reduce_max_sync(kFull, maxc);
-                for (int e = 0; e < maxc; ++e) {
-                    Entry en[SEG];
+                for (int u = 0; u < SEGM; ++u) {
+                    const int sg = s0 + u;
+                    const int i = 1 + sg / nb, b = sg - (i - 1) * nb;
+                    jb[u] = b * 32 * C + colbase;
+                    sp[u] = slot + (int64_t)b * blk_bytes + (int64_t)(i + lane) * stride;
+                    cn[u] = (sg < nseg && jb[u] < m) ? (int)*(const uint8_t*)(sp[u] + cnts_offset(C, RB) + lane) : 0;
+                }
+                int maxc = 0;
 #pragma unroll
-                    for (int u = 0; u < SEG; ++u)
-                        if (e < cn[u]) en[u] = *(const Entry*)(sp[u] + ((int64_t)e * 32 + lane) * sizeof(V2));
+                for (int u = 0; u < SEGM; ++u) {
+                    const int sg = s0 + u;
+                    if (lane == 0 && sg < nseg && sg % nb == 0) rp[sg / nb] = running;
+                    const int ex = warp_excl_scan(cn[u], lane);
+                    st[u] = running + ex + cn[u] - 1;
+                    running += __shfl_sync(kFull, ex + cn[u], 31);
+                    maxc = cn[u] > maxc ? cn[u] : maxc;
+                }
+                if (ok) {
+                    maxc = __reduce_max_sync(kFull, maxc);
+                    for (int e = 0; e < maxc; ++e) {
+                        Entry en[SEGM];
 #pragma unroll
-                    for (int u = 0; u < SEG; ++u)
-                        if (e < cn[u]) {
-                            const long long dst = (long long)poff + st[u] - e;
-                            ka.pool_col[dst] = jb[u] + en[u].k;
-                            ka.pool_val[dst] = en[u].val;
-                        }
+                        for (int u = 0; u < SEGM; ++u)
+                            if (e < cn[u]) en[u] = *(const Entry*)(sp[u] + ((int64_t)e * 32 + lane) * sizeof(V2));
+#pragma unroll
+                        for (int u = 0; u < SEGM; ++u)
+                            if (e < cn[u]) {
+                                const long long dst = (long long)poff + st[u] - e;
+                                ka.pool_col[dst] = jb[u] + en[u].k;
+                                ka.pool_val[dst] = en[u].val;
+                            }
+                    }
                 }
             }
         }

@@ -22,7 +22,7 @@ QP_FP32, QP_FP64 = 0, 1
 FLAG_SYNC_STATUS, FLAG_NO_REFINE = 1, 2
 
 EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_last_launch_count", "qp_status_string", "qp_version",
-           "qp_set_profile", "qp_get_profile"]
+           "qp_set_profile", "qp_get_profile", "qp_get_profile_classes"]
 
 
 class QpError(RuntimeError):
@@ -68,6 +68,8 @@ def _load():
     L.qp_set_profile.argtypes = [C.c_int]
     L.qp_get_profile.restype = C.c_int
     L.qp_get_profile.argtypes = [C.POINTER(C.c_float)]
+    L.qp_get_profile_classes.restype = C.c_int
+    L.qp_get_profile_classes.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]
     return L
 
 
@@ -97,6 +99,15 @@ def get_profile():
     if r != QP_OK:
         raise QpError(r)
     return dict(schedule=ms[0], pair_kernels=ms[1], refine=ms[2], csr_place=ms[3])
+
+
+def get_profile_classes():
+    """[(C, start_ms, stop_ms)] of the stripe-class kernels of the last profiled call (relative to the fork)."""
+    a, b = (C.c_float * 8)(), (C.c_float * 8)()
+    r = _lib.qp_get_profile_classes(a, b)
+    if r != QP_OK:
+        raise QpError(r)
+    return [(2 * (c + 1), round(a[c], 3), round(b[c], 3)) for c in range(8) if a[c] >= 0]
 
 
 class CParams:
@@ -167,9 +178,10 @@ class Result:
 
 
 def posteriors(d_seqs, d_offsets, k, d_pairs, cparams: CParams, workspace, *, nnz_capacity, h_rows_total,
-               want_dense_cells=0, want_logZ=False, dist=None, stream=None, check=True) -> Result:
+               want_dense_cells=0, want_logZ=False, dist=None, stream=None, check=True, reuse=None) -> Result:
     """qp_posteriors on torch CUDA tensors. `h_rows_total` = sum over pairs of (n_p + 1) (sizes row_ptr);
-    `want_dense_cells` = sum n_p*m_p to also get the dense matrices (tests), 0 otherwise."""
+    `want_dense_cells` = sum n_p*m_p to also get the dense matrices (tests), 0 otherwise. `reuse` = a previous
+    Result of the same shapes whose output tensors are written again instead of allocating new ones."""
     import torch
 
     dev = d_seqs.device
@@ -177,6 +189,10 @@ def posteriors(d_seqs, d_offsets, k, d_pairs, cparams: CParams, workspace, *, nn
     i64, i32, f32 = torch.int64, torch.int32, torch.float32
     o = _Output()
     t = dict(
+        pair_row_base=reuse.pair_row_base, pair_nnz_base=reuse.pair_nnz_base, row_ptr=reuse.row_ptr,
+        col_idx=reuse.col_idx, val=reuse.val, dist=reuse.dist, dense_P=reuse.dense_P, logZ=reuse.logZ,
+        status=reuse.status,
+    ) if reuse is not None else dict(
         pair_row_base=torch.empty(P + 1, dtype=i64, device=dev),
         pair_nnz_base=torch.empty(P + 1, dtype=i64, device=dev),
         row_ptr=torch.empty(max(int(h_rows_total), 1), dtype=i32, device=dev),
