@@ -23,12 +23,16 @@
 
 namespace qp {
 
-template <typename R, int GP, int C> cudaError_t launch_pair(const KArgs<R>& ka, int grid, cudaStream_t st);
-#define QP_DECL_F32(C)                                                                          \
-    extern template cudaError_t launch_pair<float, 1, C>(const KArgs<float>&, int, cudaStream_t); \
-    extern template cudaError_t launch_pair<float, 2, C>(const KArgs<float>&, int, cudaStream_t);
-#define QP_DECL_F64(C) \
-    extern template cudaError_t launch_pair<double, 2, C>(const KArgs<double>&, int, cudaStream_t);
+enum : int { kModeCsr = 0, kModeFull = 1, kModeDist = 2 };   // see qp_pair.cuh
+template <typename R, int GP, int C, int MODE> cudaError_t launch_pair(const KArgs<R>& ka, int grid, cudaStream_t st);
+#define QP_DECL_F32(C)                                                                                      \
+    extern template cudaError_t launch_pair<float, 1, C, kModeCsr>(const KArgs<float>&, int, cudaStream_t);  \
+    extern template cudaError_t launch_pair<float, 2, C, kModeCsr>(const KArgs<float>&, int, cudaStream_t);  \
+    extern template cudaError_t launch_pair<float, 1, C, kModeFull>(const KArgs<float>&, int, cudaStream_t); \
+    extern template cudaError_t launch_pair<float, 2, C, kModeFull>(const KArgs<float>&, int, cudaStream_t);
+#define QP_DECL_F64(C)                                                                                        \
+    extern template cudaError_t launch_pair<double, 2, C, kModeFull>(const KArgs<double>&, int, cudaStream_t); \
+    extern template cudaError_t launch_pair<double, 2, C, kModeDist>(const KArgs<double>&, int, cudaStream_t);
 QP_DECL_F32(2) QP_DECL_F32(4) QP_DECL_F32(6) QP_DECL_F32(8) QP_DECL_F32(10) QP_DECL_F32(12) QP_DECL_F32(14) QP_DECL_F32(16)
 QP_DECL_F64(2) QP_DECL_F64(4) QP_DECL_F64(6) QP_DECL_F64(8)
 
@@ -414,25 +418,26 @@ template <typename R> static int fill_kargs(const qp_params* prm, KArgs<R>& ka) 
     return QP_OK;
 }
 
-static int launch_class_f32(int gp, int cls, const KArgs<float>& ka, int grid, cudaStream_t st) {
+static int launch_class_f32(int gp, bool full, int cls, const KArgs<float>& ka, int grid, cudaStream_t st) {
     cudaError_t e = cudaErrorInvalidValue;
-#define QP_CASE(C)                                                                      \
-    case C / 2 - 1:                                                                     \
-        e = gp == 1 ? launch_pair<float, 1, C>(ka, grid, st) : launch_pair<float, 2, C>(ka, grid, st); \
+#define QP_CASE(C)                                                                                            \
+    case C / 2 - 1:                                                                                           \
+        if (full) e = gp == 1 ? launch_pair<float, 1, C, kModeFull>(ka, grid, st) : launch_pair<float, 2, C, kModeFull>(ka, grid, st); \
+        else e = gp == 1 ? launch_pair<float, 1, C, kModeCsr>(ka, grid, st) : launch_pair<float, 2, C, kModeCsr>(ka, grid, st);        \
         break;
     switch (cls) { QP_CASE(2) QP_CASE(4) QP_CASE(6) QP_CASE(8) QP_CASE(10) QP_CASE(12) QP_CASE(14) QP_CASE(16) }
 #undef QP_CASE
     ++g_launches;
     return e == cudaSuccess ? QP_OK : QP_ERR_CUDA;
 }
-static int launch_class_f64(int cls, const KArgs<double>& ka, int grid, cudaStream_t st) {
+static int launch_class_f64(bool dist_only, int cls, const KArgs<double>& ka, int grid, cudaStream_t st) {
     cudaError_t e = cudaErrorInvalidValue;
-    switch (cls) {
-        case 0: e = launch_pair<double, 2, 2>(ka, grid, st); break;
-        case 1: e = launch_pair<double, 2, 4>(ka, grid, st); break;
-        case 2: e = launch_pair<double, 2, 6>(ka, grid, st); break;
-        case 3: e = launch_pair<double, 2, 8>(ka, grid, st); break;
-    }
+#define QP_CASE(C)                                                                                                  \
+    case C / 2 - 1:                                                                                                 \
+        e = dist_only ? launch_pair<double, 2, C, kModeDist>(ka, grid, st) : launch_pair<double, 2, C, kModeFull>(ka, grid, st); \
+        break;
+    switch (cls) { QP_CASE(2) QP_CASE(4) QP_CASE(6) QP_CASE(8) }
+#undef QP_CASE
     ++g_launches;
     return e == cudaSuccess ? QP_OK : QP_ERR_CUDA;
 }
@@ -634,6 +639,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
     ka32 = new (buf32.data()) KArgs<float>();
     ka64 = new (buf64.data()) KArgs<double>();
     const bool refine = !fp64 && !(params->flags & QP_FLAG_NO_REFINE);
+    const bool full_outputs = out->dense_P != nullptr || out->logZ != nullptr;   // test outputs: separate kernel instances
     if (!fp64) {
         r = fill_kargs<float>(params, *ka32);
         if (r) return r;
@@ -655,8 +661,8 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
         QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
         const int grid = sms * ctas_per_sm(2 * (c + 1), fp64);
         prof_class(c, 0, g_ctx.st[c]);
-        r = fp64 ? launch_class_f64(c, *ka64, grid, g_ctx.st[c])
-                 : launch_class_f32(params->pf.n_ins, c, *ka32, grid, g_ctx.st[c]);
+        r = fp64 ? launch_class_f64(false, c, *ka64, grid, g_ctx.st[c])
+                 : launch_class_f32(params->pf.n_ins, full_outputs, c, *ka32, grid, g_ctx.st[c]);
         if (r) return r;
         prof_class(c, 1, g_ctx.st[c]);
         QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
@@ -675,7 +681,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
         for (int c = 0; c < kNumClasses; ++c) {
             if (!((kMaskF64 >> c) & 1)) continue;
             QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
-            r = launch_class_f64(c, *ka64, sms * ctas_per_sm(2 * (c + 1), true), g_ctx.st[c]);
+            r = launch_class_f64(true, c, *ka64, sms * ctas_per_sm(2 * (c + 1), true), g_ctx.st[c]);
             if (r) return r;
             QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
             QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));

@@ -12,9 +12,9 @@ constexpr int kNumBins = 384;         // size bins: 8 per octave of scratch byte
 constexpr int kSmAssumed = 148;       // used by the host-only workspace query when no device is visible
 
 #if defined(__CUDACC__)
-#define QP_HD2 __host__ __device__ inline
+#define QP_HD2 __host__ __device__ constexpr inline
 #else
-#define QP_HD2 inline
+#define QP_HD2 constexpr inline
 #endif
 
 // resident CTAs per SM the pair kernels are compiled for (register budget via __launch_bounds__)
@@ -31,11 +31,13 @@ struct alignas(16) PairInfo {
 };
 
 // ---- per-pair scratch slot ---------------------------------------------------------------------------------
-// block b, step t:  [C][32] vec2 (F_hmm, F_pf) | [32] int2 exponents | [32] uint8 kept-entry counts (+pad)
-// after the backward pass consumed the vec2 slots of a (t, lane) they are reused for the kept CSR entries.
-QP_HD2 int64_t step_stride(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes + 256 + 64; }
+// block b, step t:  F planes | [32] int2 exponents (e_hmm, e_pf), one per lane
+//   fp32: [C/2][32] float4 = (F_hmm, F_pf) of the lane's columns 2u and 2u+1  (every warp access is 512 B contiguous)
+//   fp64: [C][32] double2  = (F_hmm, F_pf) of the lane's column k
+// The backward pass reuses a consumed (step, lane): a kept posterior is parked as a float in the F_hmm word of
+// its own cell, and the lane's bit mask of kept cells replaces e_hmm. Sparsification adds no scratch.
+QP_HD2 int64_t step_stride(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes + 256; }
 QP_HD2 int64_t exps_offset(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes; }
-QP_HD2 int64_t cnts_offset(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes + 256; }
 QP_HD2 int num_steps(int n) { return n + 32; }
 QP_HD2 int64_t bnd_rec_bytes(int real_bytes) { return 12 * (int64_t)real_bytes + 16; }   // see BndRec in qp_pair.cuh
 QP_HD2 int64_t slot_bytes(int n, int C, int nb, int real_bytes) {

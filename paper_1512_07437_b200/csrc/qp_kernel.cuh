@@ -5,7 +5,7 @@
 
 namespace qp {
 
-template <typename R, int GP, int C>
+template <typename R, int GP, int C, int MODE>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, ctas_per_sm(C, sizeof(R) == 8))
 pair_kernel(const __grid_constant__ KArgs<R> ka) {
     using V2 = typename Traits<R>::vec2;
@@ -37,14 +37,14 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
     }
     int idx = gw;   // the first W pairs of the (largest-first) list go to warps 0..W-1; the rest are pulled
     while (idx < count) {
-        process_pair<R, GP, C>(ka, tab, list[idx], slot, lane);
+        process_pair<R, GP, C, MODE>(ka, tab, list[idx], slot, lane);
         if (lane == 0) idx = atomicAdd(cursor, 1);
         idx = __shfl_sync(kFull, idx, 0);
     }
 }
 
-template <typename R, int GP, int C> cudaError_t launch_pair(const KArgs<R>& ka, int grid, cudaStream_t st) {
-    pair_kernel<R, GP, C><<<grid, kWarpsPerCta * 32, 0, st>>>(ka);
+template <typename R, int GP, int C, int MODE> cudaError_t launch_pair(const KArgs<R>& ka, int grid, cudaStream_t st) {
+    pair_kernel<R, GP, C, MODE><<<grid, kWarpsPerCta * 32, 0, st>>>(ka);
     return cudaGetLastError();
 }
 

@@ -106,6 +106,7 @@ template <typename R, int G> struct FwdEx {   // a lane's last column of the row
 };
 template <typename R, int G> struct FwdRun {  // values carried along a row
     R Sdiag, Ml, Yl[G];
+    R mwl[G];        // wMI[g] * M(i, j-1): shared by X_g(i+1, j-1) and Y_g(i, j)
 };
 struct FwdSpecial {      // which injections/captures apply to this lane in a SPECIAL step
     bool start;          // lane holds cell (0,0) and is at row 0: inject init weights at k=0 / k=1
@@ -133,7 +134,7 @@ template <typename R, int G, int C> struct FwdModel {
     }
 
     // start of a step: optional renormalisation (incoming-aware), then bring the neighbour's values to own scale
-    QP_HD void begin(const FwdEx<R, G>& rin, bool rescale_now, FwdRun<R, G>& run, int& range_flag) {
+    QP_HD void begin(const FwdEx<R, G>& rin, bool rescale_now, FwdRun<R, G>& run, const Weights<R>& w, int& range_flag) {
         if (rescale_now) {
             R mo = Sdin;
             R mi = qmax(rin.S, rin.M);
@@ -186,6 +187,8 @@ template <typename R, int G, int C> struct FwdModel {
             for (int g = 0; g < G; ++g) run.Yl[g] = rin.Y[g] * f1 * f2;
             Sdin = rin.S * f1 * f2;
         }
+#pragma unroll
+        for (int g = 0; g < G; ++g) run.mwl[g] = w.wMI[g] * run.Ml;
     }
 
     // one cell; returns M(i,j) (at exponent e). SPECIAL adds the start injection / Z capture.
@@ -197,12 +200,14 @@ template <typename R, int G, int C> struct FwdModel {
 #pragma unroll
         for (int g = 0; g < G; ++g) {
             R X = Xn[g][k];
-            R Y = qfma(w.wII[g], run.Yl[g], w.wMI[g] * run.Ml);   // the row chain runs through one FMA only
+            R Y = qfma(w.wII[g], run.Yl[g], run.mwl[g]);            // the row chain runs through one FMA only
             if (SPECIAL && sp.start && k == 1) Y = w.initI[g];      // Y_g(0,1) = init_I[g]
             R xy = X + Y;
             acc = g == 0 ? w.wIM[g] * xy : qfma(w.wIM[g], xy, acc);
             if (SPECIAL) zacc = qfma(w.endI[g], xy, zacc);
-            Xn[g][k] = qfma(w.wMI[g], M, w.wII[g] * X);
+            const R mw = w.wMI[g] * M;                              // used by X_g(i+1,j) now and Y_g(i,j+1) next
+            Xn[g][k] = qfma(w.wII[g], X, mw);
+            run.mwl[g] = mw;
             run.Yl[g] = Y;
         }
         R Sn = qfma(w.wMM, M, acc);   // small terms first, dominant term last: one rounding at full magnitude
@@ -320,8 +325,9 @@ template <typename R, int G, int C> struct BwdModel {
             R s = bx + run.BYr[g];
             acc = g == 0 ? w.wMI[g] * s : qfma(w.wMI[g], s, acc);
             if (SPECIAL) zacc = qfma(w.initI[g], s, zacc);
-            BXn[g][k] = qfma(w.wIM[g], T, w.wII[g] * bx);
-            run.BYr[g] = qfma(w.wII[g], run.BYr[g], w.wIM[g] * T);   // row chain: one FMA per cell
+            const R tw = w.wIM[g] * T;                               // enters both BX_g(i,j) and BY_g(i,j)
+            BXn[g][k] = qfma(w.wII[g], bx, tw);
+            run.BYr[g] = qfma(w.wII[g], run.BYr[g], tw);             // row chain: one FMA per cell
         }
         R BM = qfma(w.wMM, T, acc);
         if (SPECIAL && sp.end && k == sp.kz) {                        // cell (n,m): B_s(n,m) = end_s
@@ -349,18 +355,24 @@ template <typename R, int G, int C> struct BwdModel {
 // ---------------------------------------------------------------------------------------------------------
 // combine + MEA quantisation
 // ---------------------------------------------------------------------------------------------------------
-// P_model = F*B*2^(eF+eB-eZ)/Zm, split in two power-of-two factors so no intermediate can overflow
+// P_model * sqrt(1/2) = (F*B) * c with c = 2^(eF+eB-eZ) * sqrt(1/2)/Zm. The product F*B of two mantissas cannot
+// overflow (each stays below 2^57 between renormalisations) and 0 * c is 0, so no NaN can arise. It can underflow
+// before it is scaled back only if E is large and positive; a probability never needs that (maxF*maxB <= Z/r with
+// r the smallest ratio of B inside one lane stripe), so E > kMaxE is reported as a range
+// error by the caller instead of being computed inexactly.
 template <typename R> struct PScale {
-    R s1, s2;
-    QP_HD void set(int E, R invZm) {
-        const int lim = 2 * Traits<R>::kMaxShift - 8;
-        E = E > lim ? lim : (E < -lim ? -lim : E);
-        int a = E >> 1;
-        s1 = pow2i(a, R(0));
-        s2 = pow2i(E - a, R(0)) * invZm;
+    static constexpr int kMaxE = sizeof(R) == 4 ? 64 : 512;
+    R c;
+    QP_HD bool set(int E, R invZr) {
+        const bool bad = E > kMaxE;
+        E = E > kMaxE ? kMaxE : E;
+        c = pow2i(E, R(0)) * invZr;   // pow2i clamps below: 2^E -> 0, the posterior is 0 to working precision
+        return bad;
     }
-    QP_HD R apply(R F, R B) const { return (F * s1) * (B * s2); }
+    QP_HD R apply(R F, R B) const { return (F * B) * c; }
 };
+// 1/Zm with the sqrt(1/2) of the root mean square folded in
+template <typename R> QP_HD R inv_z_rms(R Zm) { return R(0.70710678118654752440) / Zm; }
 
 QP_HD float qsqrt(float v) {
 #if defined(__CUDA_ARCH__)
@@ -373,8 +385,8 @@ QP_HD float qsqrt(float v) {
 }
 QP_HD double qsqrt(double v) { return sqrt(v); }
 
-// P = sqrt((P_hmm^2 + P_pf^2)/2)
-template <typename R> QP_HD R combine_rms(R ph, R pp) { return qsqrt(R(0.5) * qfma(ph, ph, pp * pp)); }
+// P = sqrt((P_hmm^2 + P_pf^2)/2); the arguments already carry the factor sqrt(1/2) (PScale)
+template <typename R> QP_HD R combine_rms(R ph, R pp) { return qsqrt(qfma(ph, ph, pp * pp)); }
 
 // MEA fixed point: q = round(P * 2^s). fp32: magic-constant rounding (valid while P*2^s < 2^22)
 QP_HD int32_t quantise(float p, float scale) {

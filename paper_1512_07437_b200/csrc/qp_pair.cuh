@@ -4,6 +4,12 @@
 //   warp-scan compaction of the kept entries into CSR         8(a) a6
 // Lane arithmetic lives in qp_lane.h; this file owns the wavefront (who processes which row when), the warp
 // shuffles that hand row boundaries to the neighbouring lane, and all global-memory traffic.
+//
+// MODE selects what a kernel instance writes, at compile time, so that the per-cell code carries no test for an
+// output that is not wanted:
+//   kModeCsr   CSR + distance                       (production)
+//   kModeFull  CSR + distance + optional dense_P and logZ (tests)
+//   kModeDist  distance only                        (fp64 re-evaluation of near-identical pairs)
 #pragma once
 #include <cuda_runtime.h>
 
@@ -12,6 +18,8 @@
 #include "qp_internal.h"
 
 namespace qp {
+
+enum : int { kModeCsr = 0, kModeFull = 1, kModeDist = 2 };
 
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -40,17 +48,18 @@ template <typename R, int G> __device__ __forceinline__ BwdEx<R, G> shfl_dn_ex(c
     r.e = shfl_dn1(a.e);
     return r;
 }
-template <typename R, int G> __device__ __forceinline__ void zero_ex(FwdEx<R, G>& a) {
+// "nothing comes in": zero values at the receiving lane's own exponent (so that no rescaling is triggered)
+template <typename R, int G> __device__ __forceinline__ void zero_ex(FwdEx<R, G>& a, int e) {
     a.S = a.M = R(0);
 #pragma unroll
     for (int g = 0; g < G; ++g) a.Y[g] = R(0);
-    a.e = 0;
+    a.e = e;
 }
-template <typename R, int G> __device__ __forceinline__ void zero_ex(BwdEx<R, G>& a) {
+template <typename R, int G> __device__ __forceinline__ void zero_ex(BwdEx<R, G>& a, int e) {
     a.TL = R(0);
 #pragma unroll
     for (int g = 0; g < G; ++g) a.BY[g] = R(0);
-    a.e = 0;
+    a.e = e;
 }
 
 // boundary column handed from one 32*C-column block to the next (multi-block pairs only), one record per row
@@ -63,20 +72,6 @@ template <typename R, int GP> struct BwdBnd {
     BwdEx<R, GP> p;
     typename Traits<R>::acc_t A;
 };
-
-struct alignas(8) Entry {   // a kept posterior, parked in the consumed forward slot of its (step, lane)
-    float val;
-    int32_t k;              // column offset inside the lane's stripe
-};
-
-// park a kept entry without a branch (predicated 8-byte store)
-__device__ __forceinline__ void st_entry_if(void* ptr, float val, int k, bool keep) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %3, 0;\n\t@p st.global.v2.b32 [%0], {%1, %2};\n\t}"
-        :
-        : "l"(ptr), "r"(__float_as_int(val)), "r"(k), "r"((int)keep)
-        : "memory");
-}
 
 __device__ __forceinline__ int warp_sum(int v) {
 #pragma unroll
@@ -107,27 +102,89 @@ template <typename T> __device__ __forceinline__ T ld_volatile(const T* p) {
     return r;
 }
 
+// ---- scratch addressing of one (step, lane): see qp_internal.h for the layout ------------------------------
+// `lp` points at the lane's first F word of the step: step base + lane * kLaneBytes.
+template <typename R> struct Slot;
+template <> struct Slot<float> {
+    static constexpr int kLaneBytes = 16;                                         // one float4 = two cells
+    static __device__ __forceinline__ int cell_off(int k) { return (k >> 1) * 512 + (k & 1) * 8; }
+};
+template <> struct Slot<double> {
+    static constexpr int kLaneBytes = 16;                                         // one double2 = one cell
+    static __device__ __forceinline__ int cell_off(int k) { return k * 512; }
+};
+// byte distance from `lp` to the lane's int2 exponent record of the same step
+template <typename R, int C> __device__ __forceinline__ int exps_delta(int lane) {
+    return (int)exps_offset(C, (int)sizeof(R)) + lane * 8 - lane * Slot<R>::kLaneBytes;
+}
+
+// F planes of one lane-step in registers
+template <typename R, int C> struct FRegs;
+template <int C> struct FRegs<float, C> {
+    float4 v[C / 2];
+    __device__ __forceinline__ void load(const char* lp, int u) { v[u] = *(const float4*)(lp + u * 512); }
+    __device__ __forceinline__ float h(int k) const { return (k & 1) ? v[k >> 1].z : v[k >> 1].x; }
+    __device__ __forceinline__ float p(int k) const { return (k & 1) ? v[k >> 1].w : v[k >> 1].y; }
+    __device__ __forceinline__ void kill(bool keep) {
+#pragma unroll
+        for (int u = 0; u < C / 2; ++u) {
+            v[u].x = keep ? v[u].x : 0.f; v[u].y = keep ? v[u].y : 0.f;
+            v[u].z = keep ? v[u].z : 0.f; v[u].w = keep ? v[u].w : 0.f;
+        }
+    }
+    // the unit holding cell k can be reloaded once both of its cells are consumed (columns are walked downwards)
+    static __device__ __forceinline__ bool unit_done(int k) { return (k & 1) == 0; }
+    static __device__ __forceinline__ int unit_of(int k) { return k >> 1; }
+    static constexpr int kUnits = C / 2;
+};
+template <int C> struct FRegs<double, C> {
+    double2 v[C];
+    __device__ __forceinline__ void load(const char* lp, int u) { v[u] = *(const double2*)(lp + u * 512); }
+    __device__ __forceinline__ double h(int k) const { return v[k].x; }
+    __device__ __forceinline__ double p(int k) const { return v[k].y; }
+    __device__ __forceinline__ void kill(bool keep) {
+#pragma unroll
+        for (int u = 0; u < C; ++u) { v[u].x = keep ? v[u].x : 0.0; v[u].y = keep ? v[u].y : 0.0; }
+    }
+    static __device__ __forceinline__ bool unit_done(int) { return true; }
+    static __device__ __forceinline__ int unit_of(int k) { return k; }
+    static constexpr int kUnits = C;
+};
+
+// park a kept posterior in the F_hmm word of its own (consumed) cell: predicated 4-byte store, no branch
+__device__ __forceinline__ void st_f32_if(void* ptr, float val, bool keep) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %2, 0;\n\t@p st.global.b32 [%0], %1;\n\t}"
+        :
+        : "l"(ptr), "r"(__float_as_int(val)), "r"((int)keep)
+        : "memory");
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // the pair pipeline
 // ---------------------------------------------------------------------------------------------------------
-template <typename R, int GP, int C>
+template <typename R, int GP, int C, int MODE>
 __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2* __restrict__ tab, int p, char* slot,
                              int lane) {
     using V2 = typename Traits<R>::vec2;
     using Acc = typename Traits<R>::acc_t;
+    using SL = Slot<R>;
     constexpr int RB = (int)sizeof(R);
     constexpr int GH = 2;
+    constexpr bool kCsr = MODE != kModeDist;
+    static_assert(C % 2 == 0, "stripe widths are even (fp32 stores two cells per 16-byte word)");
 
     const PairInfo pi = ka.info[p];
     const int n = pi.n, m = pi.m;
     const int nb = (m + 1 + 32 * C - 1) / (32 * C);   // column blocks (column 0 included)
     const uint8_t* __restrict__ xs = ka.seqs + pi.xoff;
     const uint8_t* __restrict__ ys = ka.seqs + pi.yoff;
-    const int64_t stride = step_stride(C, RB);
+    constexpr int stride = (int)step_stride(C, RB);
     const int64_t blk_bytes = (int64_t)num_steps(n) * stride;
     const int cols_last = (m + 1) - (nb - 1) * 32 * C;   // columns (incl. column 0) that fall in the last block
     const int lz = (cols_last - 1) / C, kz = (cols_last - 1) % C;   // lane / stripe offset of column m
     const int mask = ka.rescale_mask;
+    const int dE = exps_delta<R, C>(lane);
     char* bnd0 = slot + (int64_t)nb * blk_bytes;
     char* bnd1 = bnd0 + (int64_t)(n + 1) * bnd_rec_bytes(RB);
     int range_flag = 0;
@@ -147,15 +204,15 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             int j = b * 32 * C + lane * C + k;
             ycode[k] = (j >= 1 && j <= m) ? (int)ys[j - 1] : kSentinel;
         }
-        char* blk = slot + (int64_t)b * blk_bytes;
         const bool last = (b == nb - 1);
         const int tend = n + (last ? lz : 31);
         const FwdBnd<R, GP>* bin = (const FwdBnd<R, GP>*)((b & 1) ? bnd0 : bnd1);   // written by block b-1
         FwdBnd<R, GP>* bout = (FwdBnd<R, GP>*)((b & 1) ? bnd1 : bnd0);
+        char* lp = slot + (int64_t)b * blk_bytes + lane * SL::kLaneBytes;   // this lane's F words of step t
         int xnext = xcode_at(0 - lane);   // residue code of the row of the NEXT step, loaded one step ahead
-        for (int t = 0; t <= tend; ++t) {
+        for (int t = 0; t <= tend; ++t, lp += stride) {
             const int i = t - lane;
-            const bool active = (i >= 0) && (i <= n);
+            const bool active = (unsigned)i <= (unsigned)n;
             const int xcode = xnext;
             xnext = xcode_at(i + 1);
             FwdEx<R, GH> rh = shfl_up_ex(H.ex);
@@ -166,50 +223,48 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     rh = rec.h;
                     rp = rec.p;
                 } else {
-                    zero_ex(rh);
-                    zero_ex(rp);
+                    zero_ex(rh, H.e);
+                    zero_ex(rp, Pm.e);
                 }
             }
             const bool resc = ((t & mask) == 0) || (i == 0);   // periodic, and on the lane's first row
             const V2* row = tab + xcode * kTabDim;
-            V2* out = (V2*)(blk + (int64_t)t * stride);
             FwdRun<R, GH> runH;
             FwdRun<R, GP> runP;
-            H.begin(rh, resc, runH, range_flag);
-            Pm.begin(rp, resc, runP, range_flag);
+            H.begin(rh, resc, runH, ka.wh, range_flag);
+            Pm.begin(rp, resc, runP, ka.wp, range_flag);
             const bool special = (b == 0 && t == 0) || (last && t == tend);   // warp-uniform
-            if (special) {
-                FwdSpecial sp;
-                sp.start = (b == 0 && lane == 0 && i == 0);
-                sp.capture = (last && lane == lz && i == n);
-                sp.kz = kz;
+            FwdSpecial sp;
+            sp.start = special && (b == 0 && lane == 0 && i == 0);
+            sp.capture = special && (last && lane == lz && i == n);
+            sp.kz = kz;
+            auto body = [&](auto SPEC) {
+                constexpr bool S = decltype(SPEC)::value;
+                R dh = R(0), dp = R(0);
+                V2 prev;
 #pragma unroll
                 for (int k = 0; k < C; ++k) {
-                    V2 em = row[ycode[k]];
+                    const V2 em = row[ycode[k]];
                     V2 o;
-                    o.x = H.template cell<true>(k, em.x, runH, ka.wh, sp, zcap_h);
-                    o.y = Pm.template cell<true>(k, em.y, runP, ka.wp, sp, zcap_p);
-                    if (active) out[(C - 1 - k) * 32 + lane] = o;
+                    o.x = H.template cell<S>(k, em.x, runH, ka.wh, sp, S ? zcap_h : dh);
+                    o.y = Pm.template cell<S>(k, em.y, runP, ka.wp, sp, S ? zcap_p : dp);
+                    if constexpr (sizeof(R) == 4) {
+                        if (k & 1) {
+                            if (active) *(float4*)(lp + (k >> 1) * 512) = make_float4(prev.x, prev.y, o.x, o.y);
+                        } else {
+                            prev = o;
+                        }
+                    } else {
+                        if (active) *(V2*)(lp + k * 512) = o;
+                    }
                 }
-            } else {
-                FwdSpecial sp;
-                sp.start = sp.capture = false;
-                sp.kz = 0;
-                R dummy = R(0);
-#pragma unroll
-                for (int k = 0; k < C; ++k) {
-                    V2 em = row[ycode[k]];
-                    V2 o;
-                    o.x = H.template cell<false>(k, em.x, runH, ka.wh, sp, dummy);
-                    o.y = Pm.template cell<false>(k, em.y, runP, ka.wp, sp, dummy);
-                    if (active) out[(C - 1 - k) * 32 + lane] = o;
-                }
-            }
+            };
+            if (special) body(std::true_type{});
+            else body(std::false_type{});
             H.end(runH);
             Pm.end(runP);
             if (active) {
-                int2 ee = make_int2(H.e, Pm.e);
-                *(int2*)(blk + (int64_t)t * stride + exps_offset(C, RB) + lane * 8) = ee;
+                *(int2*)(lp + dE) = make_int2(H.e, Pm.e);
                 if (nb > 1 && !last && lane == 31) {
                     bout[i].h = H.ex;
                     bout[i].p = Pm.ex;
@@ -239,7 +294,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         ez_h += kh;
         ez_p += kp;
     }
-    const R invZh = R(1) / zcap_h, invZp = R(1) / zcap_p;
+    const R invZh = inv_z_rms(zcap_h), invZp = inv_z_rms(zcap_p);
 
     // ================================ backward + combine + sparsify + MEA ================================
     const int minnm = n < m ? n : m;
@@ -252,8 +307,8 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         if (sbits > cap) sbits = cap;
     }
     const R mea_scale = (R)ldexp(1.0, sbits);
-    const bool want_csr = !ka.refine_pass;
-    float* dense = (ka.dense_P != nullptr && want_csr) ? ka.dense_P + ka.dense_off[p] : nullptr;
+    float* dense = nullptr;
+    if constexpr (MODE == kModeFull) dense = ka.dense_P != nullptr ? ka.dense_P + ka.dense_off[p] : nullptr;
     R zb_h = R(0), zb_p = R(0);
     int ezb_h = 0, ezb_p = 0;
     int nnz_lane = 0;
@@ -265,45 +320,31 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         Pm.init();
         Acc An[C];
         int ycode[C];
-        unsigned jvalid = 0;
 #pragma unroll
         for (int k = 0; k < C; ++k) {
             An[k] = 0;
             int j = b * 32 * C + lane * C + k;
-            bool v = (j >= 1 && j <= m);
-            ycode[k] = v ? (int)ys[j - 1] : kSentinel;
-            jvalid |= (v ? 1u : 0u) << k;
+            ycode[k] = (j >= 1 && j <= m) ? (int)ys[j - 1] : kSentinel;
         }
         Acc Adin = 0, exA = 0;
-        char* blk = slot + (int64_t)b * blk_bytes;
         const bool last = (b == nb - 1);
         const int tstart = n + (last ? lz : 31);
         const BwdBnd<R, GP>* bin = (const BwdBnd<R, GP>*)((b & 1) ? bnd0 : bnd1);   // written by block b+1
         BwdBnd<R, GP>* bout = (BwdBnd<R, GP>*)((b & 1) ? bnd1 : bnd0);
         const int jbase = b * 32 * C + lane * C;
         int xnext = xcode_at(tstart - lane);
-        // F values and exponents of a step are loaded one step ahead (at the end of the previous iteration)
-        V2 Fv[C];
-        int2 eF;
-        auto load_step = [&](int t2) {
-            const int i2 = t2 - lane;
-            const bool act2 = (i2 >= 0) && (i2 <= n);
-            const char* stp2 = blk + (int64_t)t2 * stride;
-            const V2* in2 = (const V2*)stp2;
+        // F values and exponents of step t-1 are loaded while step t is computed: a 16-byte word is reloaded as
+        // soon as its cells are consumed, so every load has a whole step to land
+        char* lp = slot + (int64_t)b * blk_bytes + (int64_t)tstart * stride + lane * SL::kLaneBytes;
+        FRegs<R, C> Fv;
 #pragma unroll
-            for (int k = 0; k < C; ++k) {
-                if (act2) Fv[k] = in2[(C - 1 - k) * 32 + lane];
-                else { Fv[k].x = R(0); Fv[k].y = R(0); }
-            }
-            eF = act2 ? *(const int2*)(stp2 + exps_offset(C, RB) + lane * 8) : make_int2(0, 0);
-        };
-        load_step(tstart);
-        for (int t = tstart; t >= 0; --t) {
+        for (int u = 0; u < FRegs<R, C>::kUnits; ++u) Fv.load(lp, u);
+        int2 eF = *(const int2*)(lp + dE);
+        for (int t = tstart; t >= 0; --t, lp -= stride) {
             const int i = t - lane;
-            const bool active = (i >= 0) && (i <= n);
+            const bool active = (unsigned)i <= (unsigned)n;
             const int xcode = xnext;
             xnext = xcode_at(i - 1);
-            char* stp = blk + (int64_t)t * stride;
             BwdEx<R, GH> rh = shfl_dn_ex(H.ex);
             BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex);
             Acc rA = shfl_dn1(exA);
@@ -314,8 +355,8 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     rp = rec.p;
                     rA = rec.A;
                 } else {
-                    zero_ex(rh);
-                    zero_ex(rp);
+                    zero_ex(rh, H.e);
+                    zero_ex(rp, Pm.e);
                     rA = 0;
                 }
             }
@@ -325,68 +366,72 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             BwdRun<R, GP> runP;
             H.begin(rh, resc, runH, range_flag);
             Pm.begin(rp, resc, runP, range_flag);
+            // rows outside 0..n exist only while the wavefront ramps up and down: their F words were never written
+            if (t < 31 || t > n) {   // warp-uniform
+                Fv.kill(active);
+                if (!active) eF = make_int2(0, 0);
+            }
             PScale<R> psh, psp;
-            psh.set(eF.x + H.e - ez_h, invZh);
-            psp.set(eF.y + Pm.e - ez_p, invZp);
+            const bool bad_h = psh.set(eF.x + H.e - ez_h, invZh);
+            const bool bad_p = psp.set(eF.y + Pm.e - ez_p, invZp);
+            if ((bad_h || bad_p) && active && jbase <= m) range_flag = 1;   // padding lanes hold B = 0 at exponent 0
             const bool special = (last && t == tstart) || (b == 0 && t == 0);   // warp-uniform
             BwdSpecial sp;
             sp.end = special && (last && lane == lz && i == n);
             sp.capture = special && (b == 0 && lane == 0 && i == 0);
             sp.kz = kz;
-            // loop 1: the two backward recurrences; F(i,j) is replaced in place by the model posteriors
-            auto rec_body = [&](auto SPEC, int k) {
-                constexpr bool S = decltype(SPEC)::value;
-                V2 em = row[ycode[k]];
-                R zh = R(0), zp = R(0);
-                R bmh = H.template cell<S>(k, em.x, runH, ka.wh, sp, zh);
-                R bmp = Pm.template cell<S>(k, em.y, runP, ka.wp, sp, zp);
-                if (S && sp.capture && k == 0) {
-                    zb_h = zh;
-                    zb_p = zp;
-                    ezb_h = H.e;
-                    ezb_p = Pm.e;
-                }
-                Fv[k].x = psh.apply(Fv[k].x, bmh);
-                Fv[k].y = psp.apply(Fv[k].y, bmp);
-            };
-            if (special) {
-#pragma unroll
-                for (int k = C - 1; k >= 0; --k) rec_body(std::true_type{}, k);
-            } else {
-#pragma unroll
-                for (int k = C - 1; k >= 0; --k) rec_body(std::false_type{}, k);
-            }
-            // loop 2: combine, expected-accuracy max-plus, threshold + parking of kept entries
             Acc Adiag = Adin, Aright = rA;
-            int cnt = 0;
-            char* park = stp + (int64_t)lane * sizeof(V2);
+            unsigned kept = 0;
+            const bool more = t > 0;
+            const bool row_ok = (i >= 1) && (i <= n);
+            auto body = [&](auto SPEC) {
+                constexpr bool S = decltype(SPEC)::value;
 #pragma unroll
-            for (int k = C - 1; k >= 0; --k) {
-                const R P = combine_rms(Fv[k].x, Fv[k].y);
-                const Acc q = quantise(P, mea_scale);
-                Acc a = Adiag + q;
-                a = a > An[k] ? a : An[k];
-                a = a > Aright ? a : Aright;
-                Adiag = An[k];
-                An[k] = a;
-                Aright = a;
-                if (want_csr) {
-                    const bool keep = P >= ka.tau;
-                    st_entry_if(park, (float)P, k, keep);
-                    park += keep ? 32 * (int)sizeof(V2) : 0;
-                    cnt += keep ? 1 : 0;
-                    if (dense != nullptr && i >= 1 && i <= n && ((jvalid >> k) & 1))
-                        dense[(int64_t)(i - 1) * m + (jbase + k - 1)] = (float)P;
+                for (int k = C - 1; k >= 0; --k) {
+                    // the two backward recurrences
+                    const V2 em = row[ycode[k]];
+                    R zh = R(0), zp = R(0);
+                    const R bmh = H.template cell<S>(k, em.x, runH, ka.wh, sp, zh);
+                    const R bmp = Pm.template cell<S>(k, em.y, runP, ka.wp, sp, zp);
+                    if (S && sp.capture && k == 0) {
+                        zb_h = zh;
+                        zb_p = zp;
+                        ezb_h = H.e;
+                        ezb_p = Pm.e;
+                    }
+                    // combine, expected-accuracy max-plus, threshold + parking of the kept entry
+                    const R P = combine_rms(psh.apply(Fv.h(k), bmh), psp.apply(Fv.p(k), bmp));
+                    const Acc q = quantise(P, mea_scale);
+                    Acc a = Adiag + q;
+                    a = a > An[k] ? a : An[k];
+                    a = a > Aright ? a : Aright;
+                    Adiag = An[k];
+                    An[k] = a;
+                    Aright = a;
+                    if constexpr (kCsr) {
+                        const bool keep = P >= ka.tau;
+                        st_f32_if(lp + SL::cell_off(k), (float)P, keep);
+                        kept |= (keep ? 1u : 0u) << k;
+                    }
+                    if constexpr (MODE == kModeFull) {
+                        const int j = jbase + k;
+                        if (dense != nullptr && row_ok && j >= 1 && j <= m) dense[(int64_t)(i - 1) * m + (j - 1)] = (float)P;
+                    }
+                    if (FRegs<R, C>::unit_done(k) && more) Fv.load(lp - stride, FRegs<R, C>::unit_of(k));
                 }
-            }
-            if (t > 0) load_step(t - 1);
+            };
+            if (special) body(std::true_type{});
+            else body(std::false_type{});
+            if (more) eF = *(const int2*)(lp - stride + dE);
             H.end(runH);
             Pm.end(runP);
             exA = An[0];
             Adin = rA;
             if (active) {
-                if (want_csr) *(uint8_t*)(stp + cnts_offset(C, RB) + lane) = (uint8_t)cnt;
-                nnz_lane += cnt;
+                if constexpr (kCsr) {
+                    *(int*)(lp + dE) = (int)kept;   // replaces e_hmm of this (step, lane), already consumed
+                    nnz_lane += __popc(kept);
+                }
                 if (nb > 1 && b > 0 && lane == 0) {
                     bout[i].h = H.ex;
                     bout[i].p = Pm.ex;
@@ -409,7 +454,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         const int xi = ka.pairs[2 * (int64_t)p], yi = ka.pairs[2 * (int64_t)p + 1];
         ka.dist[(int64_t)xi * ka.k + yi] = (float)dist;
         ka.dist[(int64_t)yi * ka.k + xi] = (float)dist;
-        if (!ka.refine_pass && (float)dist < ka.refine_below) {
+        if (MODE != kModeDist && sizeof(R) == 4 && (float)dist < ka.refine_below) {
             int nbd;
             const int c64 = choose_class(m + 1, ka.refine_cmask, &nbd);
             const int pos = atomicAdd(&ka.hdr->refine_count[c64], 1);
@@ -419,34 +464,37 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         }
     }
 
-    // ---- logZ (optional): undo the background normalisation, ln Z = ln2*(log2 Zm + eZ) + sum lx ---------
-    if (ka.logZ != nullptr && want_csr) {
-        double ch = 0.0, cp = 0.0;
-        for (int q = lane; q < n; q += 32) { ch += ka.lx_h[xs[q]]; cp += ka.lx_p[xs[q]]; }
-        for (int q = lane; q < m; q += 32) { ch += ka.lx_h[ys[q]]; cp += ka.lx_p[ys[q]]; }
+    // ---- logZ (tests): undo the background normalisation, ln Z = ln2*(log2 Zm + eZ) + sum lx ----------------
+    if constexpr (MODE == kModeFull) {
+        if (ka.logZ != nullptr) {
+            double ch = 0.0, cp = 0.0;
+            for (int q = lane; q < n; q += 32) { ch += ka.lx_h[xs[q]]; cp += ka.lx_p[xs[q]]; }
+            for (int q = lane; q < m; q += 32) { ch += ka.lx_h[ys[q]]; cp += ka.lx_p[ys[q]]; }
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            ch += __shfl_xor_sync(kFull, ch, o);
-            cp += __shfl_xor_sync(kFull, cp, o);
-        }
-        zb_h = __shfl_sync(kFull, zb_h, 0);
-        zb_p = __shfl_sync(kFull, zb_p, 0);
-        ezb_h = __shfl_sync(kFull, ezb_h, 0);
-        ezb_p = __shfl_sync(kFull, ezb_p, 0);
-        if (lane == 0) {
-            const double ln2 = 0.69314718055994530942;
-            double* o = ka.logZ + 4 * (int64_t)p;
-            o[0] = ln2 * (log2_real(zcap_h) + ez_h) + ch;
-            o[1] = ln2 * (log2_real(zb_h) + ezb_h) + ch;
-            o[2] = ln2 * (log2_real(zcap_p) + ez_p) + cp;
-            o[3] = ln2 * (log2_real(zb_p) + ezb_p) + cp;
+            for (int o = 16; o > 0; o >>= 1) {
+                ch += __shfl_xor_sync(kFull, ch, o);
+                cp += __shfl_xor_sync(kFull, cp, o);
+            }
+            zb_h = __shfl_sync(kFull, zb_h, 0);
+            zb_p = __shfl_sync(kFull, zb_p, 0);
+            ezb_h = __shfl_sync(kFull, ezb_h, 0);
+            ezb_p = __shfl_sync(kFull, ezb_p, 0);
+            if (lane == 0) {
+                const double ln2 = 0.69314718055994530942;
+                double* o = ka.logZ + 4 * (int64_t)p;
+                o[0] = ln2 * (log2_real(zcap_h) + ez_h) + ch;
+                o[1] = ln2 * (log2_real(zb_h) + ezb_h) + ch;
+                o[2] = ln2 * (log2_real(zcap_p) + ez_p) + cp;
+                o[3] = ln2 * (log2_real(zb_p) + ezb_p) + cp;
+            }
         }
     }
 
     // ---- CSR: warp-scan compaction of the parked entries, rows ascending, columns ascending ---------------
-    // Row i's entries sit at (step i+l, lane l) for l = 0..31 and blocks 0..nb-1: ascending (block, lane) is
-    // ascending column; inside a lane they were parked right-to-left, so they are read back reversed.
-    if (want_csr) {
+    // Row i's cells sit at (block b, step i+l, lane l): ascending (block, lane, k) is ascending column. A segment
+    // is one (row, block); segments are walked in row-major order, SEG at a time so that the mask loads of a
+    // batch are independent. Two segments share one warp scan (16-bit fields: a segment holds <= 32*16 entries).
+    if constexpr (kCsr) {
         const int nnz = warp_sum(nnz_lane);
         unsigned long long poff = 0;
         if (lane == 0) poff = atomicAdd(&ka.hdr->pool_cursor, (unsigned long long)nnz);
@@ -456,93 +504,56 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             if (atomicCAS(&ka.hdr->status[0], 0, -6 /*QP_ERR_NNZ_CAPACITY*/) == 0) ka.hdr->status[1] = p;
         }
         int32_t* rp = ka.row_ptr + ka.pair_row_base[p];
+        int32_t* pcol = ka.pool_col + poff;
+        float* pval = ka.pool_val + poff;
         int running = 0;
-        // Segments (row i, block b) in row-major order, SEG at a time so that the loads of a batch are
-        // independent: (1) the SEG count bytes, (2) SEG warp scans, (3) e-th entry of every segment, stores.
-        constexpr int SEGM = 8;    // multi-block batch
-        const int32_t colbase = lane * C - 1;
-        if (nb == 1) {
-            constexpr int SEG = 8;   // rows per batch (larger batches cost registers in the DP loops: measured slower)
-            const char* base = slot + (int64_t)(1 + lane) * stride;          // row 1
-            const char* cbase = base + cnts_offset(C, RB) + lane;
-            const bool lane_in = colbase < m;                                 // lane owns at least one real column
-            int cnx[SEG];   // counts of the NEXT batch, loaded while the current one is compacted
+        constexpr int SEG = 8;
+        const int nseg = n * nb;
+        const char* lane0 = slot + (int64_t)lane * stride + lane * SL::kLaneBytes;   // (step l, lane l) of block 0
+        for (int s0 = 0; s0 < nseg; s0 += SEG) {
+            unsigned mk[SEG];
+            const char* sp[SEG];
+            int jb[SEG];
+            int i = 1 + s0 / nb, b = s0 - (i - 1) * nb;
 #pragma unroll
-            for (int u = 0; u < SEG; ++u) cnx[u] = (lane_in && u < n) ? (int)*(const uint8_t*)(cbase + (int64_t)u * stride) : 0;
-            for (int r0 = 0; r0 < n; r0 += SEG) {
-                int cn[SEG], st[SEG];
+            for (int u = 0; u < SEG; ++u) {
+                jb[u] = b * 32 * C + lane * C;                       // first column (1-based grid index) of the lane
+                sp[u] = lane0 + (int64_t)b * blk_bytes + (int64_t)i * stride;
+                mk[u] = (s0 + u < nseg && jb[u] <= m) ? (unsigned)*(const int*)(sp[u] + dE) : 0u;
+                if (++b == nb) { b = 0; ++i; }
+            }
+            int st[SEG];
+#pragma unroll
+            for (int u = 0; u < SEG; u += 2) {
+                const int c0 = __popc(mk[u]), c1 = __popc(mk[u + 1]);
+                const int v = c0 | (c1 << 16);
+                const int ex = warp_excl_scan(v, lane);
+                const int tot = __shfl_sync(kFull, ex + v, 31);
+                st[u] = running + (ex & 0xffff);
+                running += tot & 0xffff;
+                st[u + 1] = running + (ex >> 16);
+                running += tot >> 16;
+            }
+            // row starts: segment u opens row i iff its block is 0; its start is st[u] of lane 0
+            {
+                int i2 = 1 + s0 / nb, b2 = s0 - (i2 - 1) * nb;
 #pragma unroll
                 for (int u = 0; u < SEG; ++u) {
-                    cn[u] = cnx[u];
-                    const int rn = r0 + SEG + u;
-                    cnx[u] = (lane_in && rn < n) ? (int)*(const uint8_t*)(cbase + (int64_t)rn * stride) : 0;
-                }
-                int maxc = 0;
-#pragma unroll
-                for (int u = 0; u < SEG; ++u) {
-                    if (lane == 0 && r0 + u < n) rp[r0 + u] = running;
-                    const int ex = warp_excl_scan(cn[u], lane);
-                    st[u] = running + ex + cn[u] - 1;   // destination of this lane's FIRST parked entry (highest column)
-                    running += __shfl_sync(kFull, ex + cn[u], 31);
-                    maxc = cn[u] > maxc ? cn[u] : maxc;
-                }
-                if (ok) {
-                    maxc = __reduce_max_sync(kFull, maxc);
-                    const char* eb = base + (int64_t)r0 * stride + (int64_t)lane * sizeof(V2);
-                    for (int e = 0; e < maxc; ++e) {
-                        Entry en[SEG];
-#pragma unroll
-                        for (int u = 0; u < SEG; ++u)
-                            if (e < cn[u]) en[u] = *(const Entry*)(eb + (int64_t)u * stride + (int64_t)e * 32 * sizeof(V2));
-#pragma unroll
-                        for (int u = 0; u < SEG; ++u)
-                            if (e < cn[u]) {
-                                const long long dst = (long long)poff + st[u] - e;
-                                ka.pool_col[dst] = colbase + en[u].k;
-                                ka.pool_val[dst] = en[u].val;
-                            }
-                    }
+                    if (lane == 0 && b2 == 0 && s0 + u < nseg) rp[i2 - 1] = st[u];
+                    if (++b2 == nb) { b2 = 0; ++i2; }
                 }
             }
-        } else {
-            // segments (row i, block b) in row-major order
-            const int nseg = n * nb;
-            for (int s0 = 0; s0 < nseg; s0 += SEGM) {
-                int cn[SEGM], st[SEGM];
-                const char* sp[SEGM];
-                int32_t jb[SEGM];
+            if (ok) {
 #pragma unroll
-                for (int u = 0; u < SEGM; ++u) {
-                    const int sg = s0 + u;
-                    const int i = 1 + sg / nb, b = sg - (i - 1) * nb;
-                    jb[u] = b * 32 * C + colbase;
-                    sp[u] = slot + (int64_t)b * blk_bytes + (int64_t)(i + lane) * stride;
-                    cn[u] = (sg < nseg && jb[u] < m) ? (int)*(const uint8_t*)(sp[u] + cnts_offset(C, RB) + lane) : 0;
-                }
-                int maxc = 0;
-#pragma unroll
-                for (int u = 0; u < SEGM; ++u) {
-                    const int sg = s0 + u;
-                    if (lane == 0 && sg < nseg && sg % nb == 0) rp[sg / nb] = running;
-                    const int ex = warp_excl_scan(cn[u], lane);
-                    st[u] = running + ex + cn[u] - 1;
-                    running += __shfl_sync(kFull, ex + cn[u], 31);
-                    maxc = cn[u] > maxc ? cn[u] : maxc;
-                }
-                if (ok) {
-                    maxc = __reduce_max_sync(kFull, maxc);
-                    for (int e = 0; e < maxc; ++e) {
-                        Entry en[SEGM];
-#pragma unroll
-                        for (int u = 0; u < SEGM; ++u)
-                            if (e < cn[u]) en[u] = *(const Entry*)(sp[u] + ((int64_t)e * 32 + lane) * sizeof(V2));
-#pragma unroll
-                        for (int u = 0; u < SEGM; ++u)
-                            if (e < cn[u]) {
-                                const long long dst = (long long)poff + st[u] - e;
-                                ka.pool_col[dst] = jb[u] + en[u].k;
-                                ka.pool_val[dst] = en[u].val;
-                            }
+                for (int u = 0; u < SEG; ++u) {
+                    unsigned mm = mk[u];
+                    int d = st[u];
+                    while (mm) {
+                        const int k = __ffs(mm) - 1;
+                        mm &= mm - 1;
+                        pcol[d] = jb[u] + k - 1;                      // 0-based column in y
+                        pval[d] = *(const float*)(sp[u] + SL::cell_off(k));
+                        ++d;
                     }
                 }
             }

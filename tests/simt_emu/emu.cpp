@@ -65,7 +65,7 @@ static int emu_pair(const EmuModel& mh, const EmuModel& mp, const uint8_t* xs, i
                 bool resc = ((t & mask) == 0) || (i == 0);
                 int xcode = (i >= 1 && i <= n) ? xs[i - 1] : kSentinel;
                 FwdRun<R, 2> runH; FwdRun<R, GP> runP;
-                H[l].begin(rh[l], resc, runH, range_flag); Pm[l].begin(rp[l], resc, runP, range_flag);
+                H[l].begin(rh[l], resc, runH, wh, range_flag); Pm[l].begin(rp[l], resc, runP, wp, range_flag);
                 FwdSpecial sp; sp.start = special && (b == 0 && l == 0 && i == 0); sp.capture = special && (last && l == lz && i == n); sp.kz = kz;
                 for (int k = 0; k < C; ++k) {
                     int j = b * 32 * C + l * C + k;
@@ -87,7 +87,7 @@ static int emu_pair(const EmuModel& mh, const EmuModel& mp, const uint8_t* xs, i
     { int kh = expo(zcap_h), kp = expo(zcap_p);
       if (kh == kZeroExp || kp == kZeroExp) return -8;
       zcap_h *= pow2i(-kh, R(0)); zcap_p *= pow2i(-kp, R(0)); ez_h += kh; ez_p += kp; }
-    const R invZh = R(1) / zcap_h, invZp = R(1) / zcap_p;
+    const R invZh = inv_z_rms(zcap_h), invZp = inv_z_rms(zcap_p);
     // ---------------- backward
     const int minnm = n < m ? n : m;
     int sbits = (int)(8 * sizeof(Acc)) - 2; { int need = 1; while ((1 << need) <= minnm) ++need; sbits -= need; int cap = sizeof(R) == 4 ? 20 : 40; if (sbits > cap) sbits = cap; }
@@ -116,7 +116,8 @@ static int emu_pair(const EmuModel& mh, const EmuModel& mp, const uint8_t* xs, i
                 BwdRun<R, 2> runH; BwdRun<R, GP> runP;
                 H[l].begin(rh[l], resc, runH, range_flag); Pm[l].begin(rp[l], resc, runP, range_flag);
                 int eFh = active ? EH[((size_t)b * T + t) * 32 + l] : 0, eFp = active ? EP[((size_t)b * T + t) * 32 + l] : 0;
-                PScale<R> psh, psp; psh.set(eFh + H[l].e - ez_h, invZh); psp.set(eFp + Pm[l].e - ez_p, invZp);
+                PScale<R> psh, psp;
+                if ((psh.set(eFh + H[l].e - ez_h, invZh) | psp.set(eFp + Pm[l].e - ez_p, invZp)) && active && b * 32 * C + l * C <= m) range_flag = 1;
                 Acc Adiag = Adin[l], Aright = rA[l];
                 BwdSpecial sp; sp.end = special && (last && l == lz && i == n); sp.capture = special && (b == 0 && l == 0 && i == 0); sp.kz = kz;
                 for (int k = C - 1; k >= 0; --k) {
