@@ -34,15 +34,24 @@ struct alignas(16) PairInfo {
 // block b, step t:  F planes | [32] int2 exponents (e_hmm, e_pf), one per lane
 //   fp32: [C/2][32] float4 = (F_hmm, F_pf) of the lane's columns 2u and 2u+1  (every warp access is 512 B contiguous)
 //   fp64: [C][32] double2  = (F_hmm, F_pf) of the lane's column k
-// The backward pass reuses a consumed (step, lane): a kept posterior is parked as a float in the F_hmm word of
-// its own cell, and the lane's bit mask of kept cells replaces e_hmm. Sparsification adds no scratch.
+// The exponent record of a step is written (and read back) only on the last step of every renormalisation period
+// and on the last step of the block: a lane's exponents cannot change in between.
+// The backward pass reuses consumed step records as per-row entry buffers: the kept (value, column) entries of
+// row i (found by lane l at step i+l, highest columns first) go to the F area of step record i+32, which every
+// lane has consumed before the first of them is written; row i's entry count goes to rowcnt[b][i]. Sparsification
+// therefore adds one step record and 4 bytes per row of scratch.
 QP_HD2 int64_t step_stride(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes + 256; }
 QP_HD2 int64_t exps_offset(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes; }
-QP_HD2 int num_steps(int n) { return n + 32; }
+QP_HD2 int num_steps(int n) { return n + 33; }
 QP_HD2 int64_t bnd_rec_bytes(int real_bytes) { return 12 * (int64_t)real_bytes + 16; }   // see BndRec in qp_pair.cuh
-QP_HD2 int64_t slot_bytes(int n, int C, int nb, int real_bytes) {
+// byte offset of rowcnt[nb][n+1] (int32) inside the slot
+QP_HD2 int64_t rowcnt_offset(int n, int C, int nb, int real_bytes) {
     int64_t b = (int64_t)nb * num_steps(n) * step_stride(C, real_bytes);
     if (nb > 1) b += 2 * (int64_t)(n + 1) * bnd_rec_bytes(real_bytes);
+    return (b + 15) & ~(int64_t)15;
+}
+QP_HD2 int64_t slot_bytes(int n, int C, int nb, int real_bytes) {
+    int64_t b = rowcnt_offset(n, C, nb, real_bytes) + (int64_t)nb * (n + 1) * 4;
     return (b + 255) & ~(int64_t)255;
 }
 

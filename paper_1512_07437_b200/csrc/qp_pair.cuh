@@ -1,7 +1,7 @@
 // qp_pair.cuh -- one warp takes one sequence pair through the whole hot path:
 //   forward (pair-HMM + partition function, fused)
 //   backward (both models) fused with combine, sparsify, MEA  8(a) a2, a4, a5, a6, a7
-//   warp-scan compaction of the kept entries into CSR         8(a) a6
+//   per-row entry buffers -> CSR (rows, columns ascending)     8(a) a6
 // Lane arithmetic lives in qp_lane.h; this file owns the wavefront (who processes which row when), the warp
 // shuffles that hand row boundaries to the neighbouring lane, and all global-memory traffic.
 //
@@ -151,14 +151,20 @@ template <int C> struct FRegs<double, C> {
     static constexpr int kUnits = C;
 };
 
-// park a kept posterior in the F_hmm word of its own (consumed) cell: predicated 4-byte store, no branch
-__device__ __forceinline__ void st_f32_if(void* ptr, float val, bool keep) {
+// append a kept posterior to its row's entry buffer: predicated 8-byte store, no branch
+__device__ __forceinline__ void st_entry_if(void* ptr, float val, int col, bool keep) {
     asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %2, 0;\n\t@p st.global.b32 [%0], %1;\n\t}"
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %3, 0;\n\t@p st.global.v2.b32 [%0], {%1, %2};\n\t}"
         :
-        : "l"(ptr), "r"(__float_as_int(val)), "r"((int)keep)
+        : "l"(ptr), "r"(__float_as_int(val)), "r"(col), "r"((int)keep)
         : "memory");
 }
+// entry buffers and row counts are written by one lane and read by another lane of the same warp: read them from L2
+__device__ __forceinline__ float4 ld_cg_f4(const void* p) { return __ldcg((const float4*)p); }
+
+// Residue codes of the rows: lane l works on row t-l, so a lane's next row is its neighbour's current one. The code
+// travels with the wavefront by shuffle; only the entering lane (lane 0 forward, lane 31 backward) takes a new
+// code, from a 32-row chunk that the warp loads (coalesced) one chunk ahead of its use.
 
 // ---------------------------------------------------------------------------------------------------------
 // the pair pipeline
@@ -209,14 +215,25 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         const FwdBnd<R, GP>* bin = (const FwdBnd<R, GP>*)((b & 1) ? bnd0 : bnd1);   // written by block b-1
         FwdBnd<R, GP>* bout = (FwdBnd<R, GP>*)((b & 1) ? bnd1 : bnd0);
         char* lp = slot + (int64_t)b * blk_bytes + lane * SL::kLaneBytes;   // this lane's F words of step t
-        int xnext = xcode_at(0 - lane);   // residue code of the row of the NEXT step, loaded one step ahead
+        const bool colact = b * 32 * C + lane * C <= m;   // lanes that hold only padding columns store nothing
+        // row codes: every lane starts on a row <= 0; lane 0 enters row t+1 at the end of step t
+        int xcode = kSentinel;
+        int chunk = xcode_at(lane + 1), chunk_next = xcode_at(lane + 33);
         for (int t = 0; t <= tend; ++t, lp += stride) {
             const int i = t - lane;
             const bool active = (unsigned)i <= (unsigned)n;
-            const int xcode = xnext;
-            xnext = xcode_at(i + 1);
             FwdEx<R, GH> rh = shfl_up_ex(H.ex);
             FwdEx<R, GP> rp = shfl_up_ex(Pm.ex);
+            const V2* row = tab + xcode * kTabDim;
+            {
+                const int feed = __shfl_sync(kFull, chunk, t & 31);
+                const int up = __shfl_up_sync(kFull, xcode, 1);
+                xcode = lane == 0 ? feed : up;
+                if ((t & 31) == 31) {   // warp-uniform
+                    chunk = chunk_next;
+                    chunk_next = xcode_at(t + 34 + lane);
+                }
+            }
             if (lane == 0) {
                 if (b > 0 && active) {
                     const FwdBnd<R, GP> rec = ld_volatile(bin + i);
@@ -228,7 +245,6 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                 }
             }
             const bool resc = ((t & mask) == 0) || (i == 0);   // periodic, and on the lane's first row
-            const V2* row = tab + xcode * kTabDim;
             FwdRun<R, GH> runH;
             FwdRun<R, GP> runP;
             H.begin(rh, resc, runH, ka.wh, range_flag);
@@ -238,6 +254,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             sp.start = special && (b == 0 && lane == 0 && i == 0);
             sp.capture = special && (last && lane == lz && i == n);
             sp.kz = kz;
+            const bool st_on = active && colact;
             auto body = [&](auto SPEC) {
                 constexpr bool S = decltype(SPEC)::value;
                 R dh = R(0), dp = R(0);
@@ -250,12 +267,12 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     o.y = Pm.template cell<S>(k, em.y, runP, ka.wp, sp, S ? zcap_p : dp);
                     if constexpr (sizeof(R) == 4) {
                         if (k & 1) {
-                            if (active) *(float4*)(lp + (k >> 1) * 512) = make_float4(prev.x, prev.y, o.x, o.y);
+                            if (st_on) *(float4*)(lp + (k >> 1) * 512) = make_float4(prev.x, prev.y, o.x, o.y);
                         } else {
                             prev = o;
                         }
                     } else {
-                        if (active) *(V2*)(lp + k * 512) = o;
+                        if (st_on) *(V2*)(lp + k * 512) = o;
                     }
                 }
             };
@@ -263,12 +280,12 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             else body(std::false_type{});
             H.end(runH);
             Pm.end(runP);
-            if (active) {
-                *(int2*)(lp + dE) = make_int2(H.e, Pm.e);
-                if (nb > 1 && !last && lane == 31) {
-                    bout[i].h = H.ex;
-                    bout[i].p = Pm.ex;
-                }
+            // exponents: constant over a renormalisation period, recorded on its last step (all lanes: a lane whose
+            // last row fell inside the period has kept its exponent since)
+            if ((t & mask) == mask || t == tend) *(int2*)(lp + dE) = make_int2(H.e, Pm.e);
+            if (nb > 1 && !last && lane == 31 && active) {
+                bout[i].h = H.ex;
+                bout[i].p = Pm.ex;
             }
         }
         if (last) {
@@ -332,22 +349,50 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         const BwdBnd<R, GP>* bin = (const BwdBnd<R, GP>*)((b & 1) ? bnd0 : bnd1);   // written by block b+1
         BwdBnd<R, GP>* bout = (BwdBnd<R, GP>*)((b & 1) ? bnd1 : bnd0);
         const int jbase = b * 32 * C + lane * C;
-        int xnext = xcode_at(tstart - lane);
-        // F values and exponents of step t-1 are loaded while step t is computed: a 16-byte word is reloaded as
-        // soon as its cells are consumed, so every load has a whole step to land
+        const bool colact = jbase <= m;   // lanes that hold only padding columns: nothing was stored for them
+        // row codes: lane l starts on row tstart-l; lane 31 enters row t-32 at the end of step t
+        int xcode = xcode_at(tstart - lane);
+        int chunk = xcode_at(tstart - 32 - lane), chunk_next = xcode_at(tstart - 64 - lane);
+        // F values of step t-1 are loaded while step t is computed: a 16-byte word is reloaded as soon as its cells
+        // are consumed, so every load has a whole step to land. Exponent records exist on the last step of every
+        // renormalisation period (and of the block); they are fetched one step ahead too.
         char* lp = slot + (int64_t)b * blk_bytes + (int64_t)tstart * stride + lane * SL::kLaneBytes;
         FRegs<R, C> Fv;
+        Fv.kill(false);
+        if (colact) {
 #pragma unroll
-        for (int u = 0; u < FRegs<R, C>::kUnits; ++u) Fv.load(lp, u);
-        int2 eF = *(const int2*)(lp + dE);
+            for (int u = 0; u < FRegs<R, C>::kUnits; ++u) Fv.load(lp, u);
+        }
+        int2 eF = *(const int2*)(lp + dE), eFn = eF;
+        // entries of row i = t - lane go to step record i + 32 of this block (qp_internal.h); the row's running
+        // entry count travels down the lanes with the row
+        const int64_t dRow = (int64_t)(32 - lane) * stride - lane * SL::kLaneBytes;
+        int ecnt = 0;
+        int32_t* rowcnt = (int32_t*)(slot + rowcnt_offset(n, C, nb, RB)) + (int64_t)b * (n + 1);
         for (int t = tstart; t >= 0; --t, lp -= stride) {
             const int i = t - lane;
             const bool active = (unsigned)i <= (unsigned)n;
-            const int xcode = xnext;
-            xnext = xcode_at(i - 1);
+            const bool more = t > 0;
+            const bool enext = more && (((t - 1) & mask) == mask);   // warp-uniform: step t-1 holds a record
+            if (enext) eFn = *(const int2*)(lp - stride + dE);
             BwdEx<R, GH> rh = shfl_dn_ex(H.ex);
             BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex);
             Acc rA = shfl_dn1(exA);
+            if constexpr (kCsr) {
+                ecnt = shfl_dn1(ecnt);
+                if (lane == 31) ecnt = 0;
+            }
+            const V2* row = tab + xcode * kTabDim;
+            {
+                const int sdn = tstart - t;
+                const int feed = __shfl_sync(kFull, chunk, sdn & 31);
+                const int dn = __shfl_down_sync(kFull, xcode, 1);
+                xcode = lane == 31 ? feed : dn;
+                if ((sdn & 31) == 31) {   // warp-uniform
+                    chunk = chunk_next;
+                    chunk_next = xcode_at(t - 65 - lane);
+                }
+            }
             if (lane == 31) {
                 if (!last && active) {
                     const BwdBnd<R, GP> rec = ld_volatile(bin + i);
@@ -361,29 +406,25 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                 }
             }
             const bool resc = ((t & mask) == mask) || (i == n);
-            const V2* row = tab + xcode * kTabDim;
             BwdRun<R, GH> runH;
             BwdRun<R, GP> runP;
             H.begin(rh, resc, runH, range_flag);
             Pm.begin(rp, resc, runP, range_flag);
             // rows outside 0..n exist only while the wavefront ramps up and down: their F words were never written
-            if (t < 31 || t > n) {   // warp-uniform
-                Fv.kill(active);
-                if (!active) eF = make_int2(0, 0);
-            }
+            if (t < 31 || t > n) Fv.kill(active);   // warp-uniform
             PScale<R> psh, psp;
             const bool bad_h = psh.set(eF.x + H.e - ez_h, invZh);
             const bool bad_p = psp.set(eF.y + Pm.e - ez_p, invZp);
-            if ((bad_h || bad_p) && active && jbase <= m) range_flag = 1;   // padding lanes hold B = 0 at exponent 0
+            if ((bad_h || bad_p) && active && colact) range_flag = 1;   // padding lanes hold B = 0 at exponent 0
             const bool special = (last && t == tstart) || (b == 0 && t == 0);   // warp-uniform
             BwdSpecial sp;
             sp.end = special && (last && lane == lz && i == n);
             sp.capture = special && (b == 0 && lane == 0 && i == 0);
             sp.kz = kz;
             Acc Adiag = Adin, Aright = rA;
-            unsigned kept = 0;
-            const bool more = t > 0;
             const bool row_ok = (i >= 1) && (i <= n);
+            const bool ld_on = more && colact;
+            char* ep = lp + dRow + (int64_t)ecnt * 8;   // next free entry of this lane's row
             auto body = [&](auto SPEC) {
                 constexpr bool S = decltype(SPEC)::value;
 #pragma unroll
@@ -399,7 +440,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                         ezb_h = H.e;
                         ezb_p = Pm.e;
                     }
-                    // combine, expected-accuracy max-plus, threshold + parking of the kept entry
+                    // combine, expected-accuracy max-plus, threshold + append to the row's entry buffer
                     const R P = combine_rms(psh.apply(Fv.h(k), bmh), psp.apply(Fv.p(k), bmp));
                     const Acc q = quantise(P, mea_scale);
                     Acc a = Adiag + q;
@@ -410,33 +451,34 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     Aright = a;
                     if constexpr (kCsr) {
                         const bool keep = P >= ka.tau;
-                        st_f32_if(lp + SL::cell_off(k), (float)P, keep);
-                        kept |= (keep ? 1u : 0u) << k;
+                        st_entry_if(ep, (float)P, jbase + k - 1, keep);   // 0-based column in y
+                        ep += keep ? 8 : 0;
                     }
                     if constexpr (MODE == kModeFull) {
                         const int j = jbase + k;
                         if (dense != nullptr && row_ok && j >= 1 && j <= m) dense[(int64_t)(i - 1) * m + (j - 1)] = (float)P;
                     }
-                    if (FRegs<R, C>::unit_done(k) && more) Fv.load(lp - stride, FRegs<R, C>::unit_of(k));
+                    if (FRegs<R, C>::unit_done(k) && ld_on) Fv.load(lp - stride, FRegs<R, C>::unit_of(k));
                 }
             };
             if (special) body(std::true_type{});
             else body(std::false_type{});
-            if (more) eF = *(const int2*)(lp - stride + dE);
+            if (enext) eF = eFn;
             H.end(runH);
             Pm.end(runP);
             exA = An[0];
             Adin = rA;
-            if (active) {
-                if constexpr (kCsr) {
-                    *(int*)(lp + dE) = (int)kept;   // replaces e_hmm of this (step, lane), already consumed
-                    nnz_lane += __popc(kept);
+            if constexpr (kCsr) {
+                ecnt = (int)((ep - (lp + dRow)) >> 3);
+                if (lane == 0 && active) {   // row i of this block is complete
+                    rowcnt[i] = ecnt;
+                    nnz_lane += ecnt;
                 }
-                if (nb > 1 && b > 0 && lane == 0) {
-                    bout[i].h = H.ex;
-                    bout[i].p = Pm.ex;
-                    bout[i].A = exA;
-                }
+            }
+            if (nb > 1 && b > 0 && lane == 0 && active) {
+                bout[i].h = H.ex;
+                bout[i].p = Pm.ex;
+                bout[i].A = exA;
             }
         }
         if (b == 0) mea = An[0];   // lane 0 holds A'(0,0) = A(n,m)
@@ -490,11 +532,11 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         }
     }
 
-    // ---- CSR: warp-scan compaction of the parked entries, rows ascending, columns ascending ---------------
-    // Row i's cells sit at (block b, step i+l, lane l): ascending (block, lane, k) is ascending column. A segment
-    // is one (row, block); segments are walked in row-major order, SEG at a time so that the mask loads of a
-    // batch are independent. Two segments share one warp scan (16-bit fields: a segment holds <= 32*16 entries).
+    // ---- CSR: row counts -> row_ptr, entry buffers -> staging pool, rows ascending, columns ascending -----------
+    // 32 rows at a time, one row per lane. A row's entries sit in its buffer(s) highest column first; blocks are
+    // walked in ascending order and every buffer backwards, four entries (one 32-byte sector) per load pair.
     if constexpr (kCsr) {
+        __syncwarp();   // entry buffers and row counts were written by other lanes of this warp
         const int nnz = warp_sum(nnz_lane);
         unsigned long long poff = 0;
         if (lane == 0) poff = atomicAdd(&ka.hdr->pool_cursor, (unsigned long long)nnz);
@@ -506,54 +548,29 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         int32_t* rp = ka.row_ptr + ka.pair_row_base[p];
         int32_t* pcol = ka.pool_col + poff;
         float* pval = ka.pool_val + poff;
+        const int32_t* rowcnt = (const int32_t*)(slot + rowcnt_offset(n, C, nb, RB));
         int running = 0;
-        constexpr int SEG = 8;
-        const int nseg = n * nb;
-        const char* lane0 = slot + (int64_t)lane * stride + lane * SL::kLaneBytes;   // (step l, lane l) of block 0
-        for (int s0 = 0; s0 < nseg; s0 += SEG) {
-            unsigned mk[SEG];
-            const char* sp[SEG];
-            int jb[SEG];
-            int i = 1 + s0 / nb, b = s0 - (i - 1) * nb;
-#pragma unroll
-            for (int u = 0; u < SEG; ++u) {
-                jb[u] = b * 32 * C + lane * C;                       // first column (1-based grid index) of the lane
-                sp[u] = lane0 + (int64_t)b * blk_bytes + (int64_t)i * stride;
-                mk[u] = (s0 + u < nseg && jb[u] <= m) ? (unsigned)*(const int*)(sp[u] + dE) : 0u;
-                if (++b == nb) { b = 0; ++i; }
-            }
-            int st[SEG];
-#pragma unroll
-            for (int u = 0; u < SEG; u += 2) {
-                const int c0 = __popc(mk[u]), c1 = __popc(mk[u + 1]);
-                const int v = c0 | (c1 << 16);
-                const int ex = warp_excl_scan(v, lane);
-                const int tot = __shfl_sync(kFull, ex + v, 31);
-                st[u] = running + (ex & 0xffff);
-                running += tot & 0xffff;
-                st[u + 1] = running + (ex >> 16);
-                running += tot >> 16;
-            }
-            // row starts: segment u opens row i iff its block is 0; its start is st[u] of lane 0
-            {
-                int i2 = 1 + s0 / nb, b2 = s0 - (i2 - 1) * nb;
-#pragma unroll
-                for (int u = 0; u < SEG; ++u) {
-                    if (lane == 0 && b2 == 0 && s0 + u < nseg) rp[i2 - 1] = st[u];
-                    if (++b2 == nb) { b2 = 0; ++i2; }
-                }
-            }
-            if (ok) {
-#pragma unroll
-                for (int u = 0; u < SEG; ++u) {
-                    unsigned mm = mk[u];
-                    int d = st[u];
-                    while (mm) {
-                        const int k = __ffs(mm) - 1;
-                        mm &= mm - 1;
-                        pcol[d] = jb[u] + k - 1;                      // 0-based column in y
-                        pval[d] = *(const float*)(sp[u] + SL::cell_off(k));
-                        ++d;
+        for (int i0 = 1; i0 <= n; i0 += 32) {
+            const int i = i0 + lane;
+            const bool valid = i <= n;
+            int c = 0;
+            for (int b = 0; b < nb; ++b) c += valid ? __ldcg(rowcnt + (int64_t)b * (n + 1) + i) : 0;
+            const int ex = warp_excl_scan(c, lane);
+            const int tot = __shfl_sync(kFull, ex + c, 31);
+            int d = running + ex;
+            if (valid) rp[i - 1] = d;
+            running += tot;
+            if (ok && valid) {
+                for (int b = 0; b < nb; ++b) {
+                    const int cb = nb == 1 ? c : __ldcg(rowcnt + (int64_t)b * (n + 1) + i);
+                    const char* buf = slot + (int64_t)b * blk_bytes + (int64_t)(i + 32) * stride;
+                    for (int g = (cb - 1) >> 2; g >= 0; --g) {
+                        const float4 lo = ld_cg_f4(buf + g * 32), hi = ld_cg_f4(buf + g * 32 + 16);
+                        const int q = 4 * g;
+                        if (q + 3 < cb) { pval[d] = hi.z; pcol[d] = __float_as_int(hi.w); ++d; }
+                        if (q + 2 < cb) { pval[d] = hi.x; pcol[d] = __float_as_int(hi.y); ++d; }
+                        if (q + 1 < cb) { pval[d] = lo.z; pcol[d] = __float_as_int(lo.w); ++d; }
+                        pval[d] = lo.x; pcol[d] = __float_as_int(lo.y); ++d;
                     }
                 }
             }
