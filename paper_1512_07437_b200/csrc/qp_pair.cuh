@@ -118,38 +118,69 @@ template <typename R, int C> __device__ __forceinline__ int exps_delta(int lane)
     return (int)exps_offset(C, (int)sizeof(R)) + lane * 8 - lane * Slot<R>::kLaneBytes;
 }
 
-// F planes of one lane-step in registers
-template <typename R, int C> struct FRegs;
-template <int C> struct FRegs<float, C> {
-    float4 v[C / 2];
-    __device__ __forceinline__ void load(const char* lp, int u) { v[u] = *(const float4*)(lp + u * 512); }
-    __device__ __forceinline__ float h(int k) const { return (k & 1) ? v[k >> 1].z : v[k >> 1].x; }
-    __device__ __forceinline__ float p(int k) const { return (k & 1) ? v[k >> 1].w : v[k >> 1].y; }
-    __device__ __forceinline__ void kill(bool keep) {
-#pragma unroll
-        for (int u = 0; u < C / 2; ++u) {
-            v[u].x = keep ? v[u].x : 0.f; v[u].y = keep ? v[u].y : 0.f;
-            v[u].z = keep ? v[u].z : 0.f; v[u].w = keep ? v[u].w : 0.f;
-        }
-    }
-    // the unit holding cell k can be reloaded once both of its cells are consumed (columns are walked downwards)
-    static __device__ __forceinline__ bool unit_done(int k) { return (k & 1) == 0; }
+// ---- backward F staging: TMA bulk copies (cp.async.bulk) of the step records into a per-warp shared-memory ring ----
+// The F words of a step record are contiguous ([units][32 lanes] x 16 bytes), so one bulk copy per unit row brings
+// the active lanes' words of step t-kStages+1.. into shared memory while step t is computed; completion is
+// signalled on a per-stage mbarrier (complete_tx::bytes). The lanes then read their words with 16-byte LDS.
+constexpr int kStages = 4;
+template <typename R, int C> struct FUnits {   // 16-byte words per lane and step
+    static constexpr int k = sizeof(R) == 4 ? C / 2 : C;
+};
+template <typename R, int C> struct RingBytes {
+    static constexpr int v = kStages * FUnits<R, C>::k * 512;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t mbar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t mbar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(mbar)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\tLAB_WAIT:\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t@P1 bra DONE;\n\t"
+        "bra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(mbar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+// per-warp ring state; the sequence numbers run over the warp's whole lifetime (stage = seq % kStages,
+// parity = (seq / kStages) & 1), copies are consumed in the order they were issued
+struct FRing {
+    uint32_t data;     // shared-memory address of the ring
+    uint32_t mbar;     // shared-memory address of kStages mbarriers
+    uint32_t issued, waited;
+};
+
+// one unit (16 bytes) of a lane's F words, as (F_hmm, F_pf) per cell
+template <typename R> struct FWord;
+template <> struct FWord<float> {
+    float4 v;
+    __device__ __forceinline__ float h(int k) const { return (k & 1) ? v.z : v.x; }
+    __device__ __forceinline__ float p(int k) const { return (k & 1) ? v.w : v.y; }
     static __device__ __forceinline__ int unit_of(int k) { return k >> 1; }
-    static constexpr int kUnits = C / 2;
+    static __device__ __forceinline__ bool first_of_unit(int k) { return (k & 1) == 1; }   // columns are walked downwards
 };
-template <int C> struct FRegs<double, C> {
-    double2 v[C];
-    __device__ __forceinline__ void load(const char* lp, int u) { v[u] = *(const double2*)(lp + u * 512); }
-    __device__ __forceinline__ double h(int k) const { return v[k].x; }
-    __device__ __forceinline__ double p(int k) const { return v[k].y; }
-    __device__ __forceinline__ void kill(bool keep) {
-#pragma unroll
-        for (int u = 0; u < C; ++u) { v[u].x = keep ? v[u].x : 0.0; v[u].y = keep ? v[u].y : 0.0; }
-    }
-    static __device__ __forceinline__ bool unit_done(int) { return true; }
+template <> struct FWord<double> {
+    double2 v;
+    __device__ __forceinline__ double h(int) const { return v.x; }
+    __device__ __forceinline__ double p(int) const { return v.y; }
     static __device__ __forceinline__ int unit_of(int k) { return k; }
-    static constexpr int kUnits = C;
+    static __device__ __forceinline__ bool first_of_unit(int) { return true; }
 };
+__device__ __forceinline__ void lds16(float4& v, uint32_t addr) {
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+}
+__device__ __forceinline__ void lds16(double2& v, uint32_t addr) {
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+}
 
 // append a kept posterior to its row's entry buffer: predicated 8-byte store, no branch
 __device__ __forceinline__ void st_entry_if(void* ptr, float val, int col, bool keep) {
@@ -171,7 +202,7 @@ __device__ __forceinline__ float4 ld_cg_f4(const void* p) { return __ldcg((const
 // ---------------------------------------------------------------------------------------------------------
 template <typename R, int GP, int C, int MODE>
 __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2* __restrict__ tab, int p, char* slot,
-                             int lane) {
+                             int lane, FRing& ring) {
     using V2 = typename Traits<R>::vec2;
     using Acc = typename Traits<R>::acc_t;
     using SL = Slot<R>;
@@ -258,7 +289,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             auto body = [&](auto SPEC) {
                 constexpr bool S = decltype(SPEC)::value;
                 R dh = R(0), dp = R(0);
-                V2 prev;
+                [[maybe_unused]] V2 prev;
 #pragma unroll
                 for (int k = 0; k < C; ++k) {
                     const V2 em = row[ycode[k]];
@@ -353,16 +384,31 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         // row codes: lane l starts on row tstart-l; lane 31 enters row t-32 at the end of step t
         int xcode = xcode_at(tstart - lane);
         int chunk = xcode_at(tstart - 32 - lane), chunk_next = xcode_at(tstart - 64 - lane);
-        // F values of step t-1 are loaded while step t is computed: a 16-byte word is reloaded as soon as its cells
-        // are consumed, so every load has a whole step to land. Exponent records exist on the last step of every
-        // renormalisation period (and of the block); they are fetched one step ahead too.
+        // F words: bulk copies run kStages-1 steps ahead of the wavefront (see FRing). Only the lanes whose row is
+        // inside 0..n at the copied step are copied (a contiguous lane range); the other lanes read whatever an
+        // earlier step left in the ring (always a finite F value, the ring starts zeroed) and their posterior scale
+        // is forced to 0 below. Exponent records exist on the last step of every renormalisation period (and of the
+        // block); they are fetched one step ahead.
         char* lp = slot + (int64_t)b * blk_bytes + (int64_t)tstart * stride + lane * SL::kLaneBytes;
-        FRegs<R, C> Fv;
-        Fv.kill(false);
-        if (colact) {
-#pragma unroll
-            for (int u = 0; u < FRegs<R, C>::kUnits; ++u) Fv.load(lp, u);
-        }
+        constexpr int kUnits = FUnits<R, C>::k;
+        const int lact = last ? lz + 1 : 32;   // lanes that hold at least one real column
+        const char* blk0 = slot + (int64_t)b * blk_bytes;
+        auto issue = [&](int tt) {   // bulk-copy the F words of step tt (lanes max(0,tt-n) .. min(lact-1,tt))
+            const int lo = tt > n ? tt - n : 0, hi = tt < lact - 1 ? tt : lact - 1;
+            const uint32_t bytes = (uint32_t)(hi - lo + 1) * 16u;
+            const uint32_t st = ring.issued % kStages;
+            const uint32_t mb = ring.mbar + st * 8;
+            if (lane == 0) mbar_expect_tx(mb, bytes * kUnits);
+            if (lane < kUnits)
+                bulk_g2s(ring.data + st * (kUnits * 512) + lane * 512 + lo * 16,
+                         blk0 + (int64_t)tt * stride + lane * 512 + lo * 16, bytes, mb);
+            ++ring.issued;
+        };
+        fence_proxy_async();   // the forward pass wrote the records through the generic proxy
+        __syncwarp();
+#pragma unroll 1
+        for (int d = 0; d < kStages; ++d)
+            if (tstart - d >= 0) issue(tstart - d);
         int2 eF = *(const int2*)(lp + dE), eFn = eF;
         // entries of row i = t - lane go to step record i + 32 of this block (qp_internal.h); the row's running
         // entry count travels down the lanes with the row
@@ -410,12 +456,22 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             BwdRun<R, GP> runP;
             H.begin(rh, resc, runH, range_flag);
             Pm.begin(rp, resc, runP, range_flag);
-            // rows outside 0..n exist only while the wavefront ramps up and down: their F words were never written
-            if (t < 31 || t > n) Fv.kill(active);   // warp-uniform
             PScale<R> psh, psp;
             const bool bad_h = psh.set(eF.x + H.e - ez_h, invZh);
             const bool bad_p = psp.set(eF.y + Pm.e - ez_p, invZp);
-            if ((bad_h || bad_p) && active && colact) range_flag = 1;   // padding lanes hold B = 0 at exponent 0
+            // rows outside 0..n exist only while the wavefront ramps up and down, padding lanes hold no column: their
+            // F words were never written (nor copied), the posterior there is 0
+            if (active && colact) {
+                if (bad_h || bad_p) range_flag = 1;
+            } else {
+                psh.c = R(0);
+                psp.c = R(0);
+            }
+            // this step's F words have landed?
+            const uint32_t stg = ring.waited % kStages;
+            mbar_wait(ring.mbar + stg * 8, (ring.waited / kStages) & 1);
+            ++ring.waited;
+            const uint32_t sF = ring.data + stg * (kUnits * 512) + lane * 16;
             const bool special = (last && t == tstart) || (b == 0 && t == 0);   // warp-uniform
             BwdSpecial sp;
             sp.end = special && (last && lane == lz && i == n);
@@ -423,12 +479,17 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             sp.kz = kz;
             Acc Adiag = Adin, Aright = rA;
             const bool row_ok = (i >= 1) && (i <= n);
-            const bool ld_on = more && colact;
             char* ep = lp + dRow + (int64_t)ecnt * 8;   // next free entry of this lane's row
             auto body = [&](auto SPEC) {
                 constexpr bool S = decltype(SPEC)::value;
+                FWord<R> Fw, Fn;   // the unit in use and the next one, read one unit ahead
+                lds16(Fn.v, sF + (kUnits - 1) * 512);
 #pragma unroll
                 for (int k = C - 1; k >= 0; --k) {
+                    if (FWord<R>::first_of_unit(k)) {
+                        Fw = Fn;
+                        if (FWord<R>::unit_of(k) > 0) lds16(Fn.v, sF + (FWord<R>::unit_of(k) - 1) * 512);
+                    }
                     // the two backward recurrences
                     const V2 em = row[ycode[k]];
                     R zh = R(0), zp = R(0);
@@ -441,7 +502,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                         ezb_p = Pm.e;
                     }
                     // combine, expected-accuracy max-plus, threshold + append to the row's entry buffer
-                    const R P = combine_rms(psh.apply(Fv.h(k), bmh), psp.apply(Fv.p(k), bmp));
+                    const R P = combine_rms(psh.apply(Fw.h(k), bmh), psp.apply(Fw.p(k), bmp));
                     const Acc q = quantise(P, mea_scale);
                     Acc a = Adiag + q;
                     a = a > An[k] ? a : An[k];
@@ -458,12 +519,13 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                         const int j = jbase + k;
                         if (dense != nullptr && row_ok && j >= 1 && j <= m) dense[(int64_t)(i - 1) * m + (j - 1)] = (float)P;
                     }
-                    if (FRegs<R, C>::unit_done(k) && ld_on) Fv.load(lp - stride, FRegs<R, C>::unit_of(k));
                 }
             };
             if (special) body(std::true_type{});
             else body(std::false_type{});
             if (enext) eF = eFn;
+            __syncwarp();   // every lane has read its words of this stage: refill it
+            if (t >= kStages) issue(t - kStages);
             H.end(runH);
             Pm.end(runP);
             exA = An[0];
