@@ -9,18 +9,19 @@ template <typename R, int GP, int C, int MODE>
 __global__ void __launch_bounds__(kWarpsPerCta * 32, ctas_per_sm(C, sizeof(R) == 8))
 pair_kernel(const __grid_constant__ KArgs<R> ka) {
     using V2 = typename Traits<R>::vec2;
-    // dynamic shared memory: emission table | kStages mbarriers per warp | F ring per warp (qp_pair.cuh FRing)
+    // dynamic shared memory: emission table | kStages mbarriers per warp | F ring per warp | one zeroed stage (FRing)
     extern __shared__ __align__(128) unsigned char smem_raw[];
     V2* tab = (V2*)smem_raw;
     uint64_t* mbars = (uint64_t*)(smem_raw + sizeof(V2) * kTabDim * kTabDim);
     unsigned char* rings = smem_raw + sizeof(V2) * kTabDim * kTabDim + 128;
     static_assert(kWarpsPerCta * kStages * 8 <= 128, "mbarrier area");
     for (int q = threadIdx.x; q < kTabDim * kTabDim; q += blockDim.x) tab[q] = ka.tab[q];
-    for (int q = threadIdx.x; q < kWarpsPerCta * RingBytes<R, C>::v / 16; q += blockDim.x)
+    for (int q = threadIdx.x; q < (kWarpsPerCta * RingBytes<R, C>::v + RingBytes<R, C>::stage) / 16; q += blockDim.x)
         ((float4*)rings)[q] = make_float4(0.f, 0.f, 0.f, 0.f);
     FRing ring;
     ring.data = smem_u32(rings + (threadIdx.x >> 5) * RingBytes<R, C>::v);
     ring.mbar = smem_u32(mbars + (threadIdx.x >> 5) * kStages);
+    ring.zeros = smem_u32(rings + kWarpsPerCta * RingBytes<R, C>::v);
     ring.issued = ring.waited = 0;
     if ((threadIdx.x & 31) == 0) {
         for (int q = 0; q < kStages; ++q) mbar_init(ring.mbar + q * 8, 1);
@@ -60,7 +61,7 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
 }
 
 template <typename R, int C> constexpr size_t pair_smem_bytes() {
-    return sizeof(typename Traits<R>::vec2) * kTabDim * kTabDim + 128 + (size_t)kWarpsPerCta * RingBytes<R, C>::v;
+    return sizeof(typename Traits<R>::vec2) * kTabDim * kTabDim + 128 + (size_t)kWarpsPerCta * RingBytes<R, C>::v + RingBytes<R, C>::stage;
 }
 
 template <typename R, int GP, int C, int MODE> cudaError_t launch_pair(const KArgs<R>& ka, int grid, cudaStream_t st) {

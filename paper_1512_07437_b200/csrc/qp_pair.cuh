@@ -127,7 +127,8 @@ template <typename R, int C> struct FUnits {   // 16-byte words per lane and ste
     static constexpr int k = sizeof(R) == 4 ? C / 2 : C;
 };
 template <typename R, int C> struct RingBytes {
-    static constexpr int v = kStages * FUnits<R, C>::k * 512;
+    static constexpr int stage = FUnits<R, C>::k * 512;
+    static constexpr int v = kStages * stage;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -156,6 +157,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 struct FRing {
     uint32_t data;     // shared-memory address of the ring
     uint32_t mbar;     // shared-memory address of kStages mbarriers
+    uint32_t zeros;    // shared-memory address of a zeroed region as large as one stage (shared by the CTA)
     uint32_t issued, waited;
 };
 
@@ -384,24 +386,21 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         // row codes: lane l starts on row tstart-l; lane 31 enters row t-32 at the end of step t
         int xcode = xcode_at(tstart - lane);
         int chunk = xcode_at(tstart - 32 - lane), chunk_next = xcode_at(tstart - 64 - lane);
-        // F words: bulk copies run kStages-1 steps ahead of the wavefront (see FRing). Only the lanes whose row is
-        // inside 0..n at the copied step are copied (a contiguous lane range); the other lanes read whatever an
-        // earlier step left in the ring (always a finite F value, the ring starts zeroed) and their posterior scale
-        // is forced to 0 below. Exponent records exist on the last step of every renormalisation period (and of the
-        // block); they are fetched one step ahead.
+        // F words: one bulk copy per step brings the whole F area of a step record into the ring, kStages-1 steps
+        // ahead of the wavefront (see FRing). Lanes whose row is outside 0..n at that step, and lanes that hold only
+        // padding columns, never wrote their words: they read zeros from a shared zero region instead (posterior 0).
+        // Exponent records exist on the last step of every renormalisation period (and of the block); they are
+        // fetched one step ahead.
         char* lp = slot + (int64_t)b * blk_bytes + (int64_t)tstart * stride + lane * SL::kLaneBytes;
         constexpr int kUnits = FUnits<R, C>::k;
-        const int lact = last ? lz + 1 : 32;   // lanes that hold at least one real column
         const char* blk0 = slot + (int64_t)b * blk_bytes;
-        auto issue = [&](int tt) {   // bulk-copy the F words of step tt (lanes max(0,tt-n) .. min(lact-1,tt))
-            const int lo = tt > n ? tt - n : 0, hi = tt < lact - 1 ? tt : lact - 1;
-            const uint32_t bytes = (uint32_t)(hi - lo + 1) * 16u;
+        auto issue = [&](int tt) {   // bulk-copy the F area of step tt
             const uint32_t st = ring.issued % kStages;
-            const uint32_t mb = ring.mbar + st * 8;
-            if (lane == 0) mbar_expect_tx(mb, bytes * kUnits);
-            if (lane < kUnits)
-                bulk_g2s(ring.data + st * (kUnits * 512) + lane * 512 + lo * 16,
-                         blk0 + (int64_t)tt * stride + lane * 512 + lo * 16, bytes, mb);
+            if (lane == 0) {   // one lane issues: the copy instruction takes uniform operands
+                const uint32_t mb = ring.mbar + st * 8;
+                mbar_expect_tx(mb, kUnits * 512);
+                bulk_g2s(ring.data + st * (kUnits * 512), blk0 + (int64_t)tt * stride, kUnits * 512, mb);
+            }
             ++ring.issued;
         };
         fence_proxy_async();   // the forward pass wrote the records through the generic proxy
@@ -459,19 +458,12 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             PScale<R> psh, psp;
             const bool bad_h = psh.set(eF.x + H.e - ez_h, invZh);
             const bool bad_p = psp.set(eF.y + Pm.e - ez_p, invZp);
-            // rows outside 0..n exist only while the wavefront ramps up and down, padding lanes hold no column: their
-            // F words were never written (nor copied), the posterior there is 0
-            if (active && colact) {
-                if (bad_h || bad_p) range_flag = 1;
-            } else {
-                psh.c = R(0);
-                psp.c = R(0);
-            }
+            if ((bad_h || bad_p) && active && colact) range_flag = 1;   // padding lanes hold B = 0 at exponent 0
             // this step's F words have landed?
             const uint32_t stg = ring.waited % kStages;
             mbar_wait(ring.mbar + stg * 8, (ring.waited / kStages) & 1);
             ++ring.waited;
-            const uint32_t sF = ring.data + stg * (kUnits * 512) + lane * 16;
+            const uint32_t sF = ((active && colact) ? ring.data + stg * (kUnits * 512) : ring.zeros) + lane * 16;
             const bool special = (last && t == tstart) || (b == 0 && t == 0);   // warp-uniform
             BwdSpecial sp;
             sp.end = special && (last && lane == lz && i == n);
