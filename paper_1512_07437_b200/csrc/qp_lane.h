@@ -119,6 +119,8 @@ template <typename R, int G, int C> struct FwdModel {
     R Xn[G][C];      // X_g(i, j) for the row about to be computed
     R Sdin;          // S(i-1, j0-1): left neighbour's S of the previous row, already at exponent e
     int e;
+    R f1, f2;        // cached scale factor of the incoming values: 2^(rin.e - e) = f1 * f2 (f2 != 1 only if rare)
+    bool rare;
     FwdEx<R, G> ex;
 
     QP_HD void init() {
@@ -128,64 +130,81 @@ template <typename R, int G, int C> struct FwdModel {
         }
         Sdin = R(0);
         e = 0;
+        f1 = f2 = R(1);
+        rare = false;
         ex.S = ex.M = R(0);
         for (int g = 0; g < G; ++g) ex.Y[g] = R(0);
         ex.e = 0;
     }
 
-    // start of a step: optional renormalisation (incoming-aware), then bring the neighbour's values to own scale
-    QP_HD void begin(const FwdEx<R, G>& rin, bool rescale_now, FwdRun<R, G>& run, const Weights<R>& w, int& range_flag) {
-        if (rescale_now) {
-            R mo = Sdin;
-            R mi = qmax(rin.S, rin.M);
+    // start of a step: optional renormalisation (incoming-aware), then bring the neighbour's values to own scale.
+    // The scale factor 2^(rin.e - e) can change only when this lane or its neighbour renormalised, i.e. on the
+    // renormalisation step, on the step after it and while the wavefront ramps up (the caller's `recompute`,
+    // warp-uniform); on the other steps the cached factor is reused and rin.e is not looked at.
+    // zero_in: nothing comes in (first lane of the first block): the incoming values count as 0.
+    QP_HD void begin(const FwdEx<R, G>& rin, bool rescale_now, bool recompute, bool zero_in, FwdRun<R, G>& run,
+                     const Weights<R>& w, int& range_flag) {
+        if (recompute) {
+            if (rescale_now) {
+                R mo = Sdin;
+                R mi = qmax(rin.S, rin.M);
 #pragma unroll
-            for (int k = 0; k < C; ++k) {
-                mo = qmax(mo, S[k]);
+                for (int k = 0; k < C; ++k) {
+                    mo = qmax(mo, S[k]);
 #pragma unroll
-                for (int g = 0; g < G; ++g) mo = qmax(mo, Xn[g][k]);
-            }
-#pragma unroll
-            for (int g = 0; g < G; ++g) mi = qmax(mi, rin.Y[g]);
-            int ko = expo(mo), ki = expo(mi);
-            ki = ki == kZeroExp ? kZeroExp : ki + (rin.e - e);
-            int k = imax(ko, ki);
-            if (k != kZeroExp && k != 0) {
-                R f = pow2i(-k, R(0));
-#pragma unroll
-                for (int c = 0; c < C; ++c) {
-                    S[c] *= f;
-#pragma unroll
-                    for (int g = 0; g < G; ++g) Xn[g][c] *= f;
+                    for (int g = 0; g < G; ++g) mo = qmax(mo, Xn[g][k]);
                 }
-                Sdin *= f;
-                e += k;
+#pragma unroll
+                for (int g = 0; g < G; ++g) mi = qmax(mi, rin.Y[g]);
+                int ko = expo(mo), ki = zero_in ? kZeroExp : expo(mi);
+                ki = ki == kZeroExp ? kZeroExp : ki + (rin.e - e);
+                int k = imax(ko, ki);
+                if (k != kZeroExp && k != 0) {
+                    R f = pow2i(-k, R(0));
+#pragma unroll
+                    for (int c = 0; c < C; ++c) {
+                        S[c] *= f;
+#pragma unroll
+                        for (int g = 0; g < G; ++g) Xn[g][c] *= f;
+                    }
+                    Sdin *= f;
+                    e += k;
+                }
+            }
+            const int d = rin.e - e;
+            f2 = R(1);
+            rare = false;
+            if (zero_in) {
+                f1 = R(0);
+            } else if (d <= 60) {
+                f1 = pow2i(d, R(0));
+            } else {
+                // rare: large exponent gap (e.g. a lane that has not renormalised yet). Scale in two exact steps;
+                // only a value that would really leave the range is an error.
+                R mi = qmax(rin.S, rin.M);
+#pragma unroll
+                for (int g = 0; g < G; ++g) mi = qmax(mi, rin.Y[g]);
+                const int ki = expo(mi);
+                int dd = d;
+                if (ki != kZeroExp && ki + d > Traits<R>::kMaxShift - 27) {
+                    range_flag = 1;
+                    dd = Traits<R>::kMaxShift - 27 - ki;
+                }
+                f1 = pow2i(dd >> 1, R(0));
+                f2 = pow2i(dd - (dd >> 1), R(0));
+                rare = true;
             }
         }
-        const int d = rin.e - e;
         run.Sdiag = Sdin;
-        if (d <= 60) {
-            const R f = pow2i(d, R(0));
-            run.Ml = rin.M * f;
+        run.Ml = rin.M * f1;
+        Sdin = rin.S * f1;
 #pragma unroll
-            for (int g = 0; g < G; ++g) run.Yl[g] = rin.Y[g] * f;
-            Sdin = rin.S * f;
-        } else {
-            // rare: large exponent gap (e.g. a lane that has not renormalised yet). Scale in two exact steps;
-            // only a value that would really leave the range is an error.
-            R mi = qmax(rin.S, rin.M);
+        for (int g = 0; g < G; ++g) run.Yl[g] = rin.Y[g] * f1;
+        if (rare) {
+            run.Ml *= f2;
+            Sdin *= f2;
 #pragma unroll
-            for (int g = 0; g < G; ++g) mi = qmax(mi, rin.Y[g]);
-            const int ki = expo(mi);
-            int dd = d;
-            if (ki != kZeroExp && ki + d > Traits<R>::kMaxShift - 27) {
-                range_flag = 1;
-                dd = Traits<R>::kMaxShift - 27 - ki;
-            }
-            const R f1 = pow2i(dd >> 1, R(0)), f2 = pow2i(dd - (dd >> 1), R(0));
-            run.Ml = rin.M * f1 * f2;
-#pragma unroll
-            for (int g = 0; g < G; ++g) run.Yl[g] = rin.Y[g] * f1 * f2;
-            Sdin = rin.S * f1 * f2;
+            for (int g = 0; g < G; ++g) run.Yl[g] *= f2;
         }
 #pragma unroll
         for (int g = 0; g < G; ++g) run.mwl[g] = w.wMI[g] * run.Ml;
@@ -251,6 +270,8 @@ template <typename R, int G, int C> struct BwdModel {
     R Tn[C];         // T(i, j) for the row about to be computed
     R BXn[G][C];     // BX_g(i+1, j)
     int e;
+    R f1, f2;        // cached scale factor of the incoming values (FwdModel)
+    bool rare;
     BwdEx<R, G> ex;
 
     QP_HD void init() {
@@ -259,57 +280,71 @@ template <typename R, int G, int C> struct BwdModel {
             for (int g = 0; g < G; ++g) BXn[g][k] = R(0);
         }
         e = 0;
+        f1 = f2 = R(1);
+        rare = false;
         ex.TL = R(0);
         for (int g = 0; g < G; ++g) ex.BY[g] = R(0);
         ex.e = 0;
     }
 
-    QP_HD void begin(const BwdEx<R, G>& rin, bool rescale_now, BwdRun<R, G>& run, int& range_flag) {
-        if (rescale_now) {
-            R mo = R(0);
-            R mi = rin.TL;
+    // see FwdModel::begin; zero_in: last lane of the last block
+    QP_HD void begin(const BwdEx<R, G>& rin, bool rescale_now, bool recompute, bool zero_in, BwdRun<R, G>& run,
+                     int& range_flag) {
+        if (recompute) {
+            if (rescale_now) {
+                R mo = R(0);
+                R mi = rin.TL;
 #pragma unroll
-            for (int k = 0; k < C; ++k) {
-                mo = qmax(mo, Tn[k]);
+                for (int k = 0; k < C; ++k) {
+                    mo = qmax(mo, Tn[k]);
 #pragma unroll
-                for (int g = 0; g < G; ++g) mo = qmax(mo, BXn[g][k]);
-            }
-#pragma unroll
-            for (int g = 0; g < G; ++g) mi = qmax(mi, rin.BY[g]);
-            int ko = expo(mo), ki = expo(mi);
-            ki = ki == kZeroExp ? kZeroExp : ki + (rin.e - e);
-            int k = imax(ko, ki);
-            if (k != kZeroExp && k != 0) {
-                R f = pow2i(-k, R(0));
-#pragma unroll
-                for (int c = 0; c < C; ++c) {
-                    Tn[c] *= f;
-#pragma unroll
-                    for (int g = 0; g < G; ++g) BXn[g][c] *= f;
+                    for (int g = 0; g < G; ++g) mo = qmax(mo, BXn[g][k]);
                 }
-                e += k;
+#pragma unroll
+                for (int g = 0; g < G; ++g) mi = qmax(mi, rin.BY[g]);
+                int ko = expo(mo), ki = zero_in ? kZeroExp : expo(mi);
+                ki = ki == kZeroExp ? kZeroExp : ki + (rin.e - e);
+                int k = imax(ko, ki);
+                if (k != kZeroExp && k != 0) {
+                    R f = pow2i(-k, R(0));
+#pragma unroll
+                    for (int c = 0; c < C; ++c) {
+                        Tn[c] *= f;
+#pragma unroll
+                        for (int g = 0; g < G; ++g) BXn[g][c] *= f;
+                    }
+                    e += k;
+                }
+            }
+            const int d = rin.e - e;
+            f2 = R(1);
+            rare = false;
+            if (zero_in) {
+                f1 = R(0);
+            } else if (d <= 60) {
+                f1 = pow2i(d, R(0));
+            } else {   // rare, see FwdModel::begin
+                R mi = rin.TL;
+#pragma unroll
+                for (int g = 0; g < G; ++g) mi = qmax(mi, rin.BY[g]);
+                const int ki = expo(mi);
+                int dd = d;
+                if (ki != kZeroExp && ki + d > Traits<R>::kMaxShift - 27) {
+                    range_flag = 1;
+                    dd = Traits<R>::kMaxShift - 27 - ki;
+                }
+                f1 = pow2i(dd >> 1, R(0));
+                f2 = pow2i(dd - (dd >> 1), R(0));
+                rare = true;
             }
         }
-        const int d = rin.e - e;
-        if (d <= 60) {
-            const R f = pow2i(d, R(0));
-            run.Tc = rin.TL * f;
+        run.Tc = rin.TL * f1;
 #pragma unroll
-            for (int g = 0; g < G; ++g) run.BYr[g] = rin.BY[g] * f;
-        } else {   // rare, see FwdModel::begin
-            R mi = rin.TL;
+        for (int g = 0; g < G; ++g) run.BYr[g] = rin.BY[g] * f1;
+        if (rare) {
+            run.Tc *= f2;
 #pragma unroll
-            for (int g = 0; g < G; ++g) mi = qmax(mi, rin.BY[g]);
-            const int ki = expo(mi);
-            int dd = d;
-            if (ki != kZeroExp && ki + d > Traits<R>::kMaxShift - 27) {
-                range_flag = 1;
-                dd = Traits<R>::kMaxShift - 27 - ki;
-            }
-            const R f1 = pow2i(dd >> 1, R(0)), f2 = pow2i(dd - (dd >> 1), R(0));
-            run.Tc = rin.TL * f1 * f2;
-#pragma unroll
-            for (int g = 0; g < G; ++g) run.BYr[g] = rin.BY[g] * f1 * f2;
+            for (int g = 0; g < G; ++g) run.BYr[g] *= f2;
         }
     }
 

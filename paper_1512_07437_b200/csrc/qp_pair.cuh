@@ -31,21 +31,22 @@ __device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(k
 __device__ __forceinline__ int shfl_dn1(int v) { return __shfl_down_sync(kFull, v, 1); }
 __device__ __forceinline__ int64_t shfl_dn1(int64_t v) { return (int64_t)__shfl_down_sync(kFull, (long long)v, 1); }
 
-template <typename R, int G> __device__ __forceinline__ FwdEx<R, G> shfl_up_ex(const FwdEx<R, G>& a) {
+// the values always travel; the exponent only on the steps where the receiver recomputes its scale factor
+template <typename R, int G> __device__ __forceinline__ FwdEx<R, G> shfl_up_ex(const FwdEx<R, G>& a, bool with_e) {
     FwdEx<R, G> r;
     r.S = shfl_up1(a.S);
     r.M = shfl_up1(a.M);
 #pragma unroll
     for (int g = 0; g < G; ++g) r.Y[g] = shfl_up1(a.Y[g]);
-    r.e = shfl_up1(a.e);
+    r.e = with_e ? shfl_up1(a.e) : 0;   // with_e is warp-uniform
     return r;
 }
-template <typename R, int G> __device__ __forceinline__ BwdEx<R, G> shfl_dn_ex(const BwdEx<R, G>& a) {
+template <typename R, int G> __device__ __forceinline__ BwdEx<R, G> shfl_dn_ex(const BwdEx<R, G>& a, bool with_e) {
     BwdEx<R, G> r;
     r.TL = shfl_dn1(a.TL);
 #pragma unroll
     for (int g = 0; g < G; ++g) r.BY[g] = shfl_dn1(a.BY[g]);
-    r.e = shfl_dn1(a.e);
+    r.e = with_e ? shfl_dn1(a.e) : 0;
     return r;
 }
 // "nothing comes in": zero values at the receiving lane's own exponent (so that no rescaling is triggered)
@@ -255,8 +256,9 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         for (int t = 0; t <= tend; ++t, lp += stride) {
             const int i = t - lane;
             const bool active = (unsigned)i <= (unsigned)n;
-            FwdEx<R, GH> rh = shfl_up_ex(H.ex);
-            FwdEx<R, GP> rp = shfl_up_ex(Pm.ex);
+            const bool recompute = (t & mask) <= 1 || t < 32 || t > n;   // warp-uniform, see FwdModel::begin
+            FwdEx<R, GH> rh = shfl_up_ex(H.ex, recompute);
+            FwdEx<R, GP> rp = shfl_up_ex(Pm.ex, recompute);
             const V2* row = tab + xcode * kTabDim;
             {
                 const int feed = __shfl_sync(kFull, chunk, t & 31);
@@ -267,26 +269,28 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     chunk_next = xcode_at(t + 34 + lane);
                 }
             }
-            if (lane == 0) {
-                if (b > 0 && active) {
+            bool zero_in = lane == 0;   // nothing comes in from the left of the first block
+            if (b > 0) {                // warp-uniform: lane 0 takes the boundary column of the previous block
+                zero_in = lane == 0 && !active;
+                if (lane == 0 && active) {
                     const FwdBnd<R, GP> rec = ld_volatile(bin + i);
                     rh = rec.h;
                     rp = rec.p;
-                } else {
-                    zero_ex(rh, H.e);
-                    zero_ex(rp, Pm.e);
                 }
             }
             const bool resc = ((t & mask) == 0) || (i == 0);   // periodic, and on the lane's first row
             FwdRun<R, GH> runH;
             FwdRun<R, GP> runP;
-            H.begin(rh, resc, runH, ka.wh, range_flag);
-            Pm.begin(rp, resc, runP, ka.wp, range_flag);
+            H.begin(rh, resc, recompute, zero_in, runH, ka.wh, range_flag);
+            Pm.begin(rp, resc, recompute, zero_in, runP, ka.wp, range_flag);
             const bool special = (b == 0 && t == 0) || (last && t == tend);   // warp-uniform
             FwdSpecial sp;
-            sp.start = special && (b == 0 && lane == 0 && i == 0);
-            sp.capture = special && (last && lane == lz && i == n);
+            sp.start = sp.capture = false;
             sp.kz = kz;
+            if (special) {
+                sp.start = b == 0 && lane == 0 && i == 0;
+                sp.capture = last && lane == lz && i == n;
+            }
             const bool st_on = active && colact;
             auto body = [&](auto SPEC) {
                 constexpr bool S = decltype(SPEC)::value;
@@ -420,9 +424,11 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             const bool more = t > 0;
             const bool enext = more && (((t - 1) & mask) == mask);   // warp-uniform: step t-1 holds a record
             if (enext) eFn = *(const int2*)(lp - stride + dE);
-            BwdEx<R, GH> rh = shfl_dn_ex(H.ex);
-            BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex);
+            const bool recompute = (t & mask) >= mask - 1 || t >= n || t < 32;   // warp-uniform, see FwdModel::begin
+            BwdEx<R, GH> rh = shfl_dn_ex(H.ex, recompute);
+            BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex, recompute);
             Acc rA = shfl_dn1(exA);
+            if (lane == 31) rA = 0;
             if constexpr (kCsr) {
                 ecnt = shfl_dn1(ecnt);
                 if (lane == 31) ecnt = 0;
@@ -438,23 +444,21 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     chunk_next = xcode_at(t - 65 - lane);
                 }
             }
-            if (lane == 31) {
-                if (!last && active) {
+            bool zero_in = lane == 31;   // nothing comes in from the right of the last block
+            if (!last) {                 // warp-uniform: lane 31 takes the boundary column of the next block
+                zero_in = lane == 31 && !active;
+                if (lane == 31 && active) {
                     const BwdBnd<R, GP> rec = ld_volatile(bin + i);
                     rh = rec.h;
                     rp = rec.p;
                     rA = rec.A;
-                } else {
-                    zero_ex(rh, H.e);
-                    zero_ex(rp, Pm.e);
-                    rA = 0;
                 }
             }
             const bool resc = ((t & mask) == mask) || (i == n);
             BwdRun<R, GH> runH;
             BwdRun<R, GP> runP;
-            H.begin(rh, resc, runH, range_flag);
-            Pm.begin(rp, resc, runP, range_flag);
+            H.begin(rh, resc, recompute, zero_in, runH, range_flag);
+            Pm.begin(rp, resc, recompute, zero_in, runP, range_flag);
             PScale<R> psh, psp;
             const bool bad_h = psh.set(eF.x + H.e - ez_h, invZh);
             const bool bad_p = psp.set(eF.y + Pm.e - ez_p, invZp);
@@ -466,9 +470,12 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             const uint32_t sF = ((active && colact) ? ring.data + stg * (kUnits * 512) : ring.zeros) + lane * 16;
             const bool special = (last && t == tstart) || (b == 0 && t == 0);   // warp-uniform
             BwdSpecial sp;
-            sp.end = special && (last && lane == lz && i == n);
-            sp.capture = special && (b == 0 && lane == 0 && i == 0);
+            sp.end = sp.capture = false;
             sp.kz = kz;
+            if (special) {
+                sp.end = last && lane == lz && i == n;
+                sp.capture = b == 0 && lane == 0 && i == 0;
+            }
             Acc Adiag = Adin, Aright = rA;
             const bool row_ok = (i >= 1) && (i <= n);
             char* ep = lp + dRow + (int64_t)ecnt * 8;   // next free entry of this lane's row

@@ -57,15 +57,19 @@ static int emu_pair(const EmuModel& mh, const EmuModel& mp, const uint8_t* xs, i
                 int i = t - l; bool active = i >= 0 && i <= n;
                 if (l > 0) { rh[l] = H[l - 1].ex; rp[l] = Pm[l - 1].ex; }
                 else if (b > 0 && active) { rh[0] = bndH[i]; rp[0] = bndP[i]; }
-                else { memset(&rh[0], 0, sizeof rh[0]); memset(&rp[0], 0, sizeof rp[0]); }
+                else { rh[0] = H[0].ex; rp[0] = Pm[0].ex; }   // shfl_up leaves lane 0 its own value; zero_in makes it count as 0
             }
             const bool special = (b == 0 && t == 0) || (last && t == tend);
+            const bool recompute = (t & mask) <= 1 || t < 32 || t > n;   // qp_pair.cuh: warp-uniform
             for (int l = 0; l < 32; ++l) {
                 int i = t - l; bool active = i >= 0 && i <= n;
                 bool resc = ((t & mask) == 0) || (i == 0);
                 int xcode = (i >= 1 && i <= n) ? xs[i - 1] : kSentinel;
                 FwdRun<R, 2> runH; FwdRun<R, GP> runP;
-                H[l].begin(rh[l], resc, runH, wh, range_flag); Pm[l].begin(rp[l], resc, runP, wp, range_flag);
+                const bool zin = l == 0 && !(b > 0 && active);
+                FwdEx<R, 2> qh = rh[l]; FwdEx<R, GP> qp_ = rp[l];
+                if (!recompute) { qh.e = 123456; qp_.e = -123456; }   // the kernel does not shuffle the exponents then
+                H[l].begin(qh, resc, recompute, zin, runH, wh, range_flag); Pm[l].begin(qp_, resc, recompute, zin, runP, wp, range_flag);
                 FwdSpecial sp; sp.start = special && (b == 0 && l == 0 && i == 0); sp.capture = special && (last && l == lz && i == n); sp.kz = kz;
                 for (int k = 0; k < C; ++k) {
                     int j = b * 32 * C + l * C + k;
@@ -106,15 +110,19 @@ static int emu_pair(const EmuModel& mh, const EmuModel& mp, const uint8_t* xs, i
                 int i = t - l; bool active = i >= 0 && i <= n;
                 if (l < 31) { rh[l] = H[l + 1].ex; rp[l] = Pm[l + 1].ex; rA[l] = exA[l + 1]; }
                 else if (!last && active) { rh[l] = bH[i]; rp[l] = bP[i]; rA[l] = bA[i]; }
-                else { memset(&rh[l], 0, sizeof rh[l]); memset(&rp[l], 0, sizeof rp[l]); rA[l] = 0; }
+                else { rh[l] = H[l].ex; rp[l] = Pm[l].ex; rA[l] = 0; }   // shfl_down leaves lane 31 its own value
             }
             const bool special = (last && t == tstart) || (b == 0 && t == 0);
+            const bool recompute = (t & mask) >= mask - 1 || t >= n || t < 32;   // qp_pair.cuh: warp-uniform
             for (int l = 0; l < 32; ++l) {
                 int i = t - l; bool active = i >= 0 && i <= n;
                 bool resc = ((t & mask) == mask) || (i == n);
                 int xcode = (i >= 1 && i <= n) ? xs[i - 1] : kSentinel;
                 BwdRun<R, 2> runH; BwdRun<R, GP> runP;
-                H[l].begin(rh[l], resc, runH, range_flag); Pm[l].begin(rp[l], resc, runP, range_flag);
+                const bool zin = l == 31 && !(!last && active);
+                BwdEx<R, 2> qh = rh[l]; BwdEx<R, GP> qp_ = rp[l];
+                if (!recompute) { qh.e = 123456; qp_.e = -123456; }
+                H[l].begin(qh, resc, recompute, zin, runH, range_flag); Pm[l].begin(qp_, resc, recompute, zin, runP, range_flag);
                 int eFh = active ? EH[((size_t)b * T + t) * 32 + l] : 0, eFp = active ? EP[((size_t)b * T + t) * 32 + l] : 0;
                 PScale<R> psh, psp;
                 if ((psh.set(eFh + H[l].e - ez_h, invZh) | psp.set(eFp + Pm[l].e - ez_p, invZp)) && active && b * 32 * C + l * C <= m) range_flag = 1;
