@@ -106,7 +106,8 @@ int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int32_t* h_pai
 /*
  * The hot path. d_seqs: packed residue codes (uint8); d_offsets [k+1]: sequence s is
  * d_seqs[d_offsets[s] .. d_offsets[s+1]); d_pairs [P][2] int32. Steps, all on the device:
- *   a0 schedule (class by stripe width, longest-first order, scratch slots)
+ *   a0 schedule (length classes: short pairs packed one per warp, long pairs split over the warps of a CTA;
+ *      largest-first order, scratch slots)
  *   a1-a4 pair-HMM and partition-function forward and backward
  *   a5 combine P = sqrt((P_hmm^2+P_pf^2)/2), a6 threshold + CSR compaction
  *   a7 expected-accuracy (MEA) max-plus DP and d = 1 - A(n,m)/min(n,m)
@@ -129,9 +130,11 @@ int qp_last_launch_count(void);
  */
 void qp_set_profile(int on);
 int qp_get_profile(float ms[4]);
-/* Per stripe class (C = 2(c+1)): start and stop of its pair kernel in ms after the end of the schedule phase,
- * -1 for classes that did not run. Same preconditions as qp_get_profile. */
-int qp_get_profile_classes(float start_ms[8], float stop_ms[8]);
+/* Per scheduling class c (0..7: packed, one warp per pair, stripe width C = 2(c+1); 8..10: split, the warps of a
+ * CTA share one long pair): start and stop of its pair kernel in ms after the end of the schedule phase, -1 for
+ * classes that did not run. Same preconditions as qp_get_profile. */
+#define QP_NUM_CLASSES 11
+int qp_get_profile_classes(float start_ms[QP_NUM_CLASSES], float stop_ms[QP_NUM_CLASSES]);
 
 const char* qp_status_string(int status);
 const char* qp_version(void);

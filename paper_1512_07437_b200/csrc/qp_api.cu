@@ -24,20 +24,18 @@
 namespace qp {
 
 enum : int { kModeCsr = 0, kModeFull = 1, kModeDist = 2 };   // see qp_pair.cuh
-template <typename R, int GP, int C, int MODE> cudaError_t launch_pair(const KArgs<R>& ka, int grid, cudaStream_t st);
-#define QP_DECL_F32(C)                                                                                      \
-    extern template cudaError_t launch_pair<float, 1, C, kModeCsr>(const KArgs<float>&, int, cudaStream_t);  \
-    extern template cudaError_t launch_pair<float, 2, C, kModeCsr>(const KArgs<float>&, int, cudaStream_t);  \
-    extern template cudaError_t launch_pair<float, 1, C, kModeFull>(const KArgs<float>&, int, cudaStream_t); \
-    extern template cudaError_t launch_pair<float, 2, C, kModeFull>(const KArgs<float>&, int, cudaStream_t);
-#define QP_DECL_F64(C)                                                                                        \
-    extern template cudaError_t launch_pair<double, 2, C, kModeFull>(const KArgs<double>&, int, cudaStream_t); \
-    extern template cudaError_t launch_pair<double, 2, C, kModeDist>(const KArgs<double>&, int, cudaStream_t);
-QP_DECL_F32(2) QP_DECL_F32(4) QP_DECL_F32(6) QP_DECL_F32(8) QP_DECL_F32(10) QP_DECL_F32(12) QP_DECL_F32(14) QP_DECL_F32(16)
-QP_DECL_F64(2) QP_DECL_F64(4) QP_DECL_F64(6) QP_DECL_F64(8)
-
-constexpr uint32_t kMaskF32 = 0xff;   // C = 2..16
-constexpr uint32_t kMaskF64 = 0x0f;   // C = 2..8
+template <typename R, int GP, int C, int MODE, int W> cudaError_t launch_pair(const KArgs<R>& ka, int grid, cudaStream_t st);
+#define QP_DECL_F32(C, W)                                                                                      \
+    extern template cudaError_t launch_pair<float, 1, C, kModeCsr, W>(const KArgs<float>&, int, cudaStream_t);  \
+    extern template cudaError_t launch_pair<float, 2, C, kModeCsr, W>(const KArgs<float>&, int, cudaStream_t);  \
+    extern template cudaError_t launch_pair<float, 1, C, kModeFull, W>(const KArgs<float>&, int, cudaStream_t); \
+    extern template cudaError_t launch_pair<float, 2, C, kModeFull, W>(const KArgs<float>&, int, cudaStream_t);
+#define QP_DECL_F64(C, MODE, W) \
+    extern template cudaError_t launch_pair<double, 2, C, MODE, W>(const KArgs<double>&, int, cudaStream_t);
+QP_DECL_F32(2, 1) QP_DECL_F32(4, 1) QP_DECL_F32(6, 1) QP_DECL_F32(8, 1) QP_DECL_F32(10, 1) QP_DECL_F32(12, 1)
+QP_DECL_F32(14, 1) QP_DECL_F32(16, 1) QP_DECL_F32(8, 4) QP_DECL_F32(12, 4) QP_DECL_F32(16, 4)
+QP_DECL_F64(2, kModeFull, 1) QP_DECL_F64(4, kModeFull, 1) QP_DECL_F64(6, kModeFull, 1) QP_DECL_F64(8, kModeFull, 1)
+QP_DECL_F64(8, kModeFull, 8) QP_DECL_F64(2, kModeDist, 8) QP_DECL_F64(4, kModeDist, 8) QP_DECL_F64(8, kModeDist, 8)
 
 // ------------------------------------------------------------------------------------------------------------
 // device-side scheduling kernels
@@ -54,7 +52,7 @@ __global__ void k_check_residues(const uint8_t* __restrict__ seqs, const int64_t
 }
 
 __global__ void k_classify(const int64_t* __restrict__ offs, int k, const int32_t* __restrict__ pairs, int64_t P,
-                           uint32_t cmask, int real_bytes, PairInfo* __restrict__ info, int32_t* __restrict__ rows1,
+                           uint32_t cmask, int fp64, PairInfo* __restrict__ info, int32_t* __restrict__ rows1,
                            int64_t* __restrict__ cells, SchedHeader* h) {
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= P) return;
@@ -77,10 +75,10 @@ __global__ void k_classify(const int64_t* __restrict__ offs, int k, const int32_
             pi.n = (int)n;
             pi.m = (int)m;
             int nb;
-            const int c = choose_class((int)m + 1, cmask, &nb);
+            const int c = choose_class((int)n, (int)m + 1, cmask, fp64 != 0, &nb);
             pi.cls = (int16_t)c;
             pi.nb = (int16_t)nb;
-            pi.bin = bin_of((uint64_t)slot_bytes((int)n, 2 * (c + 1), nb, real_bytes));
+            pi.bin = bin_of((uint64_t)slot_bytes((int)n, class_C(c, fp64 != 0), nb, fp64 ? 8 : 4));
             atomicAdd(&h->hist[c][pi.bin], 1u);
         }
     }
@@ -343,10 +341,15 @@ static Layout make_layout(int64_t P, int64_t nnz_cap, bool dense, int64_t max_sl
     return L;
 }
 
-static int max_warps(int cls, bool fp64, int sms) { return sms * ctas_per_sm(2 * (cls + 1), fp64) * kWarpsPerCta; }
+// scratch slots (= pairs in flight) a class can use: one per warp (packed) or per CTA (split)
+static int max_units(int cls, bool fp64, int sms) {
+    const int C = class_C(cls, fp64), W = class_W(cls, fp64);
+    return C == 0 ? 0 : sms * ctas_per_sm(C, W, fp64) * units_per_cta(W);
+}
+static int class_grid(int cls, bool fp64, int sms) { return sms * ctas_per_sm(class_C(cls, fp64), class_W(cls, fp64), fp64); }
 static int64_t total_max_slots(int sms) {
     int64_t s = 0;
-    for (int c = 0; c < kNumClasses; ++c) s += max_warps(c, false, sms);
+    for (int c = 0; c < kNumClasses; ++c) s += std::max(max_units(c, false, sms), max_units(c, true, sms));
     return s;
 }
 
@@ -420,24 +423,36 @@ template <typename R> static int fill_kargs(const qp_params* prm, KArgs<R>& ka) 
 
 static int launch_class_f32(int gp, bool full, int cls, const KArgs<float>& ka, int grid, cudaStream_t st) {
     cudaError_t e = cudaErrorInvalidValue;
-#define QP_CASE(C)                                                                                            \
-    case C / 2 - 1:                                                                                           \
-        if (full) e = gp == 1 ? launch_pair<float, 1, C, kModeFull>(ka, grid, st) : launch_pair<float, 2, C, kModeFull>(ka, grid, st); \
-        else e = gp == 1 ? launch_pair<float, 1, C, kModeCsr>(ka, grid, st) : launch_pair<float, 2, C, kModeCsr>(ka, grid, st);        \
+#define QP_CASE(CLS, C, W)                                                                                          \
+    case CLS:                                                                                                       \
+        if (full) e = gp == 1 ? launch_pair<float, 1, C, kModeFull, W>(ka, grid, st) : launch_pair<float, 2, C, kModeFull, W>(ka, grid, st); \
+        else e = gp == 1 ? launch_pair<float, 1, C, kModeCsr, W>(ka, grid, st) : launch_pair<float, 2, C, kModeCsr, W>(ka, grid, st);        \
         break;
-    switch (cls) { QP_CASE(2) QP_CASE(4) QP_CASE(6) QP_CASE(8) QP_CASE(10) QP_CASE(12) QP_CASE(14) QP_CASE(16) }
+    switch (cls) {
+        QP_CASE(0, 2, 1) QP_CASE(1, 4, 1) QP_CASE(2, 6, 1) QP_CASE(3, 8, 1) QP_CASE(4, 10, 1) QP_CASE(5, 12, 1)
+        QP_CASE(6, 14, 1) QP_CASE(7, 16, 1) QP_CASE(8, 8, 4) QP_CASE(9, 12, 4) QP_CASE(10, 16, 4)
+    }
 #undef QP_CASE
     ++g_launches;
     return e == cudaSuccess ? QP_OK : QP_ERR_CUDA;
 }
 static int launch_class_f64(bool dist_only, int cls, const KArgs<double>& ka, int grid, cudaStream_t st) {
     cudaError_t e = cudaErrorInvalidValue;
-#define QP_CASE(C)                                                                                                  \
-    case C / 2 - 1:                                                                                                 \
-        e = dist_only ? launch_pair<double, 2, C, kModeDist>(ka, grid, st) : launch_pair<double, 2, C, kModeFull>(ka, grid, st); \
-        break;
-    switch (cls) { QP_CASE(2) QP_CASE(4) QP_CASE(6) QP_CASE(8) }
-#undef QP_CASE
+    if (!dist_only) {
+        switch (cls) {
+            case 0: e = launch_pair<double, 2, 2, kModeFull, 1>(ka, grid, st); break;
+            case 1: e = launch_pair<double, 2, 4, kModeFull, 1>(ka, grid, st); break;
+            case 2: e = launch_pair<double, 2, 6, kModeFull, 1>(ka, grid, st); break;
+            case 3: e = launch_pair<double, 2, 8, kModeFull, 1>(ka, grid, st); break;
+            case 10: e = launch_pair<double, 2, 8, kModeFull, 8>(ka, grid, st); break;
+        }
+    } else {
+        switch (cls) {
+            case 8: e = launch_pair<double, 2, 2, kModeDist, 8>(ka, grid, st); break;
+            case 9: e = launch_pair<double, 2, 4, kModeDist, 8>(ka, grid, st); break;
+            case 10: e = launch_pair<double, 2, 8, kModeDist, 8>(ka, grid, st); break;
+        }
+    }
     ++g_launches;
     return e == cudaSuccess ? QP_OK : QP_ERR_CUDA;
 }
@@ -454,7 +469,7 @@ template <typename R> static void fill_common(KArgs<R>& ka, const uint8_t* d_seq
     ka.slots = ws + L.slots;
     ka.refine_list = (int32_t*)(ws + L.refine_list);
     ka.refine_stride = P;
-    ka.refine_cmask = kMaskF64;
+    ka.refine_cmask = kMaskRefine;
     ka.pair_row_base = out->pair_row_base;
     ka.row_ptr = out->row_ptr;
     ka.pool_col = (int32_t*)(ws + L.pool_col);
@@ -484,7 +499,8 @@ extern "C" void qp_set_profile(int on) {
     if (!on) g_prof_valid = false;
 }
 
-extern "C" int qp_get_profile_classes(float start_ms[8], float stop_ms[8]) {
+extern "C" int qp_get_profile_classes(float start_ms[QP_NUM_CLASSES], float stop_ms[QP_NUM_CLASSES]) {
+    static_assert(QP_NUM_CLASSES == kNumClasses, "qp.h and qp_internal.h disagree");
     if (!g_prof_valid || !start_ms || !stop_ms) return QP_ERR_INVALID_ARG;
     for (int c = 0; c < kNumClasses; ++c) {
         start_ms[c] = stop_ms[c] = -1.0f;
@@ -531,6 +547,7 @@ extern "C" int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int
     const bool fp64 = params->precision == QP_FP64;
     const uint32_t cmask = fp64 ? kMaskF64 : kMaskF32;
     const int rb = fp64 ? 8 : 4;
+    const bool refine = !fp64 && !(params->flags & QP_FLAG_NO_REFINE);
     int sms = kSmAssumed;
     {
         int dev;
@@ -543,31 +560,37 @@ extern "C" int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int
     }
     const Layout L = make_layout(P, nnz_capacity, want_dense != 0, total_max_slots(sms));
     std::vector<std::vector<uint64_t>> sz(kNumClasses);
-    std::vector<uint64_t> sz64;   // fp64 slots of the pairs a refinement pass could see
+    uint64_t sz64[kNumClasses] = {0};   // largest fp64 slot per class among the pairs a refinement pass could see
     for (int64_t p = 0; p < P; ++p) {
         const int x = h_pairs[2 * p], y = h_pairs[2 * p + 1];
         if (x < 0 || y < 0 || x >= k || y >= k || x == y) return QP_ERR_BAD_PAIR;
         const int64_t n = h_offsets[x + 1] - h_offsets[x], m = h_offsets[y + 1] - h_offsets[y];
         if (n < 1 || m < 1 || n > QP_MAX_LEN || m > QP_MAX_LEN) return QP_ERR_EMPTY_SEQUENCE;
         int nb;
-        const int c = choose_class((int)m + 1, cmask, &nb);
-        sz[c].push_back(bin_ub(bin_of((uint64_t)slot_bytes((int)n, 2 * (c + 1), nb, rb))));
-        if (!fp64) {
-            const int c2 = choose_class((int)m + 1, kMaskF64, &nb);
-            sz64.push_back((uint64_t)slot_bytes((int)n, 2 * (c2 + 1), nb, 8));
+        const int c = choose_class((int)n, (int)m + 1, cmask, fp64, &nb);
+        sz[c].push_back(bin_ub(bin_of((uint64_t)slot_bytes((int)n, class_C(c, fp64), nb, rb))));
+        if (refine) {
+            const int c2 = choose_class((int)n, (int)m + 1, kMaskRefine, true, &nb);
+            sz64[c2] = std::max(sz64[c2], (uint64_t)slot_bytes((int)n, class_C(c2, true), nb, 8));
         }
     }
     uint64_t full = 0, minimum = 0;
     for (int c = 0; c < kNumClasses; ++c) {
         std::sort(sz[c].begin(), sz[c].end(), std::greater<uint64_t>());
-        const size_t W = std::min<size_t>(sz[c].size(), (size_t)max_warps(c, fp64, sms));
+        const size_t W = std::min<size_t>(sz[c].size(), (size_t)max_units(c, fp64, sms));
         for (size_t w = 0; w < W; ++w) full += sz[c][w];
         if (!sz[c].empty()) minimum += sz[c][0];
     }
-    // the refinement pass reuses the slot region: make sure its largest slot fits at least once
+    // the refinement pass reuses the slot region: every fp64 class must fit its largest slot at least once
     uint64_t ref_min = 0;
-    for (uint64_t v : sz64) ref_min = std::max(ref_min, v);
+    for (uint64_t v : sz64) ref_min += v;
     minimum = std::max(minimum, ref_min);
+    // ... and, budget permitting, once per resident CTA (capped at 4 GiB: which pairs get re-evaluated is only known
+    // on the device)
+    uint64_t ref_full = 0;
+    for (int c = 0; c < kNumClasses; ++c)
+        if ((kMaskRefine >> c) & 1) ref_full += sz64[c] * (uint64_t)std::min<int64_t>(P, max_units(c, true, sms));
+    full = std::max(full, std::min<uint64_t>(ref_full, 4ull << 30));
     full = std::max(full, minimum);
     const uint64_t need_min = (uint64_t)L.fixed + minimum, need_full = (uint64_t)L.fixed + full;
     if (budget_bytes != 0 && budget_bytes < need_min) {
@@ -613,15 +636,14 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
 
     // ---- a0: schedule, entirely on the device --------------------------------------------------------------
     const uint32_t cmask = fp64 ? kMaskF64 : kMaskF32;
-    const int rb = fp64 ? 8 : 4;
     const int pb = (int)((P + 255) / 256);
     k_check_residues<<<2 * sms, 256, 0, st>>>(d_seqs, d_offsets, k, params->hmm.alphabet, hdr);
-    k_classify<<<pb, 256, 0, st>>>(d_offsets, k, d_pairs, P, cmask, rb, (PairInfo*)(ws + L.info),
+    k_classify<<<pb, 256, 0, st>>>(d_offsets, k, d_pairs, P, cmask, fp64 ? 1 : 0, (PairInfo*)(ws + L.info),
                                    (int32_t*)(ws + L.rows1), dense ? (int64_t*)(ws + L.cells) : nullptr, hdr);
     k_bins<<<1, 32, 0, st>>>(hdr);
     k_scatter<<<pb, 256, 0, st>>>((const PairInfo*)(ws + L.info), P, (int32_t*)(ws + L.order), hdr);
     MaxW mw;
-    for (int c = 0; c < kNumClasses; ++c) mw.w[c] = ((cmask >> c) & 1) ? max_warps(c, fp64, sms) : 0;
+    for (int c = 0; c < kNumClasses; ++c) mw.w[c] = ((cmask >> c) & 1) ? max_units(c, fp64, sms) : 0;
     k_slots<<<1, 1024, 0, st>>>((const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), mw, avail,
                                 (int64_t*)(ws + L.slot_off), hdr);
     k_scan<int32_t><<<1, 1024, 0, st>>>((const int32_t*)(ws + L.rows1), P, out->pair_row_base);
@@ -656,10 +678,10 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
     }
     prof_mark(1, st);
     QP_CUDA(cudaEventRecord(g_ctx.fork, st));
-    for (int c = 0; c < kNumClasses; ++c) {
+    for (int c = kNumClasses - 1; c >= 0; --c) {   // split classes (long pairs) and wide stripes first
         if (!((cmask >> c) & 1)) continue;
         QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
-        const int grid = sms * ctas_per_sm(2 * (c + 1), fp64);
+        const int grid = class_grid(c, fp64, sms);
         prof_class(c, 0, g_ctx.st[c]);
         r = fp64 ? launch_class_f64(false, c, *ka64, grid, g_ctx.st[c])
                  : launch_class_f32(params->pf.n_ins, full_outputs, c, *ka32, grid, g_ctx.st[c]);
@@ -674,14 +696,14 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
     // ---- fp64 re-evaluation of the distance of near-identical pairs ----------------
     if (refine) {
         MaxW64 mw64;
-        for (int c = 0; c < kNumClasses; ++c) mw64.w[c] = ((kMaskF64 >> c) & 1) ? max_warps(c, true, sms) : 0;
+        for (int c = 0; c < kNumClasses; ++c) mw64.w[c] = ((kMaskRefine >> c) & 1) ? max_units(c, true, sms) : 0;
         k_refine_plan<<<1, 32, 0, st>>>(mw64, avail, hdr);
         ++g_launches;
         QP_CUDA(cudaEventRecord(g_ctx.fork, st));
         for (int c = 0; c < kNumClasses; ++c) {
-            if (!((kMaskF64 >> c) & 1)) continue;
+            if (!((kMaskRefine >> c) & 1)) continue;
             QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
-            r = launch_class_f64(true, c, *ka64, sms * ctas_per_sm(2 * (c + 1), true), g_ctx.st[c]);
+            r = launch_class_f64(true, c, *ka64, class_grid(c, true, sms), g_ctx.st[c]);
             if (r) return r;
             QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
             QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));

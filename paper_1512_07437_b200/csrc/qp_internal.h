@@ -6,21 +6,44 @@
 
 namespace qp {
 
-constexpr int kNumClasses = 8;        // stripe widths C = 2,4,...,16 (class c <-> C = 2(c+1))
-constexpr int kWarpsPerCta = 4;
-constexpr int kNumBins = 384;         // size bins: 8 per octave of scratch bytes
-constexpr int kSmAssumed = 148;       // used by the host-only workspace query when no device is visible
-
 #if defined(__CUDACC__)
 #define QP_HD2 __host__ __device__ constexpr inline
 #else
 #define QP_HD2 constexpr inline
 #endif
 
+// Scheduling classes. A class fixes the stripe width C (columns per lane) and the number W of warps that share one
+// pair. W = 1 ("packed"): every warp of a CTA works on a pair of its own, the pair's columns fit one 32*C-column
+// block. W > 1 ("split"): the W warps of a CTA take W neighbouring column blocks of ONE pair and run them as a
+// pipelined anti-diagonal wavefront, block boundaries handed over through shared memory (qp_pair.cuh).
+//   class 0..7  : packed, C = 2(c+1)                       (fp64: only 0..3 exist)
+//   class 8..10 : split,  fp32 (C, W) = (8,4) (12,4) (16,4);  fp64 (C, W) = (2,8) (4,8) (8,8)
+constexpr int kNumClasses = 11;
+constexpr int kNumPacked = 8;
+constexpr int kWarpsPerCta = 4;       // packed classes
+constexpr int kNumBins = 384;         // size bins: 8 per octave of scratch bytes
+constexpr int kSmAssumed = 148;       // used by the host-only workspace query when no device is visible
+
+QP_HD2 int class_C(int c, bool fp64) {
+    if (c < kNumPacked) return (fp64 && c >= 4) ? 0 : 2 * (c + 1);
+    return fp64 ? (c == 8 ? 2 : (c == 9 ? 4 : 8)) : (c == 8 ? 8 : (c == 9 ? 12 : 16));
+}
+QP_HD2 int class_W(int c, bool fp64) { return c < kNumPacked ? 1 : (fp64 ? 8 : 4); }
+QP_HD2 int class_index(int C, int W, bool fp64) {
+    if (W == 1) return C / 2 - 1;
+    return fp64 ? (C == 2 ? 8 : (C == 4 ? 9 : 10)) : (C == 8 ? 8 : (C == 12 ? 9 : 10));
+}
+constexpr uint32_t kMaskF32 = 0x7ff;       // fp32 pass: packed C = 2..16 and the three split classes
+constexpr uint32_t kMaskF64 = 0x40f;       // QP_FP64: packed C = 2..8, split (8,8)
+constexpr uint32_t kMaskRefine = 0x700;    // fp64 distance re-evaluation: split classes only (latency matters)
+
 // resident CTAs per SM the pair kernels are compiled for (register budget via __launch_bounds__)
-constexpr int ctas_per_sm(int C, bool fp64) {
+QP_HD2 int ctas_per_sm(int C, int W, bool fp64) {
+    if (W > 1) return fp64 ? 1 : (C <= 8 ? 3 : 2);
     return fp64 ? (C <= 4 ? 3 : 2) : (C <= 6 ? 4 : (C <= 10 ? 3 : 2));
 }
+// pairs in flight per CTA
+QP_HD2 int units_per_cta(int W) { return W == 1 ? kWarpsPerCta : 1; }
 
 struct alignas(16) PairInfo {
     int64_t xoff, yoff;   // start of the row / column sequence in d_seqs
@@ -55,20 +78,47 @@ QP_HD2 int64_t slot_bytes(int n, int C, int nb, int real_bytes) {
     return (b + 255) & ~(int64_t)255;
 }
 
-// choose (C, nb) for m+1 columns among the allowed stripe widths (bit c set <-> C = 2(c+1) available):
-// minimal padded width nb*32*C, ties -> fewer blocks. Returns class index.
-QP_HD2 int choose_class(int cols, uint32_t cmask, int* nb_out) {
+// choose the class of a pair with n rows and `cols` = m+1 columns among the classes of `mask`:
+//   1. the narrowest packed class whose single block holds all columns (least padding, one warp per pair);
+//   2. else the split class with the shortest pipeline: passes * (rows + 32 * active warps) * (C + per-step overhead
+//      expressed in cells), a pass = W neighbouring blocks;
+//   3. else (no split class allowed) the packed class with the least work, blocks taken one after the other.
+// Returns the class index and the number of 32*C-column blocks.
+QP_HD2 int choose_class(int n, int cols, uint32_t mask, bool fp64, int* nb_out) {
+    constexpr int kStepOverhead = 6;
     int best = -1, best_nb = 0;
-    int64_t best_w = 0;
-    for (int c = 0; c < kNumClasses; ++c) {
-        if (!((cmask >> c) & 1)) continue;
-        int C = 2 * (c + 1);
-        int nb = (cols + 32 * C - 1) / (32 * C);
-        int64_t w = (int64_t)nb * 32 * C;
-        if (best < 0 || w < best_w || (w == best_w && nb < best_nb)) {
+    int64_t best_cost = 0;
+    for (int c = 0; c < kNumPacked; ++c) {
+        const int C = class_C(c, fp64);
+        if (!((mask >> c) & 1) || C == 0) continue;
+        if (cols <= 32 * C) {
+            *nb_out = 1;
+            return c;
+        }
+    }
+    for (int c = kNumPacked; c < kNumClasses; ++c) {
+        if (!((mask >> c) & 1)) continue;
+        const int C = class_C(c, fp64), W = class_W(c, fp64);
+        const int nb = (cols + 32 * C - 1) / (32 * C);
+        const int act = nb < W ? nb : W;
+        const int64_t cost = (int64_t)((nb + W - 1) / W) * (n + 1 + 32 * act) * (C + kStepOverhead);
+        if (best < 0 || cost < best_cost) {
             best = c;
             best_nb = nb;
-            best_w = w;
+            best_cost = cost;
+        }
+    }
+    if (best < 0) {
+        for (int c = 0; c < kNumPacked; ++c) {
+            const int C = class_C(c, fp64);
+            if (!((mask >> c) & 1) || C == 0) continue;
+            const int nb = (cols + 32 * C - 1) / (32 * C);
+            const int64_t cost = (int64_t)nb * (C + kStepOverhead);
+            if (best < 0 || cost < best_cost) {
+                best = c;
+                best_nb = nb;
+                best_cost = cost;
+            }
         }
     }
     *nb_out = best_nb;
@@ -125,7 +175,7 @@ template <typename R> struct KArgs {
     char* slots;
     int32_t* refine_list;        // [kNumClasses][refine_stride] pair indices queued for fp64 re-evaluation
     int64_t refine_stride;
-    uint32_t refine_cmask;       // stripe widths the fp64 kernels exist for
+    uint32_t refine_cmask;       // classes of the fp64 distance re-evaluation
     // outputs
     const int64_t* pair_row_base;
     int32_t* row_ptr;

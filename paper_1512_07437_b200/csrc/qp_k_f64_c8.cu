@@ -1,7 +1,5 @@
-// fp64 pair kernels, stripe width C=8: QP_FP64 mode (all outputs) and the distance-only re-evaluation of
-// near-identical pairs after an fp32 pass
+// fp64 pair kernels, packed class with stripe width C=8: QP_FP64 mode (all outputs)
 #include "qp_kernel.cuh"
 namespace qp {
-template cudaError_t launch_pair<double, 2, 8, kModeFull>(const KArgs<double>&, int, cudaStream_t);
-template cudaError_t launch_pair<double, 2, 8, kModeDist>(const KArgs<double>&, int, cudaStream_t);
+template cudaError_t launch_pair<double, 2, 8, kModeFull, 1>(const KArgs<double>&, int, cudaStream_t);
 }

@@ -1,0 +1,8 @@
+// fp64 pair kernels, split class (C=8, W=8): the distance-only re-evaluation of near-identical pairs after an fp32
+// pass (few pairs, so the 8 warps of a CTA share each of them to cut its latency), and QP_FP64 mode for pairs
+// wider than one packed block
+#include "qp_kernel.cuh"
+namespace qp {
+template cudaError_t launch_pair<double, 2, 8, kModeDist, 8>(const KArgs<double>&, int, cudaStream_t);
+template cudaError_t launch_pair<double, 2, 8, kModeFull, 8>(const KArgs<double>&, int, cudaStream_t);
+}

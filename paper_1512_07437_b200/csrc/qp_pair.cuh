@@ -1,4 +1,5 @@
-// qp_pair.cuh -- one warp takes one sequence pair through the whole hot path:
+// qp_pair.cuh -- one warp (packed classes, W = 1) or the W warps of one CTA (split classes, one column block per
+// warp, pipelined anti-diagonal wavefront) take one sequence pair through the whole hot path:
 //   forward (pair-HMM + partition function, fused)
 //   backward (both models) fused with combine, sparsify, MEA  8(a) a2, a4, a5, a6, a7
 //   per-row entry buffers -> CSR (rows, columns ascending)     8(a) a6
@@ -196,6 +197,36 @@ __device__ __forceinline__ void st_entry_if(void* ptr, float val, int col, bool 
 // entry buffers and row counts are written by one lane and read by another lane of the same warp: read them from L2
 __device__ __forceinline__ float4 ld_cg_f4(const void* p) { return __ldcg((const float4*)p); }
 
+// ---- split pairs: W warps of one CTA share a pair (north_star: "splits long pairs across a CTA by anti-diagonal
+// wavefront"). Warp w takes column block b0+w of the current group of W blocks; the block boundary (the values lane 31
+// hands to lane 0 of the next block forward, lane 0 to lane 31 of the previous block backward) travels through a
+// shared-memory ring of kDepth rows per neighbour pair, guarded by two counters: rows produced (release/acquire)
+// and rows consumed (back-pressure). Every warp runs free; in steady state block w+1 trails block w by 33 steps, so
+// one pass over a group takes rows + 32*(active warps) steps instead of (rows + 32) * blocks.
+template <typename R, int GP, int W> struct CoopShared {
+    static constexpr int kDepth = 32;
+    union Rec {
+        FwdBnd<R, GP> f;
+        BwdBnd<R, GP> b;
+    };
+    Rec ring[W > 1 ? W - 1 : 1][kDepth];   // channel c: between warp c and warp c+1
+    int prod[W], cons[W];
+    R z[2];                                // forward totals (mantissas) and their exponents, from the last block's warp
+    int ez[2];
+    unsigned long long poff;               // CSR staging-pool offset of the pair
+    int ok;
+    int next;                              // next pair index (CTA-wide pull)
+};
+__device__ __forceinline__ int ld_acquire_cta(const int* p) {
+    int v;
+    asm volatile("ld.acquire.cta.shared.s32 %0, [%1];" : "=r"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release_cta(int* p, int v) {
+    asm volatile("st.release.cta.shared.s32 [%0], %1;" ::"r"(smem_u32(p)), "r"(v) : "memory");
+}
+__device__ __forceinline__ void cta_sync() { __syncthreads(); }
+
 // Residue codes of the rows: lane l works on row t-l, so a lane's next row is its neighbour's current one. The code
 // travels with the wavefront by shuffle; only the entering lane (lane 0 forward, lane 31 backward) takes a new
 // code, from a 32-row chunk that the warp loads (coalesced) one chunk ahead of its use.
@@ -203,9 +234,9 @@ __device__ __forceinline__ float4 ld_cg_f4(const void* p) { return __ldcg((const
 // ---------------------------------------------------------------------------------------------------------
 // the pair pipeline
 // ---------------------------------------------------------------------------------------------------------
-template <typename R, int GP, int C, int MODE>
+template <typename R, int GP, int C, int MODE, int W>
 __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2* __restrict__ tab, int p, char* slot,
-                             int lane, FRing& ring) {
+                             int lane, int warp, FRing& ring, CoopShared<R, GP, W>* cs) {
     using V2 = typename Traits<R>::vec2;
     using Acc = typename Traits<R>::acc_t;
     using SL = Slot<R>;
@@ -213,6 +244,9 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
     constexpr int GH = 2;
     constexpr bool kCsr = MODE != kModeDist;
     static_assert(C % 2 == 0, "stripe widths are even (fp32 stores two cells per 16-byte word)");
+    constexpr int kDepth = CoopShared<R, GP, W>::kDepth;
+    constexpr bool kSplit = W > 1;
+    if constexpr (!kSplit) warp = 0;
 
     const PairInfo pi = ka.info[p];
     const int n = pi.n, m = pi.m;
@@ -233,7 +267,14 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
     // =========================================== forward ===================================================
     R zcap_h = R(0), zcap_p = R(0);
     int ez_h = 0, ez_p = 0;
-    for (int b = 0; b < nb; ++b) {
+    for (int b0 = 0; b0 < nb; b0 += W) {
+      if constexpr (kSplit) {   // fresh ring counters for this group of W blocks
+        cta_sync();
+        if (lane == 0) cs->prod[warp] = cs->cons[warp] = 0;
+        cta_sync();
+      }
+      const int b = b0 + warp;
+      if (b < nb) {
         FwdModel<R, GH, C> H;
         FwdModel<R, GP, C> Pm;
         H.init();
@@ -246,8 +287,12 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         }
         const bool last = (b == nb - 1);
         const int tend = n + (last ? lz : 31);
-        const FwdBnd<R, GP>* bin = (const FwdBnd<R, GP>*)((b & 1) ? bnd0 : bnd1);   // written by block b-1
-        FwdBnd<R, GP>* bout = (FwdBnd<R, GP>*)((b & 1) ? bnd1 : bnd0);
+        // boundary columns between groups of W blocks go through the slot (ping-pong by group); inside a group
+        // (split pairs) through the shared-memory rings
+        const int grp = b0 / W;
+        const FwdBnd<R, GP>* bin = (const FwdBnd<R, GP>*)((grp & 1) ? bnd0 : bnd1);   // written by the previous group
+        FwdBnd<R, GP>* bout = (FwdBnd<R, GP>*)((grp & 1) ? bnd1 : bnd0);
+        const bool in_ring = kSplit && warp > 0, out_ring = kSplit && warp < W - 1;
         char* lp = slot + (int64_t)b * blk_bytes + lane * SL::kLaneBytes;   // this lane's F words of step t
         const bool colact = b * 32 * C + lane * C <= m;   // lanes that hold only padding columns store nothing
         // row codes: every lane starts on a row <= 0; lane 0 enters row t+1 at the end of step t
@@ -272,7 +317,17 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             bool zero_in = lane == 0;   // nothing comes in from the left of the first block
             if (b > 0) {                // warp-uniform: lane 0 takes the boundary column of the previous block
                 zero_in = lane == 0 && !active;
-                if (lane == 0 && active) {
+                if (in_ring) {
+                    if (t <= n) {       // warp-uniform: lane 0 is on row t; wait until the left block has produced it
+                        while (ld_acquire_cta(&cs->prod[warp - 1]) <= t) {}
+                        if (lane == 0) {
+                            const FwdBnd<R, GP> rec = cs->ring[warp - 1][t % kDepth].f;
+                            rh = rec.h;
+                            rp = rec.p;
+                            st_release_cta(&cs->cons[warp - 1], t + 1);
+                        }
+                    }
+                } else if (lane == 0 && active) {
                     const FwdBnd<R, GP> rec = ld_volatile(bin + i);
                     rh = rec.h;
                     rp = rec.p;
@@ -320,22 +375,53 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             // exponents: constant over a renormalisation period, recorded on its last step (all lanes: a lane whose
             // last row fell inside the period has kept its exponent since)
             if ((t & mask) == mask || t == tend) *(int2*)(lp + dE) = make_int2(H.e, Pm.e);
-            if (nb > 1 && !last && lane == 31 && active) {
-                bout[i].h = H.ex;
-                bout[i].p = Pm.ex;
+            if (nb > 1 && !last) {
+                if (out_ring) {
+                    const int i31 = t - 31;   // warp-uniform: the row lane 31 has just finished
+                    if (i31 >= 0 && i31 <= n) {
+                        if (i31 >= kDepth)    // back-pressure: the ring entry must have been consumed
+                            while (ld_acquire_cta(&cs->cons[warp]) < i31 - kDepth + 1) {}
+                        if (lane == 31) {
+                            FwdBnd<R, GP>& rec = cs->ring[warp][i31 % kDepth].f;
+                            rec.h = H.ex;
+                            rec.p = Pm.ex;
+                            st_release_cta(&cs->prod[warp], i31 + 1);
+                        }
+                    }
+                } else if (lane == 31 && active) {
+                    bout[i].h = H.ex;
+                    bout[i].p = Pm.ex;
+                }
             }
         }
         if (last) {
             ez_h = H.e;
             ez_p = Pm.e;
+            if constexpr (kSplit) {   // the forward totals live in lane lz of this warp: publish them to the CTA
+                if (lane == lz) {
+                    cs->z[0] = zcap_h;
+                    cs->z[1] = zcap_p;
+                    cs->ez[0] = ez_h;
+                    cs->ez[1] = ez_p;
+                }
+            }
         }
         if (nb > 1) __syncwarp();   // lane 31's boundary column must be visible to lane 0 of the next block
+      }
     }
     // Z = Zm * 2^eZ with Zm in [1,2); every lane gets a copy
-    zcap_h = __shfl_sync(kFull, zcap_h, lz);
-    zcap_p = __shfl_sync(kFull, zcap_p, lz);
-    ez_h = __shfl_sync(kFull, ez_h, lz);
-    ez_p = __shfl_sync(kFull, ez_p, lz);
+    if constexpr (kSplit) {
+        cta_sync();   // also orders the boundary column of the last group's writes before the backward reads
+        zcap_h = cs->z[0];
+        zcap_p = cs->z[1];
+        ez_h = cs->ez[0];
+        ez_p = cs->ez[1];
+    } else {
+        zcap_h = __shfl_sync(kFull, zcap_h, lz);
+        zcap_p = __shfl_sync(kFull, zcap_p, lz);
+        ez_h = __shfl_sync(kFull, ez_h, lz);
+        ez_p = __shfl_sync(kFull, ez_p, lz);
+    }
     {
         int kh = expo(zcap_h), kp = expo(zcap_p);
         if (kh == kZeroExp || kp == kZeroExp) {   // total underflow: weights outside the supported range
@@ -367,7 +453,14 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
     int ezb_h = 0, ezb_p = 0;
     int nnz_lane = 0;
     Acc mea = 0;
-    for (int b = nb - 1; b >= 0; --b) {
+    for (int b0 = ((nb - 1) / W) * W; b0 >= 0; b0 -= W) {
+      if constexpr (kSplit) {   // fresh ring counters for this group of W blocks
+        cta_sync();
+        if (lane == 0) cs->prod[warp] = cs->cons[warp] = 0;
+        cta_sync();
+      }
+      const int b = b0 + warp;
+      if (b < nb) {
         BwdModel<R, GH, C> H;
         BwdModel<R, GP, C> Pm;
         H.init();
@@ -383,8 +476,10 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         Acc Adin = 0, exA = 0;
         const bool last = (b == nb - 1);
         const int tstart = n + (last ? lz : 31);
-        const BwdBnd<R, GP>* bin = (const BwdBnd<R, GP>*)((b & 1) ? bnd0 : bnd1);   // written by block b+1
-        BwdBnd<R, GP>* bout = (BwdBnd<R, GP>*)((b & 1) ? bnd1 : bnd0);
+        const int grp = b0 / W;
+        const BwdBnd<R, GP>* bin = (const BwdBnd<R, GP>*)((grp & 1) ? bnd0 : bnd1);   // written by the next group
+        BwdBnd<R, GP>* bout = (BwdBnd<R, GP>*)((grp & 1) ? bnd1 : bnd0);
+        const bool in_ring = kSplit && warp < W - 1, out_ring = kSplit && warp > 0;
         const int jbase = b * 32 * C + lane * C;
         const bool colact = jbase <= m;   // lanes that hold only padding columns: nothing was stored for them
         // row codes: lane l starts on row tstart-l; lane 31 enters row t-32 at the end of step t
@@ -447,7 +542,20 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             bool zero_in = lane == 31;   // nothing comes in from the right of the last block
             if (!last) {                 // warp-uniform: lane 31 takes the boundary column of the next block
                 zero_in = lane == 31 && !active;
-                if (lane == 31 && active) {
+                if (in_ring) {
+                    const int i31 = t - 31;   // warp-uniform: the row lane 31 is on; rows arrive in the order n, n-1, ...
+                    if (i31 >= 0 && i31 <= n) {
+                        const int seq = n - i31;
+                        while (ld_acquire_cta(&cs->prod[warp]) <= seq) {}
+                        if (lane == 31) {
+                            const BwdBnd<R, GP> rec = cs->ring[warp][seq % kDepth].b;
+                            rh = rec.h;
+                            rp = rec.p;
+                            rA = rec.A;
+                            st_release_cta(&cs->cons[warp], seq + 1);
+                        }
+                    }
+                } else if (lane == 31 && active) {
                     const BwdBnd<R, GP> rec = ld_volatile(bin + i);
                     rh = rec.h;
                     rp = rec.p;
@@ -536,16 +644,32 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     nnz_lane += ecnt;
                 }
             }
-            if (nb > 1 && b > 0 && lane == 0 && active) {
-                bout[i].h = H.ex;
-                bout[i].p = Pm.ex;
-                bout[i].A = exA;
+            if (nb > 1 && b > 0) {
+                if (out_ring) {
+                    if (t <= n) {   // warp-uniform: lane 0 has just finished row t
+                        const int seq = n - t;
+                        if (seq >= kDepth)
+                            while (ld_acquire_cta(&cs->cons[warp - 1]) < seq - kDepth + 1) {}
+                        if (lane == 0) {
+                            BwdBnd<R, GP>& rec = cs->ring[warp - 1][seq % kDepth].b;
+                            rec.h = H.ex;
+                            rec.p = Pm.ex;
+                            rec.A = exA;
+                            st_release_cta(&cs->prod[warp - 1], seq + 1);
+                        }
+                    }
+                } else if (lane == 0 && active) {
+                    bout[i].h = H.ex;
+                    bout[i].p = Pm.ex;
+                    bout[i].A = exA;
+                }
             }
         }
         if (b == 0) mea = An[0];   // lane 0 holds A'(0,0) = A(n,m)
         if (nb > 1) __syncwarp();
+      }
     }
-    mea = __shfl_sync(kFull, mea, 0);
+    mea = __shfl_sync(kFull, mea, 0);   // split pairs: only warp 0 (block 0) holds it, and only warp 0 uses it
     const double dist = 1.0 - (double)mea / (ldexp(1.0, sbits) * (double)minnm);
 
     if (__any_sync(kFull, range_flag)) {
@@ -553,23 +677,23 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
     }
 
     // ---- distance d = 1 - A(n,m)/min(n,m), both orientations; near-identical pairs are queued for fp64 --------
-    if (lane == 0) {
+    if (lane == 0 && warp == 0) {
         const int xi = ka.pairs[2 * (int64_t)p], yi = ka.pairs[2 * (int64_t)p + 1];
         ka.dist[(int64_t)xi * ka.k + yi] = (float)dist;
         ka.dist[(int64_t)yi * ka.k + xi] = (float)dist;
         if (MODE != kModeDist && sizeof(R) == 4 && (float)dist < ka.refine_below) {
             int nbd;
-            const int c64 = choose_class(m + 1, ka.refine_cmask, &nbd);
+            const int c64 = choose_class(n, m + 1, ka.refine_cmask, true, &nbd);
             const int pos = atomicAdd(&ka.hdr->refine_count[c64], 1);
             ka.refine_list[(int64_t)c64 * ka.refine_stride + pos] = p;
             atomicMax(&ka.hdr->refine_slot_bytes[c64],
-                      (unsigned long long)slot_bytes(n, 2 * (c64 + 1), nbd, 8));
+                      (unsigned long long)slot_bytes(n, class_C(c64, true), nbd, 8));
         }
     }
 
     // ---- logZ (tests): undo the background normalisation, ln Z = ln2*(log2 Zm + eZ) + sum lx ----------------
     if constexpr (MODE == kModeFull) {
-        if (ka.logZ != nullptr) {
+        if (ka.logZ != nullptr && warp == 0) {
             double ch = 0.0, cp = 0.0;
             for (int q = lane; q < n; q += 32) { ch += ka.lx_h[xs[q]]; cp += ka.lx_p[xs[q]]; }
             for (int q = lane; q < m; q += 32) { ch += ka.lx_h[ys[q]]; cp += ka.lx_p[ys[q]]; }
@@ -596,7 +720,57 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
     // ---- CSR: row counts -> row_ptr, entry buffers -> staging pool, rows ascending, columns ascending -----------
     // 32 rows at a time, one row per lane. A row's entries sit in its buffer(s) highest column first; blocks are
     // walked in ascending order and every buffer backwards, four entries (one 32-byte sector) per load pair.
-    if constexpr (kCsr) {
+    if constexpr (kCsr && kSplit) {
+        // split pairs: warp 0 turns the row counts into row_ptr and reserves the pool range, then all W warps
+        // move the entry buffers, 32 rows per warp at a time
+        cta_sync();   // entry buffers and row counts were written by all warps of the CTA
+        int32_t* rp = ka.row_ptr + ka.pair_row_base[p];
+        const int32_t* rowcnt = (const int32_t*)(slot + rowcnt_offset(n, C, nb, RB));
+        if (warp == 0) {
+            int running = 0;
+            for (int i0 = 1; i0 <= n; i0 += 32) {
+                const int i = i0 + lane;
+                const bool valid = i <= n;
+                int c = 0;
+                for (int b = 0; b < nb; ++b) c += valid ? __ldcg(rowcnt + (int64_t)b * (n + 1) + i) : 0;
+                const int ex = warp_excl_scan(c, lane);
+                if (valid) rp[i - 1] = running + ex;
+                running += __shfl_sync(kFull, ex + c, 31);
+            }
+            if (lane == 0) {
+                const unsigned long long poff = atomicAdd(&ka.hdr->pool_cursor, (unsigned long long)running);
+                const bool ok = (long long)(poff + (unsigned long long)running) <= (long long)ka.pool_cap;
+                if (!ok && atomicCAS(&ka.hdr->status[0], 0, -6 /*QP_ERR_NNZ_CAPACITY*/) == 0) ka.hdr->status[1] = p;
+                cs->poff = poff;
+                cs->ok = ok;
+                rp[n] = running;
+                ka.nnz[p] = running;
+                ka.pool_off[p] = (int64_t)poff;
+            }
+        }
+        cta_sync();
+        if (cs->ok) {
+            int32_t* pcol = ka.pool_col + cs->poff;
+            float* pval = ka.pool_val + cs->poff;
+            for (int i0 = 1 + 32 * warp; i0 <= n; i0 += 32 * W) {
+                const int i = i0 + lane;
+                if (i > n) continue;
+                int d = __ldcg(rp + i - 1);
+                for (int b = 0; b < nb; ++b) {
+                    const int cb = __ldcg(rowcnt + (int64_t)b * (n + 1) + i);
+                    const char* buf = slot + (int64_t)b * blk_bytes + (int64_t)(i + 32) * stride;
+                    for (int g = (cb - 1) >> 2; g >= 0; --g) {
+                        const float4 lo = ld_cg_f4(buf + g * 32), hi = ld_cg_f4(buf + g * 32 + 16);
+                        const int q = 4 * g;
+                        if (q + 3 < cb) { pval[d] = hi.z; pcol[d] = __float_as_int(hi.w); ++d; }
+                        if (q + 2 < cb) { pval[d] = hi.x; pcol[d] = __float_as_int(hi.y); ++d; }
+                        if (q + 1 < cb) { pval[d] = lo.z; pcol[d] = __float_as_int(lo.w); ++d; }
+                        pval[d] = lo.x; pcol[d] = __float_as_int(lo.y); ++d;
+                    }
+                }
+            }
+        }
+    } else if constexpr (kCsr) {
         __syncwarp();   // entry buffers and row counts were written by other lanes of this warp
         const int nnz = warp_sum(nnz_lane);
         unsigned long long poff = 0;

@@ -95,8 +95,11 @@ def test_edge_lengths_and_ragged_tiles(default_params, precision):
     _compare(fam, pairs, default_params, res, run, **tol)
 
 
-def test_long_skewed_pairs_multi_block(default_params):
-    """configs[4]-style skew: multi-block columns (m > 512), 20 x 1500 and 1500 x 20, a 700 x 900 pair."""
+@pytest.mark.parametrize("precision", ["fp32", "fp64"])
+def test_long_skewed_pairs_split_classes(default_params, precision):
+    """configs[4]-style skew: pairs wider than one packed block go to the split classes (the warps of a CTA share
+    the pair). 700 x 900 / 900 x 700 (3-4 blocks), 20 x 1500 and 1500 x 20, and 2500 columns = more blocks than
+    warps (two passes, boundary column through the scratch slot)."""
     qp = _qp()
     rng = np.random.default_rng(4)
     q = inputs.background()
@@ -105,11 +108,35 @@ def test_long_skewed_pairs_multi_block(default_params):
     hit = rng.random(900) < 0.3
     mut[hit] = rng.choice(20, size=int(hit.sum()), p=q)
     fam = inputs.pack([base, mut[100:800], rng.integers(0, 20, size=20).astype(np.uint8),
-                       rng.integers(0, 20, size=1500).astype(np.uint8)])
-    pairs = np.array([[0, 1], [1, 0], [2, 3], [3, 2], [0, 3], [2, 1]], dtype=np.int32)
+                       rng.integers(0, 20, size=1500).astype(np.uint8), rng.choice(20, size=2500, p=q).astype(np.uint8),
+                       rng.choice(20, size=45, p=q).astype(np.uint8)])
+    pairs = np.array([[0, 1], [1, 0], [2, 3], [3, 2], [0, 3], [2, 1], [5, 4], [4, 5], [1, 4]], dtype=np.int32)
+    run = orc.Run(default_params, fam, pairs, keep_dense=True)
+    res = qp.run_family(fam, pairs, default_params, precision=precision, want_dense=True, want_logZ=True)
+    tol = dict(p_atol=1e-7, d_rtol=1e-6, logz_rtol=1e-11) if precision == "fp64" else {}
+    _compare(fam, pairs, default_params, res, run, **tol)
+
+
+def test_near_identical_long_pairs_refined(default_params):
+    """near-identical pairs (d < 0.25) of lengths 300 / 600 / 1100: the fp64 distance re-evaluation runs in the split
+    fp64 classes (2,8), (4,8), (8,8)."""
+    qp = _qp()
+    rng = np.random.default_rng(8)
+    q = inputs.background()
+    seqs = []
+    for L in (300, 600, 1100):
+        a = rng.choice(20, size=L, p=q).astype(np.uint8)
+        b = a.copy()
+        hit = rng.random(L) < 0.05
+        b[hit] = rng.choice(20, size=int(hit.sum()), p=q)
+        seqs += [a, np.delete(b, slice(L // 2, L // 2 + 3))]
+    fam = inputs.pack(seqs)
+    pairs = np.array([[0, 1], [1, 0], [2, 3], [3, 2], [4, 5], [5, 4]], dtype=np.int32)
     run = orc.Run(default_params, fam, pairs, keep_dense=True)
     res = qp.run_family(fam, pairs, default_params, precision="fp32", want_dense=True, want_logZ=True)
     _compare(fam, pairs, default_params, res, run)
+    assert int(res.status[3].item()) == len(pairs)
+    assert float(run.dist.max()) < 0.25
 
 
 def test_generic_models_g1_hmm_g2_pf():
