@@ -75,7 +75,7 @@ __global__ void k_classify(const int64_t* __restrict__ offs, int k, const int32_
             pi.n = (int)n;
             pi.m = (int)m;
             int nb;
-            const int c = choose_class((int)n, (int)m + 1, cmask, fp64 != 0, &nb);
+            const int c = choose_class((int)n, (int)m + 1, cmask, fp64 != 0, &nb);   // never -1: the masks hold split classes
             pi.cls = (int16_t)c;
             pi.nb = (int16_t)nb;
             pi.bin = bin_of((uint64_t)slot_bytes((int)n, class_C(c, fp64 != 0), nb, fp64 ? 8 : 4));

@@ -82,8 +82,8 @@ QP_HD2 int64_t slot_bytes(int n, int C, int nb, int real_bytes) {
 //   1. the narrowest packed class whose single block holds all columns (least padding, one warp per pair);
 //   2. else the split class with the shortest pipeline: passes * (rows + 32 * active warps) * (C + per-step overhead
 //      expressed in cells), a pass = W neighbouring blocks;
-//   3. else (no split class allowed) the packed class with the least work, blocks taken one after the other.
-// Returns the class index and the number of 32*C-column blocks.
+// Returns the class index (-1 if the mask holds no class that can take the pair: packed classes never take more than
+// one block) and the number of 32*C-column blocks.
 QP_HD2 int choose_class(int n, int cols, uint32_t mask, bool fp64, int* nb_out) {
     constexpr int kStepOverhead = 6;
     int best = -1, best_nb = 0;
@@ -106,19 +106,6 @@ QP_HD2 int choose_class(int n, int cols, uint32_t mask, bool fp64, int* nb_out) 
             best = c;
             best_nb = nb;
             best_cost = cost;
-        }
-    }
-    if (best < 0) {
-        for (int c = 0; c < kNumPacked; ++c) {
-            const int C = class_C(c, fp64);
-            if (!((mask >> c) & 1) || C == 0) continue;
-            const int nb = (cols + 32 * C - 1) / (32 * C);
-            const int64_t cost = (int64_t)nb * (C + kStepOverhead);
-            if (best < 0 || cost < best_cost) {
-                best = c;
-                best_nb = nb;
-                best_cost = cost;
-            }
         }
     }
     *nb_out = best_nb;

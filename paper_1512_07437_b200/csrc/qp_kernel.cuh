@@ -69,7 +69,7 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
     }
     int idx = unit;   // the first `granted` pairs of the (largest-first) list go to units 0..granted-1; the rest are pulled
     while (idx < count) {
-        process_pair<R, GP, C, MODE, W>(ka, tab, list[idx], slot, lane, warp, ring, cs);
+        process_pair<R, GP, C, MODE, W>(ka, smem_u32(tab), list[idx], slot, lane, warp, ring, cs);
         if constexpr (W == 1) {
             if (lane == 0) idx = atomicAdd(cursor, 1);
             idx = __shfl_sync(kFull, idx, 0);

@@ -137,13 +137,30 @@ template <typename R, int G, int C> struct FwdModel {
         ex.e = 0;
     }
 
-    // start of a step: optional renormalisation (incoming-aware), then bring the neighbour's values to own scale.
-    // The scale factor 2^(rin.e - e) can change only when this lane or its neighbour renormalised, i.e. on the
-    // renormalisation step, on the step after it and while the wavefront ramps up (the caller's `recompute`,
-    // warp-uniform); on the other steps the cached factor is reused and rin.e is not looked at.
+    // Scale bookkeeping, called only on the steps where a scale can change (warp-uniform decision of the caller):
+    //   first       this lane is on its first row (i == 0): its own values are still all zero, so it only has to pick
+    //               the exponent that normalises the values that come in (lane-divergent, a handful of instructions);
+    //   rescale_now periodic renormalisation (warp-uniform): looks at the own values AND the incoming ones, so
+    //               nothing leaves the range before the next renormalisation;
+    //   recompute   the cached factor 2^(rin.e - e) = f1 * f2 is rebuilt (renormalisation step and the step after it:
+    //               that is when this lane's or its neighbour's exponent changes).
     // zero_in: nothing comes in (first lane of the first block): the incoming values count as 0.
-    QP_HD void begin(const FwdEx<R, G>& rin, bool rescale_now, bool recompute, bool zero_in, FwdRun<R, G>& run,
-                     const Weights<R>& w, int& range_flag) {
+    QP_HD void prepare(const FwdEx<R, G>& rin, bool first, bool rescale_now, bool recompute, bool zero_in,
+                       int& range_flag) {
+        if (first) {   // own values are all zero: take the scale that normalises what comes in
+            f1 = R(0);
+            f2 = R(1);
+            rare = false;
+            if (!zero_in) {
+                R mi = qmax(rin.S, rin.M);
+#pragma unroll
+                for (int g = 0; g < G; ++g) mi = qmax(mi, rin.Y[g]);
+                int ki = expo(mi);
+                ki = ki == kZeroExp ? 0 : ki;
+                e = rin.e + ki;
+                f1 = pow2i(-ki, R(0));
+            }
+        }
         if (recompute) {
             if (rescale_now) {
                 R mo = Sdin;
@@ -195,12 +212,17 @@ template <typename R, int G, int C> struct FwdModel {
                 rare = true;
             }
         }
+    }
+
+    // every step: bring the neighbour's values to the own scale. any_rare (warp-uniform): some lane of the warp
+    // needs the second factor.
+    QP_HD void load(const FwdEx<R, G>& rin, bool any_rare, FwdRun<R, G>& run, const Weights<R>& w) {
         run.Sdiag = Sdin;
         run.Ml = rin.M * f1;
         Sdin = rin.S * f1;
 #pragma unroll
         for (int g = 0; g < G; ++g) run.Yl[g] = rin.Y[g] * f1;
-        if (rare) {
+        if (any_rare) {
             run.Ml *= f2;
             Sdin *= f2;
 #pragma unroll
@@ -287,9 +309,23 @@ template <typename R, int G, int C> struct BwdModel {
         ex.e = 0;
     }
 
-    // see FwdModel::begin; zero_in: last lane of the last block
-    QP_HD void begin(const BwdEx<R, G>& rin, bool rescale_now, bool recompute, bool zero_in, BwdRun<R, G>& run,
-                     int& range_flag) {
+    // see FwdModel::prepare; first: the lane is on row n; zero_in: last lane of the last block
+    QP_HD void prepare(const BwdEx<R, G>& rin, bool first, bool rescale_now, bool recompute, bool zero_in,
+                       int& range_flag) {
+        if (first) {   // own values are all zero: take the scale that normalises what comes in
+            f1 = R(0);
+            f2 = R(1);
+            rare = false;
+            if (!zero_in) {
+                R mi = rin.TL;
+#pragma unroll
+                for (int g = 0; g < G; ++g) mi = qmax(mi, rin.BY[g]);
+                int ki = expo(mi);
+                ki = ki == kZeroExp ? 0 : ki;
+                e = rin.e + ki;
+                f1 = pow2i(-ki, R(0));
+            }
+        }
         if (recompute) {
             if (rescale_now) {
                 R mo = R(0);
@@ -323,7 +359,7 @@ template <typename R, int G, int C> struct BwdModel {
                 f1 = R(0);
             } else if (d <= 60) {
                 f1 = pow2i(d, R(0));
-            } else {   // rare, see FwdModel::begin
+            } else {   // rare, see FwdModel::prepare
                 R mi = rin.TL;
 #pragma unroll
                 for (int g = 0; g < G; ++g) mi = qmax(mi, rin.BY[g]);
@@ -338,10 +374,13 @@ template <typename R, int G, int C> struct BwdModel {
                 rare = true;
             }
         }
+    }
+
+    QP_HD void load(const BwdEx<R, G>& rin, bool any_rare, BwdRun<R, G>& run) {
         run.Tc = rin.TL * f1;
 #pragma unroll
         for (int g = 0; g < G; ++g) run.BYr[g] = rin.BY[g] * f1;
-        if (rare) {
+        if (any_rare) {
             run.Tc *= f2;
 #pragma unroll
             for (int g = 0; g < G; ++g) run.BYr[g] *= f2;

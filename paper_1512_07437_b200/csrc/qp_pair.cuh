@@ -179,6 +179,18 @@ template <> struct FWord<double> {
     static __device__ __forceinline__ int unit_of(int k) { return k; }
     static __device__ __forceinline__ bool first_of_unit(int) { return true; }
 };
+// one (em_hmm, em_pf) entry of the emission table; explicit shared-space loads keep the generic->shared address
+// conversion out of the step loop
+__device__ __forceinline__ Traits<float>::vec2 lds_em(uint32_t addr, float) {
+    Traits<float>::vec2 v;
+    asm volatile("ld.shared.v2.f32 {%0,%1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ Traits<double>::vec2 lds_em(uint32_t addr, double) {
+    Traits<double>::vec2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
 __device__ __forceinline__ void lds16(float4& v, uint32_t addr) {
     asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
 }
@@ -186,12 +198,13 @@ __device__ __forceinline__ void lds16(double2& v, uint32_t addr) {
     asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
 }
 
-// append a kept posterior to its row's entry buffer: predicated 8-byte store, no branch
-__device__ __forceinline__ void st_entry_if(void* ptr, float val, int col, bool keep) {
+// append a kept posterior to its row's entry buffer and advance the buffer pointer: predicated 8-byte store and
+// predicated 64-bit add, no branch
+__device__ __forceinline__ void st_entry_adv(char*& ptr, float val, int col, bool keep) {
     asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %3, 0;\n\t@p st.global.v2.b32 [%0], {%1, %2};\n\t}"
-        :
-        : "l"(ptr), "r"(__float_as_int(val)), "r"(col), "r"((int)keep)
+        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %3, 0;\n\t@p st.global.v2.b32 [%0], {%1, %2};\n\t@p add.s64 %0, %0, 8;\n\t}"
+        : "+l"(ptr)
+        : "r"(__float_as_int(val)), "r"(col), "r"((int)keep)
         : "memory");
 }
 // entry buffers and row counts are written by one lane and read by another lane of the same warp: read them from L2
@@ -235,8 +248,8 @@ __device__ __forceinline__ void cta_sync() { __syncthreads(); }
 // the pair pipeline
 // ---------------------------------------------------------------------------------------------------------
 template <typename R, int GP, int C, int MODE, int W>
-__device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2* __restrict__ tab, int p, char* slot,
-                             int lane, int warp, FRing& ring, CoopShared<R, GP, W>* cs) {
+__device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared address of the emission table*/, int p,
+                             char* slot, int lane, int warp, FRing& ring, CoopShared<R, GP, W>* cs) {
     using V2 = typename Traits<R>::vec2;
     using Acc = typename Traits<R>::acc_t;
     using SL = Slot<R>;
@@ -250,7 +263,9 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
 
     const PairInfo pi = ka.info[p];
     const int n = pi.n, m = pi.m;
-    const int nb = (m + 1 + 32 * C - 1) / (32 * C);   // column blocks (column 0 included)
+    // column blocks (column 0 included); a packed class only takes pairs that fit one block (choose_class)
+    const int nb = kSplit ? (m + 1 + 32 * C - 1) / (32 * C) : 1;
+    constexpr int kEm = (int)sizeof(V2);
     const uint8_t* __restrict__ xs = ka.seqs + pi.xoff;
     const uint8_t* __restrict__ ys = ka.seqs + pi.yoff;
     constexpr int stride = (int)step_stride(C, RB);
@@ -279,14 +294,15 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         FwdModel<R, GP, C> Pm;
         H.init();
         Pm.init();
-        int ycode[C];
+        int ycode[C];   // byte offset of the column's residue inside a table row
 #pragma unroll
         for (int k = 0; k < C; ++k) {
             int j = b * 32 * C + lane * C + k;
-            ycode[k] = (j >= 1 && j <= m) ? (int)ys[j - 1] : kSentinel;
+            ycode[k] = ((j >= 1 && j <= m) ? (int)ys[j - 1] : kSentinel) * kEm;
         }
         const bool last = (b == nb - 1);
         const int tend = n + (last ? lz : 31);
+        bool rare_h = false, rare_p = false;   // warp-uniform: some lane needs the second scale factor
         // boundary columns between groups of W blocks go through the slot (ping-pong by group); inside a group
         // (split pairs) through the shared-memory rings
         const int grp = b0 / W;
@@ -301,10 +317,14 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         for (int t = 0; t <= tend; ++t, lp += stride) {
             const int i = t - lane;
             const bool active = (unsigned)i <= (unsigned)n;
-            const bool recompute = (t & mask) <= 1 || t < 32 || t > n;   // warp-uniform, see FwdModel::begin
-            FwdEx<R, GH> rh = shfl_up_ex(H.ex, recompute);
-            FwdEx<R, GP> rp = shfl_up_ex(Pm.ex, recompute);
-            const V2* row = tab + xcode * kTabDim;
+            // warp-uniform (FwdModel::prepare): lanes enter their first row while t < 32; scales change on the
+            // renormalisation step and the step after it; lane 0 of a later block of a split pair loses its input
+            // once it is past row n
+            const bool recompute = (t & mask) <= 1 || (kSplit && b > 0 && t > n);
+            const bool prep = recompute || t < 32;
+            FwdEx<R, GH> rh = shfl_up_ex(H.ex, prep);
+            FwdEx<R, GP> rp = shfl_up_ex(Pm.ex, prep);
+            const uint32_t row = tab + xcode * (kTabDim * kEm);
             {
                 const int feed = __shfl_sync(kFull, chunk, t & 31);
                 const int up = __shfl_up_sync(kFull, xcode, 1);
@@ -333,11 +353,17 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     rp = rec.p;
                 }
             }
-            const bool resc = ((t & mask) == 0) || (i == 0);   // periodic, and on the lane's first row
             FwdRun<R, GH> runH;
             FwdRun<R, GP> runP;
-            H.begin(rh, resc, recompute, zero_in, runH, ka.wh, range_flag);
-            Pm.begin(rp, resc, recompute, zero_in, runP, ka.wp, range_flag);
+            if (prep) {
+                const bool resc = (t & mask) == 0;
+                H.prepare(rh, i == 0, resc, recompute, zero_in, range_flag);
+                Pm.prepare(rp, i == 0, resc, recompute, zero_in, range_flag);
+                rare_h = __any_sync(kFull, H.rare);
+                rare_p = __any_sync(kFull, Pm.rare);
+            }
+            H.load(rh, rare_h, runH, ka.wh);
+            Pm.load(rp, rare_p, runP, ka.wp);
             const bool special = (b == 0 && t == 0) || (last && t == tend);   // warp-uniform
             FwdSpecial sp;
             sp.start = sp.capture = false;
@@ -353,7 +379,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                 [[maybe_unused]] V2 prev;
 #pragma unroll
                 for (int k = 0; k < C; ++k) {
-                    const V2 em = row[ycode[k]];
+                    const V2 em = lds_em(row + ycode[k], R(0));
                     V2 o;
                     o.x = H.template cell<S>(k, em.x, runH, ka.wh, sp, S ? zcap_h : dh);
                     o.y = Pm.template cell<S>(k, em.y, runP, ka.wp, sp, S ? zcap_p : dp);
@@ -471,9 +497,12 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
         for (int k = 0; k < C; ++k) {
             An[k] = 0;
             int j = b * 32 * C + lane * C + k;
-            ycode[k] = (j >= 1 && j <= m) ? (int)ys[j - 1] : kSentinel;
+            ycode[k] = ((j >= 1 && j <= m) ? (int)ys[j - 1] : kSentinel) * kEm;
         }
         Acc Adin = 0, exA = 0;
+        bool rare_h = false, rare_p = false;   // warp-uniform, see the forward loop
+        PScale<R> psh, psp;                    // posterior scale of this lane: changes only when an exponent does
+        psh.c = psp.c = R(0);
         const bool last = (b == nb - 1);
         const int tstart = n + (last ? lz : 31);
         const int grp = b0 / W;
@@ -519,16 +548,20 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
             const bool more = t > 0;
             const bool enext = more && (((t - 1) & mask) == mask);   // warp-uniform: step t-1 holds a record
             if (enext) eFn = *(const int2*)(lp - stride + dE);
-            const bool recompute = (t & mask) >= mask - 1 || t >= n || t < 32;   // warp-uniform, see FwdModel::begin
-            BwdEx<R, GH> rh = shfl_dn_ex(H.ex, recompute);
-            BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex, recompute);
+            // warp-uniform (FwdModel::prepare): lanes enter their first row (row n) while t >= n; scales change on the
+            // renormalisation step and the step after it (that is also where the recorded forward exponents change);
+            // lane 31 of an earlier block of a split pair loses its input once it is past row 0
+            const bool recompute = (t & mask) >= mask - 1 || (kSplit && !last && t < 32);
+            const bool prep = recompute || t >= n;
+            BwdEx<R, GH> rh = shfl_dn_ex(H.ex, prep);
+            BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex, prep);
             Acc rA = shfl_dn1(exA);
             if (lane == 31) rA = 0;
             if constexpr (kCsr) {
                 ecnt = shfl_dn1(ecnt);
                 if (lane == 31) ecnt = 0;
             }
-            const V2* row = tab + xcode * kTabDim;
+            const uint32_t row = tab + xcode * (kTabDim * kEm);
             {
                 const int sdn = tstart - t;
                 const int feed = __shfl_sync(kFull, chunk, sdn & 31);
@@ -562,15 +595,20 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     rA = rec.A;
                 }
             }
-            const bool resc = ((t & mask) == mask) || (i == n);
             BwdRun<R, GH> runH;
             BwdRun<R, GP> runP;
-            H.begin(rh, resc, recompute, zero_in, runH, range_flag);
-            Pm.begin(rp, resc, recompute, zero_in, runP, range_flag);
-            PScale<R> psh, psp;
-            const bool bad_h = psh.set(eF.x + H.e - ez_h, invZh);
-            const bool bad_p = psp.set(eF.y + Pm.e - ez_p, invZp);
-            if ((bad_h || bad_p) && active && colact) range_flag = 1;   // padding lanes hold B = 0 at exponent 0
+            if (prep) {
+                const bool resc = (t & mask) == mask;
+                H.prepare(rh, i == n, resc, recompute, zero_in, range_flag);
+                Pm.prepare(rp, i == n, resc, recompute, zero_in, range_flag);
+                rare_h = __any_sync(kFull, H.rare);
+                rare_p = __any_sync(kFull, Pm.rare);
+                const bool bad_h = psh.set(eF.x + H.e - ez_h, invZh);
+                const bool bad_p = psp.set(eF.y + Pm.e - ez_p, invZp);
+                if ((bad_h || bad_p) && active && colact) range_flag = 1;   // padding lanes hold B = 0 at exponent 0
+            }
+            H.load(rh, rare_h, runH);
+            Pm.load(rp, rare_p, runP);
             // this step's F words have landed?
             const uint32_t stg = ring.waited % kStages;
             mbar_wait(ring.mbar + stg * 8, (ring.waited / kStages) & 1);
@@ -598,7 +636,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                         if (FWord<R>::unit_of(k) > 0) lds16(Fn.v, sF + (FWord<R>::unit_of(k) - 1) * 512);
                     }
                     // the two backward recurrences
-                    const V2 em = row[ycode[k]];
+                    const V2 em = lds_em(row + ycode[k], R(0));
                     R zh = R(0), zp = R(0);
                     const R bmh = H.template cell<S>(k, em.x, runH, ka.wh, sp, zh);
                     const R bmp = Pm.template cell<S>(k, em.y, runP, ka.wp, sp, zp);
@@ -619,8 +657,7 @@ __device__ void process_pair(const KArgs<R>& ka, const typename Traits<R>::vec2*
                     Aright = a;
                     if constexpr (kCsr) {
                         const bool keep = P >= ka.tau;
-                        st_entry_if(ep, (float)P, jbase + k - 1, keep);   // 0-based column in y
-                        ep += keep ? 8 : 0;
+                        st_entry_adv(ep, (float)P, jbase + k - 1, keep);   // 0-based column in y
                     }
                     if constexpr (MODE == kModeFull) {
                         const int j = jbase + k;

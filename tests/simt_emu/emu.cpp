@@ -51,6 +51,7 @@ static int emu_pair(const EmuModel& mh, const EmuModel& mp, const uint8_t* xs, i
         for (int l = 0; l < 32; ++l) { H[l].init(); Pm[l].init(); }
         const bool last = b == nb - 1;
         const int tend = n + (last ? lz : 31);
+        bool any_rare_h = false, any_rare_p = false;
         for (int t = 0; t <= tend; ++t) {
             FwdEx<R, 2> rh[32]; FwdEx<R, GP> rp[32];
             for (int l = 0; l < 32; ++l) {
@@ -60,16 +61,25 @@ static int emu_pair(const EmuModel& mh, const EmuModel& mp, const uint8_t* xs, i
                 else { rh[0] = H[0].ex; rp[0] = Pm[0].ex; }   // shfl_up leaves lane 0 its own value; zero_in makes it count as 0
             }
             const bool special = (b == 0 && t == 0) || (last && t == tend);
-            const bool recompute = (t & mask) <= 1 || t < 32 || t > n;   // qp_pair.cuh: warp-uniform
+            // qp_pair.cuh, all warp-uniform: ramp = lanes are entering their first row; recompute = a scale can change
+            const bool ramp = t < 32, recompute = (t & mask) <= 1 || (b > 0 && t > n), prep = ramp || recompute;
+            const bool resc = (t & mask) == 0;
+            if (prep) {
+                any_rare_h = any_rare_p = false;
+                for (int l = 0; l < 32; ++l) {
+                    int i = t - l; bool active = i >= 0 && i <= n;
+                    const bool zin = l == 0 && !(b > 0 && active);
+                    H[l].prepare(rh[l], i == 0, resc, recompute, zin, range_flag); Pm[l].prepare(rp[l], i == 0, resc, recompute, zin, range_flag);
+                    any_rare_h |= H[l].rare; any_rare_p |= Pm[l].rare;
+                }
+            }
             for (int l = 0; l < 32; ++l) {
                 int i = t - l; bool active = i >= 0 && i <= n;
-                bool resc = ((t & mask) == 0) || (i == 0);
                 int xcode = (i >= 1 && i <= n) ? xs[i - 1] : kSentinel;
                 FwdRun<R, 2> runH; FwdRun<R, GP> runP;
-                const bool zin = l == 0 && !(b > 0 && active);
                 FwdEx<R, 2> qh = rh[l]; FwdEx<R, GP> qp_ = rp[l];
-                if (!recompute) { qh.e = 123456; qp_.e = -123456; }   // the kernel does not shuffle the exponents then
-                H[l].begin(qh, resc, recompute, zin, runH, wh, range_flag); Pm[l].begin(qp_, resc, recompute, zin, runP, wp, range_flag);
+                if (!prep) { qh.e = 123456; qp_.e = -123456; }   // the kernel does not shuffle the exponents then
+                H[l].load(qh, any_rare_h, runH, wh); Pm[l].load(qp_, any_rare_p, runP, wp);
                 FwdSpecial sp; sp.start = special && (b == 0 && l == 0 && i == 0); sp.capture = special && (last && l == lz && i == n); sp.kz = kz;
                 for (int k = 0; k < C; ++k) {
                     int j = b * 32 * C + l * C + k;
@@ -104,6 +114,7 @@ static int emu_pair(const EmuModel& mh, const EmuModel& mp, const uint8_t* xs, i
         std::vector<std::vector<Acc>> An(32, std::vector<Acc>(C, 0)); std::vector<Acc> Adin(32, 0), exA(32, 0);
         for (int l = 0; l < 32; ++l) { H[l].init(); Pm[l].init(); }
         const bool last = b == nb - 1; const int tstart = n + (last ? lz : 31);
+        bool any_rare_h = false, any_rare_p = false;
         for (int t = tstart; t >= 0; --t) {
             BwdEx<R, 2> rh[32]; BwdEx<R, GP> rp[32]; Acc rA[32];
             for (int l = 0; l < 32; ++l) {
@@ -113,16 +124,24 @@ static int emu_pair(const EmuModel& mh, const EmuModel& mp, const uint8_t* xs, i
                 else { rh[l] = H[l].ex; rp[l] = Pm[l].ex; rA[l] = 0; }   // shfl_down leaves lane 31 its own value
             }
             const bool special = (last && t == tstart) || (b == 0 && t == 0);
-            const bool recompute = (t & mask) >= mask - 1 || t >= n || t < 32;   // qp_pair.cuh: warp-uniform
+            const bool ramp = t >= n, recompute = (t & mask) >= mask - 1 || (!last && t < 32), prep = ramp || recompute;
+            const bool resc = (t & mask) == mask;
+            if (prep) {
+                any_rare_h = any_rare_p = false;
+                for (int l = 0; l < 32; ++l) {
+                    int i = t - l; bool active = i >= 0 && i <= n;
+                    const bool zin = l == 31 && !(!last && active);
+                    H[l].prepare(rh[l], i == n, resc, recompute, zin, range_flag); Pm[l].prepare(rp[l], i == n, resc, recompute, zin, range_flag);
+                    any_rare_h |= H[l].rare; any_rare_p |= Pm[l].rare;
+                }
+            }
             for (int l = 0; l < 32; ++l) {
                 int i = t - l; bool active = i >= 0 && i <= n;
-                bool resc = ((t & mask) == mask) || (i == n);
                 int xcode = (i >= 1 && i <= n) ? xs[i - 1] : kSentinel;
                 BwdRun<R, 2> runH; BwdRun<R, GP> runP;
-                const bool zin = l == 31 && !(!last && active);
                 BwdEx<R, 2> qh = rh[l]; BwdEx<R, GP> qp_ = rp[l];
-                if (!recompute) { qh.e = 123456; qp_.e = -123456; }
-                H[l].begin(qh, resc, recompute, zin, runH, range_flag); Pm[l].begin(qp_, resc, recompute, zin, runP, range_flag);
+                if (!prep) { qh.e = 123456; qp_.e = -123456; }
+                H[l].load(qh, any_rare_h, runH); Pm[l].load(qp_, any_rare_p, runP);
                 int eFh = active ? EH[((size_t)b * T + t) * 32 + l] : 0, eFp = active ? EP[((size_t)b * T + t) * 32 + l] : 0;
                 PScale<R> psh, psp;
                 if ((psh.set(eFh + H[l].e - ez_h, invZh) | psp.set(eFp + Pm[l].e - ez_p, invZp)) && active && b * 32 * C + l * C <= m) range_flag = 1;
