@@ -32,8 +32,9 @@ template <typename R, int GP, int C, int MODE, int W> cudaError_t launch_pair(co
     extern template cudaError_t launch_pair<float, 2, C, kModeFull, W>(const KArgs<float>&, int, cudaStream_t);
 #define QP_DECL_F64(C, MODE, W) \
     extern template cudaError_t launch_pair<double, 2, C, MODE, W>(const KArgs<double>&, int, cudaStream_t);
-QP_DECL_F32(2, 1) QP_DECL_F32(4, 1) QP_DECL_F32(6, 1) QP_DECL_F32(8, 1) QP_DECL_F32(10, 1) QP_DECL_F32(12, 1)
-QP_DECL_F32(14, 1) QP_DECL_F32(16, 1) QP_DECL_F32(8, 4) QP_DECL_F32(12, 4) QP_DECL_F32(16, 4)
+QP_DECL_F32(2, 1) QP_DECL_F32(3, 1) QP_DECL_F32(4, 1) QP_DECL_F32(5, 1) QP_DECL_F32(6, 1) QP_DECL_F32(7, 1) QP_DECL_F32(8, 1)
+QP_DECL_F32(9, 1) QP_DECL_F32(10, 1) QP_DECL_F32(11, 1) QP_DECL_F32(12, 1) QP_DECL_F32(13, 1) QP_DECL_F32(14, 1)
+QP_DECL_F32(15, 1) QP_DECL_F32(16, 1) QP_DECL_F32(8, 4) QP_DECL_F32(12, 4) QP_DECL_F32(16, 4)
 QP_DECL_F64(2, kModeFull, 1) QP_DECL_F64(4, kModeFull, 1) QP_DECL_F64(6, kModeFull, 1) QP_DECL_F64(8, kModeFull, 1)
 QP_DECL_F64(8, kModeFull, 8) QP_DECL_F64(2, kModeDist, 8) QP_DECL_F64(4, kModeDist, 8) QP_DECL_F64(8, kModeDist, 8)
 
@@ -429,8 +430,9 @@ static int launch_class_f32(int gp, bool full, int cls, const KArgs<float>& ka, 
         else e = gp == 1 ? launch_pair<float, 1, C, kModeCsr, W>(ka, grid, st) : launch_pair<float, 2, C, kModeCsr, W>(ka, grid, st);        \
         break;
     switch (cls) {
-        QP_CASE(0, 2, 1) QP_CASE(1, 4, 1) QP_CASE(2, 6, 1) QP_CASE(3, 8, 1) QP_CASE(4, 10, 1) QP_CASE(5, 12, 1)
-        QP_CASE(6, 14, 1) QP_CASE(7, 16, 1) QP_CASE(8, 8, 4) QP_CASE(9, 12, 4) QP_CASE(10, 16, 4)
+        QP_CASE(0, 2, 1) QP_CASE(1, 3, 1) QP_CASE(2, 4, 1) QP_CASE(3, 5, 1) QP_CASE(4, 6, 1) QP_CASE(5, 7, 1)
+        QP_CASE(6, 8, 1) QP_CASE(7, 9, 1) QP_CASE(8, 10, 1) QP_CASE(9, 11, 1) QP_CASE(10, 12, 1) QP_CASE(11, 13, 1)
+        QP_CASE(12, 14, 1) QP_CASE(13, 15, 1) QP_CASE(14, 16, 1) QP_CASE(15, 8, 4) QP_CASE(16, 12, 4) QP_CASE(17, 16, 4)
     }
 #undef QP_CASE
     ++g_launches;
@@ -441,16 +443,16 @@ static int launch_class_f64(bool dist_only, int cls, const KArgs<double>& ka, in
     if (!dist_only) {
         switch (cls) {
             case 0: e = launch_pair<double, 2, 2, kModeFull, 1>(ka, grid, st); break;
-            case 1: e = launch_pair<double, 2, 4, kModeFull, 1>(ka, grid, st); break;
-            case 2: e = launch_pair<double, 2, 6, kModeFull, 1>(ka, grid, st); break;
-            case 3: e = launch_pair<double, 2, 8, kModeFull, 1>(ka, grid, st); break;
-            case 10: e = launch_pair<double, 2, 8, kModeFull, 8>(ka, grid, st); break;
+            case 2: e = launch_pair<double, 2, 4, kModeFull, 1>(ka, grid, st); break;
+            case 4: e = launch_pair<double, 2, 6, kModeFull, 1>(ka, grid, st); break;
+            case 6: e = launch_pair<double, 2, 8, kModeFull, 1>(ka, grid, st); break;
+            case 17: e = launch_pair<double, 2, 8, kModeFull, 8>(ka, grid, st); break;
         }
     } else {
         switch (cls) {
-            case 8: e = launch_pair<double, 2, 2, kModeDist, 8>(ka, grid, st); break;
-            case 9: e = launch_pair<double, 2, 4, kModeDist, 8>(ka, grid, st); break;
-            case 10: e = launch_pair<double, 2, 8, kModeDist, 8>(ka, grid, st); break;
+            case 15: e = launch_pair<double, 2, 2, kModeDist, 8>(ka, grid, st); break;
+            case 16: e = launch_pair<double, 2, 4, kModeDist, 8>(ka, grid, st); break;
+            case 17: e = launch_pair<double, 2, 8, kModeDist, 8>(ka, grid, st); break;
         }
     }
     ++g_launches;

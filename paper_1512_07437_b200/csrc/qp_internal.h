@@ -16,26 +16,26 @@ namespace qp {
 // pair. W = 1 ("packed"): every warp of a CTA works on a pair of its own, the pair's columns fit one 32*C-column
 // block. W > 1 ("split"): the W warps of a CTA take W neighbouring column blocks of ONE pair and run them as a
 // pipelined anti-diagonal wavefront, block boundaries handed over through shared memory (qp_pair.cuh).
-//   class 0..7  : packed, C = 2(c+1)                       (fp64: only 0..3 exist)
-//   class 8..10 : split,  fp32 (C, W) = (8,4) (12,4) (16,4);  fp64 (C, W) = (2,8) (4,8) (8,8)
-constexpr int kNumClasses = 11;
-constexpr int kNumPacked = 8;
+//   class 0..14  : packed, C = c + 2 = 2..16                (fp64: only C = 2, 4, 6, 8 exist)
+//   class 15..17 : split,  fp32 (C, W) = (8,4) (12,4) (16,4);  fp64 (C, W) = (2,8) (4,8) (8,8)
+constexpr int kNumClasses = 18;
+constexpr int kNumPacked = 15;
 constexpr int kWarpsPerCta = 4;       // packed classes
 constexpr int kNumBins = 384;         // size bins: 8 per octave of scratch bytes
 constexpr int kSmAssumed = 148;       // used by the host-only workspace query when no device is visible
 
 QP_HD2 int class_C(int c, bool fp64) {
-    if (c < kNumPacked) return (fp64 && c >= 4) ? 0 : 2 * (c + 1);
-    return fp64 ? (c == 8 ? 2 : (c == 9 ? 4 : 8)) : (c == 8 ? 8 : (c == 9 ? 12 : 16));
+    if (c < kNumPacked) return (fp64 && (c > 6 || (c & 1))) ? 0 : c + 2;
+    return fp64 ? (c == 15 ? 2 : (c == 16 ? 4 : 8)) : (c == 15 ? 8 : (c == 16 ? 12 : 16));
 }
 QP_HD2 int class_W(int c, bool fp64) { return c < kNumPacked ? 1 : (fp64 ? 8 : 4); }
 QP_HD2 int class_index(int C, int W, bool fp64) {
-    if (W == 1) return C / 2 - 1;
-    return fp64 ? (C == 2 ? 8 : (C == 4 ? 9 : 10)) : (C == 8 ? 8 : (C == 12 ? 9 : 10));
+    if (W == 1) return C - 2;
+    return fp64 ? (C == 2 ? 15 : (C == 4 ? 16 : 17)) : (C == 8 ? 15 : (C == 12 ? 16 : 17));
 }
-constexpr uint32_t kMaskF32 = 0x7ff;       // fp32 pass: packed C = 2..16 and the three split classes
-constexpr uint32_t kMaskF64 = 0x40f;       // QP_FP64: packed C = 2..8, split (8,8)
-constexpr uint32_t kMaskRefine = 0x700;    // fp64 distance re-evaluation: split classes only (latency matters)
+constexpr uint32_t kMaskF32 = 0x3ffff;     // fp32 pass: packed C = 2..16 and the three split classes
+constexpr uint32_t kMaskF64 = 0x20055;     // QP_FP64: packed C = 2, 4, 6, 8, split (8,8)
+constexpr uint32_t kMaskRefine = 0x38000;  // fp64 distance re-evaluation: split classes only (latency matters)
 
 // resident CTAs per SM the pair kernels are compiled for (register budget via __launch_bounds__)
 QP_HD2 int ctas_per_sm(int C, int W, bool fp64) {
@@ -55,7 +55,7 @@ struct alignas(16) PairInfo {
 
 // ---- per-pair scratch slot ---------------------------------------------------------------------------------
 // block b, step t:  F planes | [32] int2 exponents (e_hmm, e_pf), one per lane
-//   fp32: [C/2][32] float4 = (F_hmm, F_pf) of the lane's columns 2u and 2u+1  (every warp access is 512 B contiguous)
+//   fp32: [ceil(C/2)][32] float4 = (F_hmm, F_pf) of the lane's columns 2u and 2u+1  (every warp access is 512 B contiguous)
 //   fp64: [C][32] double2  = (F_hmm, F_pf) of the lane's column k
 // The exponent record of a step is written (and read back) only on the last step of every renormalisation period
 // and on the last step of the block: a lane's exponents cannot change in between.
@@ -63,8 +63,9 @@ struct alignas(16) PairInfo {
 // row i (found by lane l at step i+l, highest columns first) go to the F area of step record i+32, which every
 // lane has consumed before the first of them is written; row i's entry count goes to rowcnt[b][i]. Sparsification
 // therefore adds one step record and 4 bytes per row of scratch.
-QP_HD2 int64_t step_stride(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes + 256; }
-QP_HD2 int64_t exps_offset(int C, int real_bytes) { return (int64_t)C * 32 * 2 * real_bytes; }
+QP_HD2 int f_units(int C, int real_bytes) { return real_bytes == 4 ? (C + 1) / 2 : C; }   // 16-byte words per lane and step
+QP_HD2 int64_t exps_offset(int C, int real_bytes) { return (int64_t)f_units(C, real_bytes) * 512; }
+QP_HD2 int64_t step_stride(int C, int real_bytes) { return exps_offset(C, real_bytes) + 256; }
 QP_HD2 int num_steps(int n) { return n + 33; }
 QP_HD2 int64_t bnd_rec_bytes(int real_bytes) { return 12 * (int64_t)real_bytes + 16; }   // see BndRec in qp_pair.cuh
 // byte offset of rowcnt[nb][n+1] (int32) inside the slot

@@ -126,7 +126,7 @@ template <typename R, int C> __device__ __forceinline__ int exps_delta(int lane)
 // signalled on a per-stage mbarrier (complete_tx::bytes). The lanes then read their words with 16-byte LDS.
 constexpr int kStages = 4;
 template <typename R, int C> struct FUnits {   // 16-byte words per lane and step
-    static constexpr int k = sizeof(R) == 4 ? C / 2 : C;
+    static constexpr int k = f_units(C, (int)sizeof(R));
 };
 template <typename R, int C> struct RingBytes {
     static constexpr int stage = FUnits<R, C>::k * 512;
@@ -170,14 +170,15 @@ template <> struct FWord<float> {
     __device__ __forceinline__ float h(int k) const { return (k & 1) ? v.z : v.x; }
     __device__ __forceinline__ float p(int k) const { return (k & 1) ? v.w : v.y; }
     static __device__ __forceinline__ int unit_of(int k) { return k >> 1; }
-    static __device__ __forceinline__ bool first_of_unit(int k) { return (k & 1) == 1; }   // columns are walked downwards
+    // columns are walked downwards: a unit starts at its odd column, or at the last column of an odd-width stripe
+    static __device__ __forceinline__ bool first_of_unit(int k, int C) { return (k & 1) == 1 || k == C - 1; }
 };
 template <> struct FWord<double> {
     double2 v;
     __device__ __forceinline__ double h(int) const { return v.x; }
     __device__ __forceinline__ double p(int) const { return v.y; }
     static __device__ __forceinline__ int unit_of(int k) { return k; }
-    static __device__ __forceinline__ bool first_of_unit(int) { return true; }
+    static __device__ __forceinline__ bool first_of_unit(int, int) { return true; }
 };
 // one (em_hmm, em_pf) entry of the emission table; explicit shared-space loads keep the generic->shared address
 // conversion out of the step loop
@@ -256,7 +257,6 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
     constexpr int RB = (int)sizeof(R);
     constexpr int GH = 2;
     constexpr bool kCsr = MODE != kModeDist;
-    static_assert(C % 2 == 0, "stripe widths are even (fp32 stores two cells per 16-byte word)");
     constexpr int kDepth = CoopShared<R, GP, W>::kDepth;
     constexpr bool kSplit = W > 1;
     if constexpr (!kSplit) warp = 0;
@@ -386,6 +386,8 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                     if constexpr (sizeof(R) == 4) {
                         if (k & 1) {
                             if (st_on) *(float4*)(lp + (k >> 1) * 512) = make_float4(prev.x, prev.y, o.x, o.y);
+                        } else if (k == C - 1) {   // odd stripe width: the last word is half used
+                            if (st_on) *(float4*)(lp + (k >> 1) * 512) = make_float4(o.x, o.y, 0.f, 0.f);
                         } else {
                             prev = o;
                         }
@@ -631,7 +633,7 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                 lds16(Fn.v, sF + (kUnits - 1) * 512);
 #pragma unroll
                 for (int k = C - 1; k >= 0; --k) {
-                    if (FWord<R>::first_of_unit(k)) {
+                    if (FWord<R>::first_of_unit(k, C)) {
                         Fw = Fn;
                         if (FWord<R>::unit_of(k) > 0) lds16(Fn.v, sF + (FWord<R>::unit_of(k) - 1) * 512);
                     }

@@ -20,7 +20,7 @@ ERR = {"INVALID_ARG": -1, "BAD_RESIDUE": -2, "EMPTY_SEQUENCE": -3, "BAD_PAIR": -
        "NNZ_CAPACITY": -6, "CUDA": -7, "RANGE": -8}
 QP_FP32, QP_FP64 = 0, 1
 FLAG_SYNC_STATUS, FLAG_NO_REFINE = 1, 2
-NUM_CLASSES = 11
+NUM_CLASSES = 18
 
 EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_last_launch_count", "qp_status_string", "qp_version",
            "qp_set_profile", "qp_get_profile", "qp_get_profile_classes"]
@@ -109,7 +109,7 @@ def get_profile_classes():
     r = _lib.qp_get_profile_classes(a, b)
     if r != QP_OK:
         raise QpError(r)
-    names = ["C%d" % (2 * (c + 1)) for c in range(8)] + ["C8xW4", "C12xW4", "C16xW4"]
+    names = ["C%d" % (c + 2) for c in range(15)] + ["C8xW4", "C12xW4", "C16xW4"]
     return [(names[c], round(a[c], 3), round(b[c], 3)) for c in range(NUM_CLASSES) if a[c] >= 0]
 
 

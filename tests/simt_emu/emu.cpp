@@ -196,7 +196,7 @@ static std::vector<Kept> g_csr; static std::vector<int> g_rp;
 extern "C" int emu_run(int fp64, int GP, int C, const EmuModel* mh, const EmuModel* mp, const uint8_t* xs, int n, const uint8_t* ys,
                        int m, double tau, int mask, float* dense, double* logZ2, double* dist) {
 #define RUN(R, G, CC) return emu_pair<R, G, CC>(*mh, *mp, xs, n, ys, m, tau, mask, dense, logZ2, dist, g_csr, g_rp)
-    if (!fp64 && GP == 1) { switch (C) { case 2: RUN(float, 1, 2); case 4: RUN(float, 1, 4); case 8: RUN(float, 1, 8); case 10: RUN(float, 1, 10); case 16: RUN(float, 1, 16); } }
+    if (!fp64 && GP == 1) { switch (C) { case 2: RUN(float, 1, 2); case 3: RUN(float, 1, 3); case 4: RUN(float, 1, 4); case 8: RUN(float, 1, 8); case 9: RUN(float, 1, 9); case 10: RUN(float, 1, 10); case 16: RUN(float, 1, 16); } }
     if (!fp64 && GP == 2) { switch (C) { case 2: RUN(float, 2, 2); case 6: RUN(float, 2, 6); } }
     if (fp64 && GP == 2) { switch (C) { case 2: RUN(double, 2, 2); case 4: RUN(double, 2, 4); case 8: RUN(double, 2, 8); } }
     return -1;

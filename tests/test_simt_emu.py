@@ -35,7 +35,7 @@ def _check(params, x, y, C, fp64=False, GP=None, p_tol=1e-4, d_rtol=1e-4, mask=7
 
 
 @pytest.mark.parametrize("n,m,C", [(1, 1, 2), (1, 2, 2), (2, 1, 2), (3, 63, 2), (40, 31, 2), (64, 65, 4), (90, 127, 4),
-                                   (70, 255, 8), (33, 300, 10), (120, 100, 16)])
+                                   (70, 255, 8), (33, 300, 10), (120, 100, 16), (50, 90, 3), (33, 270, 9)])
 def test_emu_fp32_single_block(default_params, n, m, C):
     rng = np.random.default_rng(n * 1000 + m)
     q = inputs.background()
