@@ -40,7 +40,7 @@ constexpr uint32_t kMaskRefine = 0x38000;  // fp64 distance re-evaluation: split
 // resident CTAs per SM the pair kernels are compiled for (register budget via __launch_bounds__)
 QP_HD2 int ctas_per_sm(int C, int W, bool fp64) {
     if (W > 1) return fp64 ? 1 : (C <= 8 ? 3 : 2);
-    return fp64 ? (C <= 4 ? 3 : 2) : (C <= 6 ? 4 : (C <= 10 ? 3 : 2));
+    return fp64 ? (C <= 4 ? 3 : 2) : (C <= 6 ? 4 : (C <= 12 ? 3 : 2));
 }
 // pairs in flight per CTA
 QP_HD2 int units_per_cta(int W) { return W == 1 ? kWarpsPerCta : 1; }
