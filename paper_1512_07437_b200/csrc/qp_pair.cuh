@@ -838,13 +838,25 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                 for (int b = 0; b < nb; ++b) {
                     const int cb = nb == 1 ? c : __ldcg(rowcnt + (int64_t)b * (n + 1) + i);
                     const char* buf = slot + (int64_t)b * blk_bytes + (int64_t)(i + 32) * stride;
-                    for (int g = (cb - 1) >> 2; g >= 0; --g) {
-                        const float4 lo = ld_cg_f4(buf + g * 32), hi = ld_cg_f4(buf + g * 32 + 16);
+                    int g = (cb - 1) >> 2;
+                    float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo;
+                    if (g >= 0) {
+                        lo = ld_cg_f4(buf + g * 32);
+                        hi = ld_cg_f4(buf + g * 32 + 16);
+                    }
+                    for (; g >= 0; --g) {   // the next group's loads are in flight while this group is stored
+                        float4 nlo = lo, nhi = hi;
+                        if (g > 0) {
+                            nlo = ld_cg_f4(buf + (g - 1) * 32);
+                            nhi = ld_cg_f4(buf + (g - 1) * 32 + 16);
+                        }
                         const int q = 4 * g;
                         if (q + 3 < cb) { pval[d] = hi.z; pcol[d] = __float_as_int(hi.w); ++d; }
                         if (q + 2 < cb) { pval[d] = hi.x; pcol[d] = __float_as_int(hi.y); ++d; }
                         if (q + 1 < cb) { pval[d] = lo.z; pcol[d] = __float_as_int(lo.w); ++d; }
                         pval[d] = lo.x; pcol[d] = __float_as_int(lo.y); ++d;
+                        lo = nlo;
+                        hi = nhi;
                     }
                 }
             }
