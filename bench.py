@@ -48,13 +48,14 @@ def peaks():
 
 
 def ncu_traffic(cfg):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture, if one exists for this config."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram bytes (read + write) of the pair kernels of one step, from the committed ncu captures
+    (profiles/traffic.csv: config,dram_bytes_per_step), or None if this config was not captured."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(p):
-        try:
-            return json.load(open(p)).get(f"cfg{cfg}")
-        except Exception:
-            return None
+        for ln in open(p):
+            f = ln.strip().split(",")
+            if len(f) == 2 and f[0].isdigit() and int(f[0]) == cfg:
+                return float(f[1])
     return None
 
 
@@ -251,7 +252,9 @@ def run_ours(args):
         achieved = ALGO_BYTES_PER_CELL * my_cells / kern_s / 1e9
         roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
                     "traffic": ncu_traffic(args.config), "peak_source": peak_src,
-                    "kernel": "qp::pair_kernel<float,1,C> (8 stripe-width instances, fork..join)",
+                    "kernel": "qp::pair_kernel<float,GP,C,MODE,W>: the 18 class instances of one call (packed C=2..16, split "
+                              "C8/C12/C16 x W4), launched on side streams; duration = fork..join on the caller's stream",
+                    "traffic_note": "dram read+write bytes of those launches from ncu (profiles/traffic.csv), per step",
                     "kernel_ms": prof["pair_kernels"], "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
                     "phases_ms": {k: round(v, 3) for k, v in prof.items()},
                     "canonical_sfu_roofline": {"ops_per_cell": SFU_OPS_PER_CELL, "peak_ops_s": SFU_PEAK,
