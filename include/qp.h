@@ -125,7 +125,8 @@ int qp_last_launch_count(void);
  * record CUDA events on the caller's stream at the phase boundaries (no synchronisation is added). After the
  * caller has synchronised the stream, qp_get_profile fills ms[0..3] with the device time of the last call:
  *   ms[0] schedule (a0), ms[1] pair kernels (a1-a7, all stripe classes, fork to join),
- *   ms[2] fp64 distance refinement, ms[3] CSR placement (scan + copy).
+ *   ms[2] fp64 distance re-evaluation with the CSR placement (scan + copy) running beside it on a side stream
+ *         (QP_FP64 or QP_FLAG_NO_REFINE: the CSR placement alone), ms[3] status word.
  * Returns QP_OK, or QP_ERR_INVALID_ARG if no profiled call has completed.
  */
 void qp_set_profile(int on);

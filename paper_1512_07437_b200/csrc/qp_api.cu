@@ -708,19 +708,25 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
             r = launch_class_f64(true, c, *ka64, class_grid(c, true, sms), g_ctx.st[c]);
             if (r) return r;
             QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
-            QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));
         }
     }
 
-    prof_mark(3, st);
-
-    // ---- CSR placement in pair order ---------------------------------------------------------------------------
-    k_scan<int32_t><<<1, 1024, 0, st>>>((const int32_t*)(ws + L.nnz), P, out->pair_nnz_base);
+    // ---- CSR placement in pair order; it only needs the fp32 pass, so it runs beside the fp64 kernels ------------
+    cudaStream_t ps = refine ? g_ctx.st[0] : st;
+    if (refine) QP_CUDA(cudaStreamWaitEvent(ps, g_ctx.fork, 0));
+    k_scan<int32_t><<<1, 1024, 0, ps>>>((const int32_t*)(ws + L.nnz), P, out->pair_nnz_base);
     if (out->nnz_capacity > 0)
-        k_copy_pool<<<(int)((P + 3) / 4), 128, 0, st>>>((const int32_t*)(ws + L.nnz), (const int64_t*)(ws + L.pool_off),
+        k_copy_pool<<<(int)((P + 3) / 4), 128, 0, ps>>>((const int32_t*)(ws + L.nnz), (const int64_t*)(ws + L.pool_off),
                                                         out->pair_nnz_base, P, (const int32_t*)(ws + L.pool_col),
                                                         (const float*)(ws + L.pool_val), out->nnz_capacity,
                                                         out->col_idx, out->val);
+    if (refine) {
+        QP_CUDA(cudaEventRecord(g_ctx.join[0], ps));
+        QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[0], 0));
+        for (int c = 0; c < kNumClasses; ++c)
+            if ((kMaskRefine >> c) & 1) QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));
+    }
+    prof_mark(3, st);
     k_finish<<<1, 32, 0, st>>>(hdr, out->status);
     g_launches += 3;
     prof_mark(4, st);

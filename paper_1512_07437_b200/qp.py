@@ -94,7 +94,9 @@ def set_profile(on: bool) -> None:
 
 
 def get_profile():
-    """Device ms of the last profiled call: dict(schedule, pair_kernels, refine, csr_place). Sync the stream first."""
+    """Device ms of the last profiled call: dict(schedule, pair_kernels, refine, csr_place); `refine` = the fp64
+    distance re-evaluation AND the CSR placement, which runs beside it; `csr_place` = what is left after their join
+    (the status word). Sync the stream first."""
     ms = (C.c_float * 4)()
     r = _lib.qp_get_profile(ms)
     if r != QP_OK:
