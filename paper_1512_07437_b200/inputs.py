@@ -99,6 +99,14 @@ def default_params(threshold: float = 0.01) -> Params:
     return Params(hmm=default_hmm(), pf=default_pf(), threshold=threshold)
 
 
+def nucleotide_params(threshold: float = 0.01) -> Params:
+    """Nucleotide mode ("HOXD substitution matrices and GTR evolutionary model"): the same two
+    automata over a 4-letter alphabet. The HOXD and GTR tables are not in the container and are not reconstructed;
+    this is the synthetic F81-type model of c-5 with A = 4, a stand-in with the right shape."""
+    return Params(hmm=default_hmm(alphabet=4, lam=0.55), pf=default_pf(alphabet=4, lam=0.45, gap_open=8.0),
+                  threshold=threshold)
+
+
 def random_model(rng: np.random.Generator, n_ins: int, alphabet: int = 4) -> Model:
     """A random symmetric model for parameter-agnostic pins (brute force, fwd=bwd, transposition)."""
     lm = rng.normal(0.0, 1.0, size=(alphabet, alphabet))

@@ -152,6 +152,37 @@ def test_generic_models_g1_hmm_g2_pf():
         _compare(fam, pairs, prm, res, run, **tol)
 
 
+def test_nucleotide_mode_alphabet_4():
+    """PAPER.md:69 nucleotide mode: alphabet 4 through the same kernels (synthetic 4-letter model, the HOXD/GTR
+    tables are not in the container). Related sequences (12 % substitutions, a few indels), lengths 150-600."""
+    qp = _qp()
+    rng = np.random.default_rng(9)
+    prm = inputs.nucleotide_params()
+    q = inputs.background(4)
+    root = rng.choice(4, size=600, p=q).astype(np.uint8)
+    seqs = []
+    for L in (600, 450, 300, 150, 520):
+        s = root.copy()
+        hit = rng.random(600) < 0.12
+        s[hit] = rng.choice(4, size=int(hit.sum()), p=q)
+        cut = int(rng.integers(0, 600 - L + 1))
+        s = s[cut:cut + L]
+        seqs.append(np.delete(s, slice(L // 3, L // 3 + int(rng.integers(1, 6)))))
+    fam = inputs.pack(seqs)
+    pairs = inputs.all_pairs(fam.k)
+    run = orc.Run(prm, fam, pairs, keep_dense=True)
+    for precision in ("fp32", "fp64"):
+        res = qp.run_family(fam, pairs, prm, precision=precision, want_dense=True, want_logZ=True)
+        tol = dict(p_atol=1e-7, d_rtol=1e-6, logz_rtol=1e-11) if precision == "fp64" else {}
+        _compare(fam, pairs, prm, res, run, **tol)
+    # a residue code outside the 4-letter alphabet is an error
+    bad = inputs.Family(seqs=fam.seqs.copy(), offsets=fam.offsets.copy())
+    bad.seqs[3] = 4
+    with pytest.raises(qp.QpError) as ei:
+        qp.run_family(bad, pairs, prm)
+    assert ei.value.code == qp.ERR["BAD_RESIDUE"]
+
+
 def test_error_paths(default_params):
     qp = _qp()
     import torch
