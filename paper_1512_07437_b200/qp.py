@@ -182,6 +182,20 @@ class Result:
                 self.val[nb[0]:nb[1]].cpu().numpy())
 
 
+def alloc_outputs(device, max_pairs, max_rows_total, nnz_capacity, k, dist=None) -> Result:
+    """Output tensors large enough for any call with P <= max_pairs, sum(n_p+1) <= max_rows_total (pass as `reuse=`)."""
+    import torch
+    i64, i32, f32 = torch.int64, torch.int32, torch.float32
+    return Result(
+        pair_row_base=torch.empty(max_pairs + 1, dtype=i64, device=device),
+        pair_nnz_base=torch.empty(max_pairs + 1, dtype=i64, device=device),
+        row_ptr=torch.empty(max(int(max_rows_total), 1), dtype=i32, device=device),
+        col_idx=torch.empty(max(int(nnz_capacity), 1), dtype=i32, device=device),
+        val=torch.empty(max(int(nnz_capacity), 1), dtype=f32, device=device),
+        dist=dist if dist is not None else torch.zeros((k, k), dtype=f32, device=device),
+        dense_P=None, dense_off=None, logZ=None, status=torch.zeros(4, dtype=i32, device=device), code=0, launches=0)
+
+
 def posteriors(d_seqs, d_offsets, k, d_pairs, cparams: CParams, workspace, *, nnz_capacity, h_rows_total,
                want_dense_cells=0, want_logZ=False, dist=None, stream=None, check=True, reuse=None) -> Result:
     """qp_posteriors on torch CUDA tensors. `h_rows_total` = sum over pairs of (n_p + 1) (sizes row_ptr);

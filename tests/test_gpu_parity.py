@@ -214,3 +214,28 @@ def test_error_paths(default_params):
     r = qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp, ws, nnz_capacity=3,
                       h_rows_total=int((L[pairs[:, 0]] + 1).sum()), check=False)
     assert r.code == qp.ERR["NNZ_CAPACITY"] and int(r.pair_nnz_base[-1].item()) == int(run.nnz.sum())
+
+
+def test_host_streamer_matches_single_call(default_params):
+    """stream.HostStreamer (host buffers, pair batches, two in flight) returns the same CSR and distances as one call."""
+    qp = _qp()
+    import torch
+    from paper_1512_07437_b200 import stream
+    fam = inputs.config_family(1)
+    pairs = inputs.all_pairs(fam.k)
+    ref = qp.run_family(fam, pairs, default_params)
+    rb, nb = ref.pair_row_base.cpu().numpy(), ref.pair_nnz_base.cpu().numpy()
+    rp, col, val = ref.row_ptr.cpu().numpy(), ref.col_idx.cpu().numpy(), ref.val.cpu().numpy()
+    hs = stream.HostStreamer(fam, pairs, default_params, batch_cells=1.0e7)     # 8 batches
+    assert len(hs.bounds) - 1 >= 5
+    for rep in range(2):                                                        # the streamer is reusable
+        seen = 0
+        for b in hs.run():
+            assert b.lo == seen
+            seen = b.hi
+            n0, n1 = nb[b.lo], nb[b.hi]
+            assert np.array_equal(b.nnz_base.numpy() - b.nnz_base.numpy()[0], nb[b.lo:b.hi + 1] - n0)
+            assert np.array_equal(b.row_ptr.numpy(), rp[rb[b.lo]:rb[b.hi]])
+            assert np.array_equal(b.col.numpy(), col[n0:n1]) and np.array_equal(b.val.numpy(), val[n0:n1])
+        assert seen == len(pairs)
+        assert torch.equal(hs.dist, ref.dist.cpu())
