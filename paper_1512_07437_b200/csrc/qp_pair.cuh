@@ -32,22 +32,24 @@ __device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(k
 __device__ __forceinline__ int shfl_dn1(int v) { return __shfl_down_sync(kFull, v, 1); }
 __device__ __forceinline__ int64_t shfl_dn1(int64_t v) { return (int64_t)__shfl_down_sync(kFull, (long long)v, 1); }
 
-// the values always travel; the exponent only on the steps where the receiver recomputes its scale factor
-template <typename R, int G> __device__ __forceinline__ FwdEx<R, G> shfl_up_ex(const FwdEx<R, G>& a, bool with_e) {
+// the values always travel; the exponent only on the steps where the receiver rebuilds its scale factor (the caller
+// shuffles it separately, under a warp-uniform test, after ALL unconditional shuffles of the step: one convergence
+// check per step instead of one per group)
+template <typename R, int G> __device__ __forceinline__ FwdEx<R, G> shfl_up_ex(const FwdEx<R, G>& a) {
     FwdEx<R, G> r;
     r.S = shfl_up1(a.S);
     r.M = shfl_up1(a.M);
 #pragma unroll
     for (int g = 0; g < G; ++g) r.Y[g] = shfl_up1(a.Y[g]);
-    r.e = with_e ? shfl_up1(a.e) : 0;   // with_e is warp-uniform
+    r.e = 0;
     return r;
 }
-template <typename R, int G> __device__ __forceinline__ BwdEx<R, G> shfl_dn_ex(const BwdEx<R, G>& a, bool with_e) {
+template <typename R, int G> __device__ __forceinline__ BwdEx<R, G> shfl_dn_ex(const BwdEx<R, G>& a) {
     BwdEx<R, G> r;
     r.TL = shfl_dn1(a.TL);
 #pragma unroll
     for (int g = 0; g < G; ++g) r.BY[g] = shfl_dn1(a.BY[g]);
-    r.e = with_e ? shfl_dn1(a.e) : 0;
+    r.e = 0;
     return r;
 }
 // "nothing comes in": zero values at the receiving lane's own exponent (so that no rescaling is triggered)
@@ -322,12 +324,16 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             // once it is past row n
             const bool recompute = (t & mask) <= 1 || (kSplit && b > 0 && t > n);
             const bool prep = recompute || t < 32;
-            FwdEx<R, GH> rh = shfl_up_ex(H.ex, prep);
-            FwdEx<R, GP> rp = shfl_up_ex(Pm.ex, prep);
+            FwdEx<R, GH> rh = shfl_up_ex(H.ex);
+            FwdEx<R, GP> rp = shfl_up_ex(Pm.ex);
             const uint32_t row = tab + xcode * (kTabDim * kEm);
             {
                 const int feed = __shfl_sync(kFull, chunk, t & 31);
                 const int up = __shfl_up_sync(kFull, xcode, 1);
+                if (prep) {
+                    rh.e = shfl_up1(H.ex.e);
+                    rp.e = shfl_up1(Pm.ex.e);
+                }
                 xcode = lane == 0 ? feed : up;
                 if ((t & 31) == 31) {   // warp-uniform
                     chunk = chunk_next;
@@ -555,19 +561,23 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             // lane 31 of an earlier block of a split pair loses its input once it is past row 0
             const bool recompute = (t & mask) >= mask - 1 || (kSplit && !last && t < 32);
             const bool prep = recompute || t >= n;
-            BwdEx<R, GH> rh = shfl_dn_ex(H.ex, prep);
-            BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex, prep);
+            BwdEx<R, GH> rh = shfl_dn_ex(H.ex);
+            BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex);
             Acc rA = shfl_dn1(exA);
-            if (lane == 31) rA = 0;
-            if constexpr (kCsr) {
-                ecnt = shfl_dn1(ecnt);
-                if (lane == 31) ecnt = 0;
-            }
+            if constexpr (kCsr) ecnt = shfl_dn1(ecnt);
             const uint32_t row = tab + xcode * (kTabDim * kEm);
             {
                 const int sdn = tstart - t;
                 const int feed = __shfl_sync(kFull, chunk, sdn & 31);
                 const int dn = __shfl_down_sync(kFull, xcode, 1);
+                if (prep) {
+                    rh.e = shfl_dn1(H.ex.e);
+                    rp.e = shfl_dn1(Pm.ex.e);
+                }
+                if (lane == 31) rA = 0;
+                if constexpr (kCsr) {
+                    if (lane == 31) ecnt = 0;
+                }
                 xcode = lane == 31 ? feed : dn;
                 if ((sdn & 31) == 31) {   // warp-uniform
                     chunk = chunk_next;
