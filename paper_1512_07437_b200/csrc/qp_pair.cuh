@@ -833,43 +833,52 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
         int32_t* pcol = ka.pool_col + poff;
         float* pval = ka.pool_val + poff;
         const int32_t* rowcnt = (const int32_t*)(slot + rowcnt_offset(n, C, nb, RB));
+        // one block per pair here (packed class). Software pipeline over the 32-row chunks: the row counts are
+        // fetched two chunks ahead and a row's first entry group one chunk ahead, so that a chunk starts with its
+        // loads already landed instead of paying two dependent L2 round trips.
+        auto cnt_at = [&](int i) -> int { return i <= n ? __ldcg(rowcnt + i) : 0; };
+        auto grp_at = [&](int i, int g, float4& lo, float4& hi) {
+            const char* q = slot + (int64_t)(i + 32) * stride + g * 32;
+            lo = ld_cg_f4(q);
+            hi = ld_cg_f4(q + 16);
+        };
         int running = 0;
+        int c_cur = cnt_at(1 + lane), c_nxt = cnt_at(33 + lane);
+        float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo;
+        if (ok && c_cur > 0) grp_at(1 + lane, (c_cur - 1) >> 2, lo, hi);
         for (int i0 = 1; i0 <= n; i0 += 32) {
             const int i = i0 + lane;
             const bool valid = i <= n;
-            int c = 0;
-            for (int b = 0; b < nb; ++b) c += valid ? __ldcg(rowcnt + (int64_t)b * (n + 1) + i) : 0;
+            const int c = c_cur;
+            const int c_nn = cnt_at(i + 64);
+            float4 lo_n = make_float4(0.f, 0.f, 0.f, 0.f), hi_n = lo_n;
+            if (ok && c_nxt > 0) grp_at(i + 32, (c_nxt - 1) >> 2, lo_n, hi_n);
             const int ex = warp_excl_scan(c, lane);
             const int tot = __shfl_sync(kFull, ex + c, 31);
             int d = running + ex;
             if (valid) rp[i - 1] = d;
             running += tot;
             if (ok && valid) {
-                for (int b = 0; b < nb; ++b) {
-                    const int cb = nb == 1 ? c : __ldcg(rowcnt + (int64_t)b * (n + 1) + i);
-                    const char* buf = slot + (int64_t)b * blk_bytes + (int64_t)(i + 32) * stride;
-                    int g = (cb - 1) >> 2;
-                    float4 lo = make_float4(0.f, 0.f, 0.f, 0.f), hi = lo;
-                    if (g >= 0) {
-                        lo = ld_cg_f4(buf + g * 32);
-                        hi = ld_cg_f4(buf + g * 32 + 16);
+                const char* buf = slot + (int64_t)(i + 32) * stride;
+                for (int g = (c - 1) >> 2; g >= 0; --g) {   // the next group's loads are in flight while this one is stored
+                    float4 nlo = lo, nhi = hi;
+                    if (g > 0) {
+                        nlo = ld_cg_f4(buf + (g - 1) * 32);
+                        nhi = ld_cg_f4(buf + (g - 1) * 32 + 16);
                     }
-                    for (; g >= 0; --g) {   // the next group's loads are in flight while this group is stored
-                        float4 nlo = lo, nhi = hi;
-                        if (g > 0) {
-                            nlo = ld_cg_f4(buf + (g - 1) * 32);
-                            nhi = ld_cg_f4(buf + (g - 1) * 32 + 16);
-                        }
-                        const int q = 4 * g;
-                        if (q + 3 < cb) { pval[d] = hi.z; pcol[d] = __float_as_int(hi.w); ++d; }
-                        if (q + 2 < cb) { pval[d] = hi.x; pcol[d] = __float_as_int(hi.y); ++d; }
-                        if (q + 1 < cb) { pval[d] = lo.z; pcol[d] = __float_as_int(lo.w); ++d; }
-                        pval[d] = lo.x; pcol[d] = __float_as_int(lo.y); ++d;
-                        lo = nlo;
-                        hi = nhi;
-                    }
+                    const int q = 4 * g;
+                    if (q + 3 < c) { pval[d] = hi.z; pcol[d] = __float_as_int(hi.w); ++d; }
+                    if (q + 2 < c) { pval[d] = hi.x; pcol[d] = __float_as_int(hi.y); ++d; }
+                    if (q + 1 < c) { pval[d] = lo.z; pcol[d] = __float_as_int(lo.w); ++d; }
+                    pval[d] = lo.x; pcol[d] = __float_as_int(lo.y); ++d;
+                    lo = nlo;
+                    hi = nhi;
                 }
             }
+            c_cur = c_nxt;
+            c_nxt = c_nn;
+            lo = lo_n;
+            hi = hi_n;
         }
         if (lane == 0) {
             rp[n] = running;
