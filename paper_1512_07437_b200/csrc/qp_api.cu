@@ -235,19 +235,22 @@ struct MaxW64 {
 };
 __global__ void k_refine_plan(MaxW64 maxw, int64_t avail, SchedHeader* h) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    unsigned long long used = 0;
+    // one slot for every class that has pairs, then the rest of the slot region class by class
+    unsigned long long base = 0;
     int total = 0;
+    for (int c = 0; c < kNumClasses; ++c)
+        if (h->refine_count[c] > 0) base += h->refine_slot_bytes[c];
+    const bool fits = base <= (unsigned long long)avail;
+    if (!fits) set_status(h, QP_ERR_WORKSPACE_TOO_SMALL, -1);
+    unsigned long long spare = fits ? (unsigned long long)avail - base : 0, used = 0;
     for (int c = 0; c < kNumClasses; ++c) {
         const int cnt = h->refine_count[c];
         int W = 0;
-        if (cnt > 0) {
+        if (cnt > 0 && fits) {
             const unsigned long long sb = h->refine_slot_bytes[c];
-            const long long fit = (long long)(((unsigned long long)avail - used) / sb);
-            W = (int)min((long long)min(cnt, maxw.w[c]), fit);
-            if (W <= 0) {
-                W = 0;
-                set_status(h, QP_ERR_WORKSPACE_TOO_SMALL, -1);
-            }
+            const long long extra = min((long long)min(cnt, maxw.w[c]) - 1, (long long)(spare / sb));
+            W = 1 + (int)max(extra, 0ll);
+            spare -= (unsigned long long)(W - 1) * sb;
             h->refine_slot0[c] = used;
             used += (unsigned long long)W * sb;
             total += cnt;

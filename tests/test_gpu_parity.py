@@ -239,3 +239,43 @@ def test_host_streamer_matches_single_call(default_params):
             assert np.array_equal(b.col.numpy(), col[n0:n1]) and np.array_equal(b.val.numpy(), val[n0:n1])
         assert seen == len(pairs)
         assert torch.equal(hs.dist, ref.dist.cpu())
+
+
+def test_fuzz_random_pairs_models_thresholds():
+    """Seeded fuzz: random lengths (1..400, incl. very skewed pairs), random symmetric models with G in {1,2} for
+    either automaton, alphabets 4 / 12 / 20 / 31, thresholds 0.001 .. 0.2, both precisions."""
+    qp = _qp()
+    rng = np.random.default_rng(20240607)
+    for trial in range(6):
+        A = int(rng.choice([4, 12, 20, 31]))
+        gh, gp = int(rng.integers(1, 3)), int(rng.integers(1, 3))
+        prm = inputs.Params(hmm=inputs.random_model(rng, gh, A), pf=inputs.random_model(rng, gp, A),
+                            threshold=float(rng.choice([0.001, 0.01, 0.05, 0.2])))
+        lens = [int(v) for v in rng.integers(1, 400, size=7)] + [1, 2]
+        fam = inputs.pack([rng.integers(0, A, size=n).astype(np.uint8) for n in lens])
+        pairs = inputs.all_pairs(fam.k)
+        pairs = pairs[rng.permutation(len(pairs))[:20]]
+        flip = rng.random(len(pairs)) < 0.5
+        pairs[flip] = pairs[flip][:, ::-1]
+        run = orc.Run(prm, fam, pairs, keep_dense=True)
+        for precision in ("fp32", "fp64"):
+            res = qp.run_family(fam, pairs, prm, precision=precision, want_dense=True, want_logZ=True)
+            tol = dict(p_atol=1e-7, d_rtol=1e-6, logz_rtol=1e-11) if precision == "fp64" else dict(logz_rtol=5e-6)
+            _compare(fam, pairs, prm, res, run, **tol)
+
+
+def test_workspace_budget_gives_same_result(default_params):
+    """A capped workspace (fewer scratch slots, pairs wait for a slot) changes the schedule, not the result."""
+    qp = _qp()
+    fam = inputs.config_family(1)
+    pairs = inputs.all_pairs(fam.k)
+    full = qp.run_family(fam, pairs, default_params)
+    cp = qp.CParams(default_params)
+    cap = int(full.pair_nnz_base[-1].item()) + 16
+    need = qp.workspace_bytes(fam.offsets, fam.k, pairs, cp, cap)
+    small = qp.run_family(fam, pairs, default_params, nnz_capacity=cap, budget=need // 6)
+    assert qp.workspace_bytes(fam.offsets, fam.k, pairs, cp, cap, budget=need // 6) <= need // 6
+    for name in ("pair_nnz_base", "row_ptr", "dist"):
+        assert (getattr(full, name).cpu().numpy()[: len(getattr(small, name))] == getattr(small, name).cpu().numpy()).all(), name
+    nz = int(full.pair_nnz_base[-1].item())
+    assert (full.col_idx[:nz] == small.col_idx[:nz]).all() and (full.val[:nz] == small.val[:nz]).all()
