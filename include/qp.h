@@ -117,6 +117,21 @@ int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, co
                   const qp_params* params, void* d_workspace, size_t workspace_bytes, const qp_output* out,
                   void* cuda_stream);
 
+/*
+ * Memory-limited mode ("a memory-limited mode ... by decreasing sparsity coefficient"; PAPER.md:192:
+ * memory for the posterior matrices is the limit on the set size). The caller's CSR capacity out->nnz_capacity is the
+ * budget (8 bytes per entry); if the CSR at params->threshold does not fit, the threshold is raised and the pass is
+ * repeated, at most max_passes times in all: tau <- tau * max(1.25, (required / capacity)^1.5) with `required` the
+ * entry count the failed pass reported. On success *tau_used is the threshold the returned CSR was cut at and
+ * *passes the number of passes run; every output is exactly what qp_posteriors returns for that threshold.
+ * Synchronises the stream after every pass (it has to read the status). Returns QP_ERR_NNZ_CAPACITY if max_passes
+ * did not suffice (pair_nnz_base[P] = entries required at the last threshold, *tau_used = that threshold), any other
+ * error of qp_posteriors unchanged. tau_used and passes are HOST pointers (may be NULL).
+ */
+int qp_posteriors_budgeted(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, const int32_t* d_pairs, int64_t P,
+                           const qp_params* params, void* d_workspace, size_t workspace_bytes, const qp_output* out,
+                           void* cuda_stream, int max_passes, double* tau_used, int* passes);
+
 /* Number of kernels the last qp_posteriors call on this thread launched (bench.py's gpu_launches). */
 int qp_last_launch_count(void);
 

@@ -743,3 +743,32 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
     }
     return QP_OK;
 }
+
+extern "C" int qp_posteriors_budgeted(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, const int32_t* d_pairs,
+                                      int64_t P, const qp_params* params, void* d_workspace, size_t workspace_bytes,
+                                      const qp_output* out, void* cuda_stream, int max_passes, double* tau_used,
+                                      int* passes) {
+    if (!params || !out || max_passes < 1) return QP_ERR_INVALID_ARG;
+    qp_params prm = *params;
+    prm.flags |= QP_FLAG_SYNC_STATUS;
+    int r = QP_OK, launches = 0, done = 0;
+    for (int pass = 0; pass < max_passes; ++pass) {
+        r = qp_posteriors(d_seqs, d_offsets, k, d_pairs, P, &prm, d_workspace, workspace_bytes, out, cuda_stream);
+        launches += g_launches;
+        done = pass + 1;
+        if (r != QP_ERR_NNZ_CAPACITY || pass + 1 == max_passes) break;
+        int64_t required = 0;   // the failed pass left the entry count it needs in pair_nnz_base[P]
+        if (cudaMemcpyAsync(&required, out->pair_nnz_base + P, sizeof required, cudaMemcpyDeviceToHost,
+                            (cudaStream_t)cuda_stream) != cudaSuccess ||
+            cudaStreamSynchronize((cudaStream_t)cuda_stream) != cudaSuccess) {
+            r = QP_ERR_CUDA;
+            break;
+        }
+        const double ratio = (double)required / (double)std::max<int64_t>(out->nnz_capacity, 1);
+        prm.threshold = std::min(1.0, prm.threshold * std::max(1.25, std::pow(ratio, 1.5)));
+    }
+    g_launches = launches;
+    if (tau_used) *tau_used = prm.threshold;
+    if (passes) *passes = done;
+    return r;
+}

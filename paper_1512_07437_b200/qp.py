@@ -22,7 +22,7 @@ QP_FP32, QP_FP64 = 0, 1
 FLAG_SYNC_STATUS, FLAG_NO_REFINE = 1, 2
 NUM_CLASSES = 18
 
-EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_last_launch_count", "qp_status_string", "qp_version",
+EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_posteriors_budgeted", "qp_last_launch_count", "qp_status_string", "qp_version",
            "qp_set_profile", "qp_get_profile", "qp_get_profile_classes"]
 
 
@@ -61,6 +61,8 @@ def _load():
     L.qp_posteriors.restype = C.c_int
     L.qp_posteriors.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.POINTER(_Params),
                                 C.c_void_p, C.c_size_t, C.POINTER(_Output), C.c_void_p]
+    L.qp_posteriors_budgeted.restype = C.c_int
+    L.qp_posteriors_budgeted.argtypes = L.qp_posteriors.argtypes + [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int)]
     L.qp_last_launch_count.restype = C.c_int
     L.qp_status_string.restype = C.c_char_p
     L.qp_status_string.argtypes = [C.c_int]
@@ -173,6 +175,8 @@ class Result:
     status: object
     code: int
     launches: int
+    tau_used: float = 0.0   # threshold the CSR was cut at (differs from the requested one in memory-limited mode)
+    passes: int = 1
 
     def csr(self, p):
         """(row_ptr, col, val) of pair p as numpy arrays."""
@@ -197,7 +201,8 @@ def alloc_outputs(device, max_pairs, max_rows_total, nnz_capacity, k, dist=None)
 
 
 def posteriors(d_seqs, d_offsets, k, d_pairs, cparams: CParams, workspace, *, nnz_capacity, h_rows_total,
-               want_dense_cells=0, want_logZ=False, dist=None, stream=None, check=True, reuse=None) -> Result:
+               want_dense_cells=0, want_logZ=False, dist=None, stream=None, check=True, reuse=None,
+               budget_passes=0) -> Result:
     """qp_posteriors on torch CUDA tensors. `h_rows_total` = sum over pairs of (n_p + 1) (sizes row_ptr);
     `want_dense_cells` = sum n_p*m_p to also get the dense matrices (tests), 0 otherwise. `reuse` = a previous
     Result of the same shapes whose output tensors are written again instead of allocating new ones."""
@@ -226,11 +231,16 @@ def posteriors(d_seqs, d_offsets, k, d_pairs, cparams: CParams, workspace, *, nn
         setattr(o, name, v.data_ptr() if v is not None else None)
     o.nnz_capacity = int(nnz_capacity)
     st = stream if stream is not None else torch.cuda.current_stream(dev)
+    tau, passes = C.c_double(float(cparams.s.threshold)), C.c_int(1)
     with torch.cuda.device(dev):
-        code = _lib.qp_posteriors(d_seqs.data_ptr(), d_offsets.data_ptr(), int(k), d_pairs.data_ptr(), P,
-                                  cparams.ref, workspace.data_ptr(), workspace.numel() * workspace.element_size(),
-                                  C.byref(o), C.c_void_p(st.cuda_stream))
+        args = (d_seqs.data_ptr(), d_offsets.data_ptr(), int(k), d_pairs.data_ptr(), P, cparams.ref, workspace.data_ptr(),
+                workspace.numel() * workspace.element_size(), C.byref(o), C.c_void_p(st.cuda_stream))
+        if budget_passes:   # memory-limited mode: nnz_capacity is the budget, the threshold is raised until the CSR fits
+            code = _lib.qp_posteriors_budgeted(*args, int(budget_passes), C.byref(tau), C.byref(passes))
+        else:
+            code = _lib.qp_posteriors(*args)
     res = Result(dense_off=None, code=int(code), launches=last_launch_count(), **t)
+    res.tau_used, res.passes = float(tau.value), int(passes.value)
     if check and code != QP_OK:
         raise QpError(code)
     return res

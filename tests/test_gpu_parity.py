@@ -279,3 +279,33 @@ def test_workspace_budget_gives_same_result(default_params):
         assert (getattr(full, name).cpu().numpy()[: len(getattr(small, name))] == getattr(small, name).cpu().numpy()).all(), name
     nz = int(full.pair_nnz_base[-1].item())
     assert (full.col_idx[:nz] == small.col_idx[:nz]).all() and (full.val[:nz] == small.val[:nz]).all()
+
+
+def test_memory_limited_mode_raises_threshold(default_params):
+    """PAPER.md:73 memory-limited mode: the CSR capacity is the budget; the threshold is raised until the CSR fits and
+    the result is exactly the posterior stage at the threshold that is reported back."""
+    qp = _qp()
+    import torch
+    fam = inputs.config_family(1)
+    pairs = inputs.all_pairs(fam.k)[:300]
+    full = qp.run_family(fam, pairs, default_params)
+    nnz_full = int(full.pair_nnz_base[-1].item())
+    cap = nnz_full // 3
+    dev = torch.device("cuda:0")
+    cp = qp.CParams(default_params)
+    L = fam.lengths
+    ws = torch.empty(qp.workspace_bytes(fam.offsets, fam.k, pairs, cp, cap), dtype=torch.uint8, device=dev)
+    args = (torch.from_numpy(fam.seqs).to(dev), torch.from_numpy(fam.offsets).to(dev), fam.k, torch.from_numpy(pairs).to(dev), cp, ws)
+    kw = dict(nnz_capacity=cap, h_rows_total=int((L[pairs[:, 0]] + 1).sum()))
+    res = qp.posteriors(*args, budget_passes=8, **kw)
+    assert res.code == 0 and res.passes >= 2 and res.tau_used > default_params.threshold
+    nnz = int(res.pair_nnz_base[-1].item())
+    assert nnz <= cap
+    print(f"budget {cap} entries of {nnz_full}: tau {default_params.threshold} -> {res.tau_used:.4f} in {res.passes} passes, nnz {nnz}")
+    prm = inputs.Params(hmm=default_params.hmm, pf=default_params.pf, threshold=res.tau_used)
+    run = orc.Run(prm, fam, pairs, keep_dense=True)
+    _compare(fam, pairs, prm, res, run, dense=False, logZ=False)
+    assert abs(nnz - int(run.nnz.sum())) <= 0.001 * nnz + 5          # only threshold-band entries may differ
+    # one pass is not enough: the capacity error comes back with the threshold that was tried last
+    r1 = qp.posteriors(*args, budget_passes=1, check=False, **kw)
+    assert r1.code == qp.ERR["NNZ_CAPACITY"] and r1.passes == 1 and int(r1.pair_nnz_base[-1].item()) == nnz_full
