@@ -132,6 +132,26 @@ int qp_posteriors_budgeted(const uint8_t* d_seqs, const int64_t* d_offsets, int3
                            const qp_params* params, void* d_workspace, size_t workspace_bytes, const qp_output* out,
                            void* cuda_stream, int max_passes, double* tau_used, int* passes);
 
+/*
+ * Stage II ("pairwise distances ... are given as an input for weighted UPGMA
+ * algorithm for guide tree construction"; tree-guided distance = "a number of nodes in a minimal
+ * subtree containing both x and y", Figure 2).
+ *   d_dist     [k*k] fp32, symmetric, entries >= 0 (the matrix qp_posteriors wrote); only i != j is read
+ *   d_merge    [k-1][2] node ids of the two children of merge t (leaves 0..k-1, the node made by merge t is k+t);
+ *              the child that lived in the smaller slot first
+ *   d_height   [k-1] distance at which merge t happened (non-decreasing)
+ *   d_leaves   [2k-1] leaf count of every node;  d_parent [2k-1] parent node id, -1 for the root
+ *   d_treedist optional [k*k] int32: 2*leaves(lca(x,y)) - 1, diagonal 1 (NULL: not computed)
+ * Weighted UPGMA: merge the closest pair of clusters (ties: the lexicographically smallest slot pair i < j, a cluster
+ * keeps the slot of its smaller-slot child), d(u,m) = (d(i,m) + d(j,m)) / 2 evaluated in fp32. All device pointers
+ * are caller-owned; the workspace holds a working copy of the matrix and the per-row nearest neighbours
+ * (qp_guide_tree_workspace_bytes). Work is enqueued on the stream, nothing is synchronised.
+ * Errors: QP_ERR_INVALID_ARG (NULL pointer, k < 1, workspace too small or misaligned), QP_ERR_CUDA.
+ */
+size_t qp_guide_tree_workspace_bytes(int32_t k);
+int qp_guide_tree(const float* d_dist, int32_t k, int32_t* d_merge, float* d_height, int32_t* d_leaves,
+                  int32_t* d_parent, int32_t* d_treedist, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
 /* Number of kernels the last qp_posteriors call on this thread launched (bench.py's gpu_launches). */
 int qp_last_launch_count(void);
 

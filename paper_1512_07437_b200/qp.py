@@ -22,7 +22,7 @@ QP_FP32, QP_FP64 = 0, 1
 FLAG_SYNC_STATUS, FLAG_NO_REFINE = 1, 2
 NUM_CLASSES = 18
 
-EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_posteriors_budgeted", "qp_last_launch_count", "qp_status_string", "qp_version",
+EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_posteriors_budgeted", "qp_guide_tree", "qp_guide_tree_workspace_bytes", "qp_last_launch_count", "qp_status_string", "qp_version",
            "qp_set_profile", "qp_get_profile", "qp_get_profile_classes"]
 
 
@@ -63,6 +63,11 @@ def _load():
                                 C.c_void_p, C.c_size_t, C.POINTER(_Output), C.c_void_p]
     L.qp_posteriors_budgeted.restype = C.c_int
     L.qp_posteriors_budgeted.argtypes = L.qp_posteriors.argtypes + [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_int)]
+    L.qp_guide_tree_workspace_bytes.restype = C.c_size_t
+    L.qp_guide_tree_workspace_bytes.argtypes = [C.c_int32]
+    L.qp_guide_tree.restype = C.c_int
+    L.qp_guide_tree.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                C.c_void_p, C.c_size_t, C.c_void_p]
     L.qp_last_launch_count.restype = C.c_int
     L.qp_status_string.restype = C.c_char_p
     L.qp_status_string.argtypes = [C.c_int]
@@ -277,3 +282,38 @@ def run_family(family, pairs, params, *, precision="fp32", want_dense=False, wan
     if want_dense:
         res.dense_off = np.concatenate([[0], np.cumsum(n.astype(np.int64) * m.astype(np.int64))])
     return res
+
+
+@dataclass
+class GuideTree:
+    """Device tensors written by qp_guide_tree (layout: include/qp.h)."""
+    merge: object      # int32 [k-1, 2]
+    height: object     # float32 [k-1]
+    leaves: object     # int32 [2k-1]
+    parent: object     # int32 [2k-1]
+    treedist: object   # int32 [k, k] or None
+
+
+def guide_tree(dist, want_treedist=True, stream=None, workspace=None) -> GuideTree:
+    """qp_guide_tree on a k x k float32 CUDA tensor (the distance matrix of qp_posteriors): weighted UPGMA guide tree
+    and, optionally, the tree-guided distances. Marshalling only; enqueued on the stream, not synchronised."""
+    import torch
+    assert dist.is_cuda and dist.dtype == torch.float32 and dist.dim() == 2 and dist.shape[0] == dist.shape[1]
+    dist = dist.contiguous()
+    k, dev = int(dist.shape[0]), dist.device
+    i32 = torch.int32
+    t = GuideTree(merge=torch.empty((max(k - 1, 0), 2), dtype=i32, device=dev),
+                  height=torch.empty(max(k - 1, 0), dtype=torch.float32, device=dev),
+                  leaves=torch.empty(2 * k - 1, dtype=i32, device=dev), parent=torch.empty(2 * k - 1, dtype=i32, device=dev),
+                  treedist=torch.empty((k, k), dtype=i32, device=dev) if want_treedist else None)
+    need = int(_lib.qp_guide_tree_workspace_bytes(k))
+    ws = workspace if workspace is not None else torch.empty(need, dtype=torch.uint8, device=dev)
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    with torch.cuda.device(dev):
+        code = _lib.qp_guide_tree(dist.data_ptr(), k, t.merge.data_ptr(), t.height.data_ptr(), t.leaves.data_ptr(),
+                                  t.parent.data_ptr(), t.treedist.data_ptr() if want_treedist else None, ws.data_ptr(),
+                                  ws.numel(), C.c_void_p(st.cuda_stream))
+    if code != QP_OK:
+        raise QpError(code)
+    t._ws = ws   # keep the workspace alive until the stream has run
+    return t
