@@ -422,6 +422,7 @@ template <typename R> static int fill_kargs(const qp_params* prm, KArgs<R>& ka) 
     if (every * g > room) return QP_ERR_RANGE;
     ka.rescale_mask = every - 1;
     ka.tau = (R)prm->threshold;
+    if constexpr (sizeof(R) == 4) ka.w2.set(ka.wh, ka.wp);
     return QP_OK;
 }
 

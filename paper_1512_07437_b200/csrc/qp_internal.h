@@ -3,6 +3,7 @@
 #include <stdint.h>
 
 #include "qp_lane.h"
+#include "qp_both.cuh"
 
 namespace qp {
 
@@ -148,6 +149,7 @@ struct SchedHeader {
 template <typename R> struct KArgs {
     typename Traits<R>::vec2 tab[kTabDim * kTabDim];   // (em_hmm, em_pf)[x*32+y], sentinel row/col zero
     Weights<R> wh, wp;
+    W2 w2;                       // fp32: (hmm, pf) weight pairs for the packed recurrences (qp_both.cuh)
     R tau;
     int rescale_mask;            // renormalise every (mask+1) steps
     int32_t k;                   // number of sequences (dist is k x k)

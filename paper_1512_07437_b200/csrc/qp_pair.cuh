@@ -169,16 +169,24 @@ struct FRing {
 template <typename R> struct FWord;
 template <> struct FWord<float> {
     float4 v;
-    __device__ __forceinline__ float h(int k) const { return (k & 1) ? v.z : v.x; }
-    __device__ __forceinline__ float p(int k) const { return (k & 1) ? v.w : v.y; }
+    __device__ __forceinline__ Traits<float>::vec2 pair(int k) const {   // (F_hmm, F_pf) of column k: a register pair
+        Traits<float>::vec2 r;
+        r.x = (k & 1) ? v.z : v.x;
+        r.y = (k & 1) ? v.w : v.y;
+        return r;
+    }
     static __device__ __forceinline__ int unit_of(int k) { return k >> 1; }
     // columns are walked downwards: a unit starts at its odd column, or at the last column of an odd-width stripe
     static __device__ __forceinline__ bool first_of_unit(int k, int C) { return (k & 1) == 1 || k == C - 1; }
 };
 template <> struct FWord<double> {
     double2 v;
-    __device__ __forceinline__ double h(int) const { return v.x; }
-    __device__ __forceinline__ double p(int) const { return v.y; }
+    __device__ __forceinline__ Traits<double>::vec2 pair(int) const {
+        Traits<double>::vec2 r;
+        r.x = v.x;
+        r.y = v.y;
+        return r;
+    }
     static __device__ __forceinline__ int unit_of(int k) { return k; }
     static __device__ __forceinline__ bool first_of_unit(int, int) { return true; }
 };
@@ -292,10 +300,8 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
       }
       const int b = b0 + warp;
       if (b < nb) {
-        FwdModel<R, GH, C> H;
-        FwdModel<R, GP, C> Pm;
-        H.init();
-        Pm.init();
+        FwdBoth<R, GP, C> FB;   // both automata of this lane (qp_both.cuh)
+        FB.init();
         int ycode[C];   // byte offset of the column's residue inside a table row
 #pragma unroll
         for (int k = 0; k < C; ++k) {
@@ -324,15 +330,15 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             // once it is past row n
             const bool recompute = (t & mask) <= 1 || (kSplit && b > 0 && t > n);
             const bool prep = recompute || t < 32;
-            FwdEx<R, GH> rh = shfl_up_ex(H.ex);
-            FwdEx<R, GP> rp = shfl_up_ex(Pm.ex);
+            FwdEx<R, GH> rh = shfl_up_ex(FB.exh());
+            FwdEx<R, GP> rp = shfl_up_ex(FB.exp());
             const uint32_t row = tab + xcode * (kTabDim * kEm);
             {
                 const int feed = __shfl_sync(kFull, chunk, t & 31);
                 const int up = __shfl_up_sync(kFull, xcode, 1);
                 if (prep) {
-                    rh.e = shfl_up1(H.ex.e);
-                    rp.e = shfl_up1(Pm.ex.e);
+                    rh.e = shfl_up1(FB.exh().e);
+                    rp.e = shfl_up1(FB.exp().e);
                 }
                 xcode = lane == 0 ? feed : up;
                 if ((t & 31) == 31) {   // warp-uniform
@@ -359,17 +365,13 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                     rp = rec.p;
                 }
             }
-            FwdRun<R, GH> runH;
-            FwdRun<R, GP> runP;
             if (prep) {
                 const bool resc = (t & mask) == 0;
-                H.prepare(rh, i == 0, resc, recompute, zero_in, range_flag);
-                Pm.prepare(rp, i == 0, resc, recompute, zero_in, range_flag);
-                rare_h = __any_sync(kFull, H.rare);
-                rare_p = __any_sync(kFull, Pm.rare);
+                FB.prepare(rh, rp, i == 0, resc, recompute, zero_in, range_flag);
+                rare_h = __any_sync(kFull, FB.rare_h());
+                rare_p = __any_sync(kFull, FB.rare_p());
             }
-            H.load(rh, rare_h, runH, ka.wh);
-            Pm.load(rp, rare_p, runP, ka.wp);
+            FB.load(rh, rp, rare_h, rare_p, ka.wh, ka.wp, ka.w2);
             const bool special = (b == 0 && t == 0) || (last && t == tend);   // warp-uniform
             FwdSpecial sp;
             sp.start = sp.capture = false;
@@ -386,9 +388,7 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
 #pragma unroll
                 for (int k = 0; k < C; ++k) {
                     const V2 em = lds_em(row + ycode[k], R(0));
-                    V2 o;
-                    o.x = H.template cell<S>(k, em.x, runH, ka.wh, sp, S ? zcap_h : dh);
-                    o.y = Pm.template cell<S>(k, em.y, runP, ka.wp, sp, S ? zcap_p : dp);
+                    const V2 o = FB.template cell<S>(k, em, ka.wh, ka.wp, ka.w2, sp, S ? zcap_h : dh, S ? zcap_p : dp);
                     if constexpr (sizeof(R) == 4) {
                         if (k & 1) {
                             if (st_on) *(float4*)(lp + (k >> 1) * 512) = make_float4(prev.x, prev.y, o.x, o.y);
@@ -404,11 +404,10 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             };
             if (special) body(std::true_type{});
             else body(std::false_type{});
-            H.end(runH);
-            Pm.end(runP);
+            FB.end();
             // exponents: constant over a renormalisation period, recorded on its last step (all lanes: a lane whose
             // last row fell inside the period has kept its exponent since)
-            if ((t & mask) == mask || t == tend) *(int2*)(lp + dE) = make_int2(H.e, Pm.e);
+            if ((t & mask) == mask || t == tend) *(int2*)(lp + dE) = make_int2(FB.eh(), FB.ep());
             if (nb > 1 && !last) {
                 if (out_ring) {
                     const int i31 = t - 31;   // warp-uniform: the row lane 31 has just finished
@@ -417,20 +416,20 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                             while (ld_acquire_cta(&cs->cons[warp]) < i31 - kDepth + 1) {}
                         if (lane == 31) {
                             FwdBnd<R, GP>& rec = cs->ring[warp][i31 % kDepth].f;
-                            rec.h = H.ex;
-                            rec.p = Pm.ex;
+                            rec.h = FB.exh();
+                            rec.p = FB.exp();
                             st_release_cta(&cs->prod[warp], i31 + 1);
                         }
                     }
                 } else if (lane == 31 && active) {
-                    bout[i].h = H.ex;
-                    bout[i].p = Pm.ex;
+                    bout[i].h = FB.exh();
+                    bout[i].p = FB.exp();
                 }
             }
         }
         if (last) {
-            ez_h = H.e;
-            ez_p = Pm.e;
+            ez_h = FB.eh();
+            ez_p = FB.ep();
             if constexpr (kSplit) {   // the forward totals live in lane lz of this warp: publish them to the CTA
                 if (lane == lz) {
                     cs->z[0] = zcap_h;
@@ -495,10 +494,8 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
       }
       const int b = b0 + warp;
       if (b < nb) {
-        BwdModel<R, GH, C> H;
-        BwdModel<R, GP, C> Pm;
-        H.init();
-        Pm.init();
+        BwdBoth<R, GP, C> BB;   // both automata of this lane (qp_both.cuh)
+        BB.init();
         Acc An[C];
         int ycode[C];
 #pragma unroll
@@ -561,8 +558,8 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             // lane 31 of an earlier block of a split pair loses its input once it is past row 0
             const bool recompute = (t & mask) >= mask - 1 || (kSplit && !last && t < 32);
             const bool prep = recompute || t >= n;
-            BwdEx<R, GH> rh = shfl_dn_ex(H.ex);
-            BwdEx<R, GP> rp = shfl_dn_ex(Pm.ex);
+            BwdEx<R, GH> rh = shfl_dn_ex(BB.exh());
+            BwdEx<R, GP> rp = shfl_dn_ex(BB.exp());
             Acc rA = shfl_dn1(exA);
             if constexpr (kCsr) ecnt = shfl_dn1(ecnt);
             const uint32_t row = tab + xcode * (kTabDim * kEm);
@@ -571,8 +568,8 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                 const int feed = __shfl_sync(kFull, chunk, sdn & 31);
                 const int dn = __shfl_down_sync(kFull, xcode, 1);
                 if (prep) {
-                    rh.e = shfl_dn1(H.ex.e);
-                    rp.e = shfl_dn1(Pm.ex.e);
+                    rh.e = shfl_dn1(BB.exh().e);
+                    rp.e = shfl_dn1(BB.exp().e);
                 }
                 if (lane == 31) rA = 0;
                 if constexpr (kCsr) {
@@ -607,20 +604,16 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                     rA = rec.A;
                 }
             }
-            BwdRun<R, GH> runH;
-            BwdRun<R, GP> runP;
             if (prep) {
                 const bool resc = (t & mask) == mask;
-                H.prepare(rh, i == n, resc, recompute, zero_in, range_flag);
-                Pm.prepare(rp, i == n, resc, recompute, zero_in, range_flag);
-                rare_h = __any_sync(kFull, H.rare);
-                rare_p = __any_sync(kFull, Pm.rare);
-                const bool bad_h = psh.set(eF.x + H.e - ez_h, invZh);
-                const bool bad_p = psp.set(eF.y + Pm.e - ez_p, invZp);
+                BB.prepare(rh, rp, i == n, resc, recompute, zero_in, range_flag);
+                rare_h = __any_sync(kFull, BB.rare_h());
+                rare_p = __any_sync(kFull, BB.rare_p());
+                const bool bad_h = psh.set(eF.x + BB.eh() - ez_h, invZh);
+                const bool bad_p = psp.set(eF.y + BB.ep() - ez_p, invZp);
                 if ((bad_h || bad_p) && active && colact) range_flag = 1;   // padding lanes hold B = 0 at exponent 0
             }
-            H.load(rh, rare_h, runH);
-            Pm.load(rp, rare_p, runP);
+            BB.load(rh, rp, rare_h, rare_p);
             // this step's F words have landed?
             const uint32_t stg = ring.waited % kStages;
             mbar_wait(ring.mbar + stg * 8, (ring.waited / kStages) & 1);
@@ -650,16 +643,16 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                     // the two backward recurrences
                     const V2 em = lds_em(row + ycode[k], R(0));
                     R zh = R(0), zp = R(0);
-                    const R bmh = H.template cell<S>(k, em.x, runH, ka.wh, sp, zh);
-                    const R bmp = Pm.template cell<S>(k, em.y, runP, ka.wp, sp, zp);
+                    const V2 bm = BB.template cell<S>(k, em, ka.wh, ka.wp, ka.w2, sp, zh, zp);
                     if (S && sp.capture && k == 0) {
                         zb_h = zh;
                         zb_p = zp;
-                        ezb_h = H.e;
-                        ezb_p = Pm.e;
+                        ezb_h = BB.eh();
+                        ezb_p = BB.ep();
                     }
                     // combine, expected-accuracy max-plus, threshold + append to the row's entry buffer
-                    const R P = combine_rms(psh.apply(Fw.h(k), bmh), psp.apply(Fw.p(k), bmp));
+                    const V2 pm = BB.posterior(Fw.pair(k), bm, psh, psp);
+                    const R P = combine_rms(pm.x, pm.y);
                     const Acc q = quantise(P, mea_scale);
                     Acc a = Adiag + q;
                     a = a > An[k] ? a : An[k];
@@ -682,8 +675,7 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             if (enext) eF = eFn;
             __syncwarp();   // every lane has read its words of this stage: refill it
             if (t >= kStages) issue(t - kStages);
-            H.end(runH);
-            Pm.end(runP);
+            BB.end();
             exA = An[0];
             Adin = rA;
             if constexpr (kCsr) {
@@ -701,15 +693,15 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                             while (ld_acquire_cta(&cs->cons[warp - 1]) < seq - kDepth + 1) {}
                         if (lane == 0) {
                             BwdBnd<R, GP>& rec = cs->ring[warp - 1][seq % kDepth].b;
-                            rec.h = H.ex;
-                            rec.p = Pm.ex;
+                            rec.h = BB.exh();
+                            rec.p = BB.exp();
                             rec.A = exA;
                             st_release_cta(&cs->prod[warp - 1], seq + 1);
                         }
                     }
                 } else if (lane == 0 && active) {
-                    bout[i].h = H.ex;
-                    bout[i].p = Pm.ex;
+                    bout[i].h = BB.exh();
+                    bout[i].p = BB.exp();
                     bout[i].A = exA;
                 }
             }
