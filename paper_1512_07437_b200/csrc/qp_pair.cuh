@@ -391,9 +391,9 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                     const V2 o = FB.template cell<S>(k, em, ka.wh, ka.wp, ka.w2, sp, S ? zcap_h : dh, S ? zcap_p : dp);
                     if constexpr (sizeof(R) == 4) {
                         if (k & 1) {
-                            if (st_on) *(float4*)(lp + (k >> 1) * 512) = make_float4(prev.x, prev.y, o.x, o.y);
+                            if (st_on) __stcs((float4*)(lp + (k >> 1) * 512), make_float4(prev.x, prev.y, o.x, o.y));
                         } else if (k == C - 1) {   // odd stripe width: the last word is half used
-                            if (st_on) *(float4*)(lp + (k >> 1) * 512) = make_float4(o.x, o.y, 0.f, 0.f);
+                            if (st_on) __stcs((float4*)(lp + (k >> 1) * 512), make_float4(o.x, o.y, 0.f, 0.f));
                         } else {
                             prev = o;
                         }
