@@ -32,6 +32,9 @@ template <typename R, int GP, int C, int MODE, int W> cudaError_t launch_pair(co
     extern template cudaError_t launch_pair<float, 2, C, kModeFull, W>(const KArgs<float>&, int, cudaStream_t);
 #define QP_DECL_F64(C, MODE, W) \
     extern template cudaError_t launch_pair<double, 2, C, MODE, W>(const KArgs<double>&, int, cudaStream_t);
+#define QP_DECL_F64_G1(C, MODE, W) \
+    extern template cudaError_t launch_pair<double, 1, C, MODE, W>(const KArgs<double>&, int, cudaStream_t);
+QP_DECL_F64_G1(2, kModeDist, 8) QP_DECL_F64_G1(4, kModeDist, 8) QP_DECL_F64_G1(8, kModeDist, 8)
 QP_DECL_F32(2, 1) QP_DECL_F32(3, 1) QP_DECL_F32(4, 1) QP_DECL_F32(5, 1) QP_DECL_F32(6, 1) QP_DECL_F32(7, 1) QP_DECL_F32(8, 1)
 QP_DECL_F32(9, 1) QP_DECL_F32(10, 1) QP_DECL_F32(11, 1) QP_DECL_F32(12, 1) QP_DECL_F32(13, 1) QP_DECL_F32(14, 1)
 QP_DECL_F32(15, 1) QP_DECL_F32(16, 1) QP_DECL_F32(8, 4) QP_DECL_F32(12, 4) QP_DECL_F32(16, 4)
@@ -442,7 +445,7 @@ static int launch_class_f32(int gp, bool full, int cls, const KArgs<float>& ka, 
     ++g_launches;
     return e == cudaSuccess ? QP_OK : QP_ERR_CUDA;
 }
-static int launch_class_f64(bool dist_only, int cls, const KArgs<double>& ka, int grid, cudaStream_t st) {
+static int launch_class_f64(bool dist_only, int gp, int cls, const KArgs<double>& ka, int grid, cudaStream_t st) {
     cudaError_t e = cudaErrorInvalidValue;
     if (!dist_only) {
         switch (cls) {
@@ -454,9 +457,10 @@ static int launch_class_f64(bool dist_only, int cls, const KArgs<double>& ka, in
         }
     } else {
         switch (cls) {
-            case 15: e = launch_pair<double, 2, 2, kModeDist, 8>(ka, grid, st); break;
-            case 16: e = launch_pair<double, 2, 4, kModeDist, 8>(ka, grid, st); break;
-            case 17: e = launch_pair<double, 2, 8, kModeDist, 8>(ka, grid, st); break;
+            // the distance-only kernels exist for one and for two insert-state pairs in the partition function
+            case 15: e = gp == 1 ? launch_pair<double, 1, 2, kModeDist, 8>(ka, grid, st) : launch_pair<double, 2, 2, kModeDist, 8>(ka, grid, st); break;
+            case 16: e = gp == 1 ? launch_pair<double, 1, 4, kModeDist, 8>(ka, grid, st) : launch_pair<double, 2, 4, kModeDist, 8>(ka, grid, st); break;
+            case 17: e = gp == 1 ? launch_pair<double, 1, 8, kModeDist, 8>(ka, grid, st) : launch_pair<double, 2, 8, kModeDist, 8>(ka, grid, st); break;
         }
     }
     ++g_launches;
@@ -689,7 +693,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
         QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
         const int grid = class_grid(c, fp64, sms);
         prof_class(c, 0, g_ctx.st[c]);
-        r = fp64 ? launch_class_f64(false, c, *ka64, grid, g_ctx.st[c])
+        r = fp64 ? launch_class_f64(false, 2, c, *ka64, grid, g_ctx.st[c])
                  : launch_class_f32(params->pf.n_ins, full_outputs, c, *ka32, grid, g_ctx.st[c]);
         if (r) return r;
         prof_class(c, 1, g_ctx.st[c]);
@@ -709,7 +713,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
         for (int c = 0; c < kNumClasses; ++c) {
             if (!((kMaskRefine >> c) & 1)) continue;
             QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
-            r = launch_class_f64(true, c, *ka64, class_grid(c, true, sms), g_ctx.st[c]);
+            r = launch_class_f64(true, params->pf.n_ins, c, *ka64, class_grid(c, true, sms), g_ctx.st[c]);
             if (r) return r;
             QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
         }

@@ -3,5 +3,6 @@
 #include "qp_kernel.cuh"
 namespace qp {
 template cudaError_t launch_pair<double, 2, 2, kModeDist, 8>(const KArgs<double>&, int, cudaStream_t);
+template cudaError_t launch_pair<double, 1, 2, kModeDist, 8>(const KArgs<double>&, int, cudaStream_t);   // GP = 1
 
 }

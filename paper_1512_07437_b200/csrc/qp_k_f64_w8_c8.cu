@@ -4,5 +4,6 @@
 #include "qp_kernel.cuh"
 namespace qp {
 template cudaError_t launch_pair<double, 2, 8, kModeDist, 8>(const KArgs<double>&, int, cudaStream_t);
+template cudaError_t launch_pair<double, 1, 8, kModeDist, 8>(const KArgs<double>&, int, cudaStream_t);   // GP = 1
 template cudaError_t launch_pair<double, 2, 8, kModeFull, 8>(const KArgs<double>&, int, cudaStream_t);
 }
