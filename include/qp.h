@@ -75,7 +75,8 @@ typedef struct {
     int32_t precision;       /* QP_FP32 | QP_FP64: arithmetic of the DP kernels                                */
     int32_t flags;           /* QP_FLAG_*                                                                      */
     double refine_below;     /* QP_FP32: pairs whose fp32 distance is below this are re-evaluated in fp64
-                                (distance only). <= 0 selects the default 0.25. See DESIGN.md "Precision".      */
+                                (distance only). <= 0 selects the default 0.25; for pairs with n + m > 4000 the
+                                limit is scaled by sqrt((n + m) / 4000). See DESIGN.md "Distances".             */
 } qp_params;
 
 /* Outputs. All device memory, caller-allocated. Optional members may be NULL. */

@@ -722,7 +722,10 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
         const int xi = ka.pairs[2 * (int64_t)p], yi = ka.pairs[2 * (int64_t)p + 1];
         ka.dist[(int64_t)xi * ka.k + yi] = (float)dist;
         ka.dist[(int64_t)yi * ka.k + xi] = (float)dist;
-        if (MODE != kModeDist && sizeof(R) == 4 && (float)dist < ka.refine_below) {
+        // fp32 distance error grows like sqrt(n + m) (measured <= 3.7e-8 * sqrt(n + m) absolute): beyond 4000 rows +
+        // columns the re-evaluation limit grows with it, so that relative 1e-5 keeps its margin on very long pairs
+        const float lim = ka.refine_below * fmaxf(1.f, sqrtf((float)(n + m) * (1.f / 4000.f)));
+        if (MODE != kModeDist && sizeof(R) == 4 && (float)dist < lim) {
             int nbd;
             const int c64 = choose_class(n, m + 1, ka.refine_cmask, true, &nbd);
             const int pos = atomicAdd(&ka.hdr->refine_count[c64], 1);
