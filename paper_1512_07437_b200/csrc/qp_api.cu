@@ -3,7 +3,8 @@
 // Schedule ("redesigning graphics processor calculations to handle sequences of
 // any length ... more efficient memory allocation model"): everything below runs on the device, the host never
 // sees a sequence length.
-//   classify : per pair -> (rows n, cols m, stripe class C, scratch bytes -> size bin); histogram per class/bin
+//   classify : per pair -> (rows n, cols m, class: packed stripe width or split (C, W), scratch bytes -> size bin);
+//              histogram per class/bin
 //   bins     : per class, bins ordered largest first -> start position of every bin
 //   scatter  : counting sort of the pair indices into order[] (class-major, largest scratch first)
 //   slots    : grant W_c resident warps per class under the workspace budget; warp w's scratch slot is sized for
@@ -275,7 +276,7 @@ static thread_local int g_launches = 0;
 static thread_local int g_profile = 0;
 static thread_local bool g_prof_valid = false;
 static thread_local cudaEvent_t g_pev[5];
-static thread_local cudaEvent_t g_cev[2 * kNumClasses];   // per stripe class: start / stop on its side stream
+static thread_local cudaEvent_t g_cev[2 * kNumClasses];   // per class: start / stop on its side stream
 static thread_local bool g_pev_ok = false;
 
 static void prof_class(int c, int which, cudaStream_t st) {
@@ -664,7 +665,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
     }
     QP_CUDA(cudaGetLastError());
 
-    // ---- a1..a7: one persistent kernel per stripe class, forked onto side streams ---------------------------
+    // ---- a1..a7: one persistent kernel per class, forked onto side streams ----------------------------------
     KArgs<float>* ka32 = nullptr;
     KArgs<double>* ka64 = nullptr;
     std::vector<char> buf32(sizeof(KArgs<float>)), buf64(sizeof(KArgs<double>));

@@ -111,11 +111,9 @@ template <typename T> __device__ __forceinline__ T ld_volatile(const T* p) {
 template <typename R> struct Slot;
 template <> struct Slot<float> {
     static constexpr int kLaneBytes = 16;                                         // one float4 = two cells
-    static __device__ __forceinline__ int cell_off(int k) { return (k >> 1) * 512 + (k & 1) * 8; }
 };
 template <> struct Slot<double> {
     static constexpr int kLaneBytes = 16;                                         // one double2 = one cell
-    static __device__ __forceinline__ int cell_off(int k) { return k * 512; }
 };
 // byte distance from `lp` to the lane's int2 exponent record of the same step
 template <typename R, int C> __device__ __forceinline__ int exps_delta(int lane) {
