@@ -220,8 +220,8 @@ template <typename T> __global__ void k_scan(const T* __restrict__ in, int64_t P
 }
 
 __global__ void k_copy_pool(const int32_t* __restrict__ nnz, const int64_t* __restrict__ pool_off,
-                            const int64_t* __restrict__ base, int64_t P, const int32_t* __restrict__ pool_col,
-                            const float* __restrict__ pool_val, int64_t cap, int32_t* __restrict__ col,
+                            const int64_t* __restrict__ base, int64_t P, const float2* __restrict__ pool,
+                            int64_t cap, int32_t* __restrict__ col,
                             float* __restrict__ val) {
     const int64_t p = blockIdx.x * (int64_t)(blockDim.x >> 5) + (threadIdx.x >> 5);
     if (p >= P) return;
@@ -229,8 +229,9 @@ __global__ void k_copy_pool(const int32_t* __restrict__ nnz, const int64_t* __re
     const int64_t cnt = nnz[p], src = pool_off[p], dst = base[p];
     if (src + cnt > cap || dst + cnt > cap) return;
     for (int64_t q = lane; q < cnt; q += 32) {
-        col[dst + q] = pool_col[src + q];
-        val[dst + q] = pool_val[src + q];
+        const float2 e = pool[src + q];
+        col[dst + q] = __float_as_int(e.y);
+        val[dst + q] = e.x;
     }
 }
 
@@ -320,7 +321,7 @@ static bool ctx_init() {
 static inline int64_t align256(int64_t v) { return (v + 255) & ~(int64_t)255; }
 
 struct Layout {   // byte offsets inside the workspace
-    int64_t hdr, info, order, rows1, cells, nnz, pool_off, dense_off, slot_off, refine_list, pool_col, pool_val, slots;
+    int64_t hdr, info, order, rows1, cells, nnz, pool_off, dense_off, slot_off, refine_list, pool, slots;
     int64_t fixed;   // everything before the slots
 };
 
@@ -342,8 +343,7 @@ static Layout make_layout(int64_t P, int64_t nnz_cap, bool dense, int64_t max_sl
     L.dense_off = take(dense ? (P + 1) * 8 : 0);
     L.slot_off = take(max_slots * 8);
     L.refine_list = take((int64_t)kNumClasses * P * 4);
-    L.pool_col = take(nnz_cap * 4);
-    L.pool_val = take(nnz_cap * 4);
+    L.pool = take(nnz_cap * 8);
     L.slots = o;
     L.fixed = o;
     return L;
@@ -483,8 +483,7 @@ template <typename R> static void fill_common(KArgs<R>& ka, const uint8_t* d_seq
     ka.refine_cmask = kMaskRefine;
     ka.pair_row_base = out->pair_row_base;
     ka.row_ptr = out->row_ptr;
-    ka.pool_col = (int32_t*)(ws + L.pool_col);
-    ka.pool_val = (float*)(ws + L.pool_val);
+    ka.pool = (float2*)(ws + L.pool);
     ka.pool_cap = out->nnz_capacity;
     ka.nnz = (int32_t*)(ws + L.nnz);
     ka.pool_off = (int64_t*)(ws + L.pool_off);
@@ -726,8 +725,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
     k_scan<int32_t><<<1, 1024, 0, ps>>>((const int32_t*)(ws + L.nnz), P, out->pair_nnz_base);
     if (out->nnz_capacity > 0)
         k_copy_pool<<<(int)((P + 3) / 4), 128, 0, ps>>>((const int32_t*)(ws + L.nnz), (const int64_t*)(ws + L.pool_off),
-                                                        out->pair_nnz_base, P, (const int32_t*)(ws + L.pool_col),
-                                                        (const float*)(ws + L.pool_val), out->nnz_capacity,
+                                                        out->pair_nnz_base, P, (const float2*)(ws + L.pool), out->nnz_capacity,
                                                         out->col_idx, out->val);
     if (refine) {
         QP_CUDA(cudaEventRecord(g_ctx.join[0], ps));

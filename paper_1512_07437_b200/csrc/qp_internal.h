@@ -169,8 +169,7 @@ template <typename R> struct KArgs {
     // outputs
     const int64_t* pair_row_base;
     int32_t* row_ptr;
-    int32_t* pool_col;
-    float* pool_val;
+    float2* pool;                // CSR staging pool: (value, column bits) per entry, completion order
     int64_t pool_cap;
     int32_t* nnz;                // per pair
     int64_t* pool_off;           // per pair

@@ -792,8 +792,7 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
         }
         cta_sync();
         if (cs->ok) {
-            int32_t* pcol = ka.pool_col + cs->poff;
-            float* pval = ka.pool_val + cs->poff;
+            float2* pool = ka.pool + cs->poff;   // (value, column bits) per entry
             for (int i0 = 1 + 32 * warp; i0 <= n; i0 += 32 * W) {
                 const int i = i0 + lane;
                 if (i > n) continue;
@@ -804,10 +803,10 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                     for (int g = (cb - 1) >> 2; g >= 0; --g) {
                         const float4 lo = ld_cg_f4(buf + g * 32), hi = ld_cg_f4(buf + g * 32 + 16);
                         const int q = 4 * g;
-                        if (q + 3 < cb) { pval[d] = hi.z; pcol[d] = __float_as_int(hi.w); ++d; }
-                        if (q + 2 < cb) { pval[d] = hi.x; pcol[d] = __float_as_int(hi.y); ++d; }
-                        if (q + 1 < cb) { pval[d] = lo.z; pcol[d] = __float_as_int(lo.w); ++d; }
-                        pval[d] = lo.x; pcol[d] = __float_as_int(lo.y); ++d;
+                        if (q + 3 < cb) { pool[d] = make_float2(hi.z, hi.w); ++d; }
+                        if (q + 2 < cb) { pool[d] = make_float2(hi.x, hi.y); ++d; }
+                        if (q + 1 < cb) { pool[d] = make_float2(lo.z, lo.w); ++d; }
+                        pool[d] = make_float2(lo.x, lo.y); ++d;
                     }
                 }
             }
@@ -823,8 +822,7 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             if (atomicCAS(&ka.hdr->status[0], 0, -6 /*QP_ERR_NNZ_CAPACITY*/) == 0) ka.hdr->status[1] = p;
         }
         int32_t* rp = ka.row_ptr + ka.pair_row_base[p];
-        int32_t* pcol = ka.pool_col + poff;
-        float* pval = ka.pool_val + poff;
+        float2* pool = ka.pool + poff;   // (value, column bits) per entry: one 8-byte store each
         const int32_t* rowcnt = (const int32_t*)(slot + rowcnt_offset(n, C, nb, RB));
         // one block per pair here (packed class). Software pipeline over the 32-row chunks: the row counts are
         // fetched two chunks ahead and a row's first entry group one chunk ahead, so that a chunk starts with its
@@ -860,10 +858,10 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
                         nhi = ld_cg_f4(buf + (g - 1) * 32 + 16);
                     }
                     const int q = 4 * g;
-                    if (q + 3 < c) { pval[d] = hi.z; pcol[d] = __float_as_int(hi.w); ++d; }
-                    if (q + 2 < c) { pval[d] = hi.x; pcol[d] = __float_as_int(hi.y); ++d; }
-                    if (q + 1 < c) { pval[d] = lo.z; pcol[d] = __float_as_int(lo.w); ++d; }
-                    pval[d] = lo.x; pcol[d] = __float_as_int(lo.y); ++d;
+                    if (q + 3 < c) { pool[d] = make_float2(hi.z, hi.w); ++d; }
+                    if (q + 2 < c) { pool[d] = make_float2(hi.x, hi.y); ++d; }
+                    if (q + 1 < c) { pool[d] = make_float2(lo.z, lo.w); ++d; }
+                    pool[d] = make_float2(lo.x, lo.y); ++d;
                     lo = nlo;
                     hi = nhi;
                 }
