@@ -135,32 +135,30 @@ def workload_name(cfg, fam, pairs):
             f"{int(L.min())}-{int(L.max())} (mean {L.mean():.0f}), all {len(pairs)} pairs")
 
 
-def run_ours(args):
+# warp instructions per cell of the pair kernels (forward + backward, all per-step and per-pair code included), from
+# the ncu instruction census of the busiest class (profiles/r02_hotloop.md); the issue bound of the kernel is
+# this count x cells / (SMs x 4 schedulers x SM clock)
+WARP_INSTR_PER_CELL = 2.52
+N_SMS = 148
+
+
+def measure(cfg, steps, warmup, dev, prm, rank=0, world=1, shard=False, sample_clocks=True):
+    """Device-resident timing of `steps` passes of the whole hot path over BASELINE.json configs[cfg].
+    Returns a dict with the aggregate numbers of this rank (ms_total is the max over ranks when world > 1)."""
     import torch
     import torch.distributed as td
     from paper_1512_07437_b200 import inputs, multi, qp
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        td.init_process_group("nccl", device_id=dev)
-
-    prm = inputs.default_params()
-    # N > 1, default ("weak"): the paper's bulk mode -- every rank takes one whole family of the
-    # same configuration (rank r: the same recipe with seed + 1000 r), independent problems, no collective.
-    # --shard-one-family ("strong"): ONE family, its pair list sharded over the ranks by balanced cell count,
-    # and the one real exchange of the path, the k x k distance matrix, all-reduced over NCCL every step.
-    shard = bool(args.shard_one_family) and world > 1
+    # N > 1, default ("strong"): SURVEY.md 8(e) -- ONE family, its pair list sharded over the ranks by balanced cell
+    # count, and the one real exchange of the path, the k x k distance matrix, all-reduced over NCCL every step.
+    # --bulk ("weak"): the paper's bulk mode (PAPER.md:73) -- every rank takes one whole family of the same
+    # configuration (rank r: the same recipe with seed + 1000 r), independent problems, no collective.
     if world > 1 and not shard:
-        c = inputs._CONFIGS[args.config]
-        fam = inputs.gen_family(c["k"], c["law"], c["r_sub"], c["r_indel"], seed=inputs.SEED_BASE + args.config + 1000 * rank,
-                                tree=c["tree"], name=f"cfg{args.config}-rank{rank}")
+        c = inputs._CONFIGS[cfg]
+        fam = inputs.gen_family(c["k"], c["law"], c["r_sub"], c["r_indel"], seed=inputs.SEED_BASE + cfg + 1000 * rank,
+                                tree=c["tree"], name=f"cfg{cfg}-rank{rank}")
     else:
-        fam = inputs.config_family(args.config)
+        fam = inputs.config_family(cfg)
     all_pairs = inputs.all_pairs(fam.k)
     L = fam.lengths
     mine = multi.shard_pairs(all_pairs, L, world, rank) if shard else np.arange(len(all_pairs))
@@ -198,8 +196,8 @@ def run_ours(args):
     torch.cuda.empty_cache()
     ws = alloc(cap)
     out_kw = dict(nnz_capacity=cap, h_rows_total=rows_total, dist=dist, check=False)
-
     state = {"res": None}
+    xbuf = torch.empty_like(dist) if shard else None
 
     def step():
         r = qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp_async, ws, reuse=state["res"], **out_kw)
@@ -207,75 +205,141 @@ def run_ours(args):
         if shard:
             # the one exchange of the path: every rank's distance entries (disjoint supports) summed over NCCL
             # (on a copy: the next step rewrites this rank's own entries of `dist` in place)
-            multi.exchange_distances(r.dist.clone())
+            xbuf.copy_(r.dist)
+            multi.exchange_distances(xbuf)
         return r
 
-    for _ in range(max(args.warmup, 3)):
+    for _ in range(max(warmup, 3)):
         res = step()
     torch.cuda.synchronize()
     assert int(res.status[0].item()) == 0, qp.status_string(int(res.status[0].item()))
     nnz = int(res.pair_nnz_base[-1].item())
+    refined = int(res.status[3].item())
     launches_per_step = res.launches
 
     # ---- timed region: K steps, CUDA events on the launching stream, barrier + sync on both sides -----------
-    sampler = ClockSampler(local)
+    sampler = ClockSampler(dev.index) if sample_clocks else None
     qp.set_profile(True)
     if world > 1:
         td.barrier()
     torch.cuda.synchronize()
-    sampler.start()
+    if sampler:
+        sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
-    for _ in range(args.steps):
+    for _ in range(steps):
         res = step()
     e1.record()
     torch.cuda.synchronize()
     if world > 1:
         td.barrier()
-    sampler.stop_flag = True
+    if sampler:
+        sampler.stop_flag = True
     ms_total = e0.elapsed_time(e1)
     prof = qp.get_profile()            # device ms of the phases of the LAST timed step (events recorded inside the region)
+    classes = qp.get_profile_classes()
     qp.set_profile(False)
     if world > 1:
         t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
         td.all_reduce(t, op=td.ReduceOp.MAX)
         ms_total = float(t.item())
-    ms_step = ms_total / args.steps
+    clocks = None
+    if sampler:
+        sampler.join(timeout=2)
+        clocks = sampler.summary()
+    return dict(fam=fam, all_pairs=all_pairs, pairs=pairs, my_cells=my_cells, total_cells=total_cells, nnz=nnz,
+                refined=refined, launches_per_step=launches_per_step, ms_step=ms_total / steps, prof=prof, classes=classes,
+                clocks=clocks, shard=shard)
+
+
+def roofline_of(cfg, m, clocks):
+    """HBM roofline of the hot path: algorithmic bytes (16 B/cell) over the WHOLE step's device time
+    (`frac`) and over the pair kernels alone (`kernel_frac`: fork..join of the class kernels, the dominant kernels),
+    with the issue bound of the pair kernels beside it."""
+    hbm_peak, peak_src = peaks()
+    prof = m["prof"]
+    step_s, kern_s = m["ms_step"] * 1e-3, prof["pair_kernels"] * 1e-3
+    cells = m["my_cells"]
+    achieved = ALGO_BYTES_PER_CELL * cells / step_s / 1e9
+    kernel_achieved = ALGO_BYTES_PER_CELL * cells / kern_s / 1e9
+    mhz = (clocks or {}).get("sm_mhz") or 1965
+    issue_s = WARP_INSTR_PER_CELL * cells / (N_SMS * 4 * mhz * 1e6)
+    return {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
+            "traffic": ncu_traffic(cfg), "peak_source": peak_src,
+            "frac_note": "whole step (schedule + pair kernels + fp64 distance queues + CSR placement) over the HBM peak",
+            "kernel": "qp::pair_kernel<float,GP,C,MODE,W>: the 18 class instances of one call (packed C=2..16, split "
+                      "C8/C12/C16 x W4), launched on side streams; duration = fork..join on the caller's stream",
+            "kernel_ms": prof["pair_kernels"], "kernel_achieved": kernel_achieved, "kernel_frac": kernel_achieved / hbm_peak,
+            "traffic_note": "dram read+write bytes of those launches from ncu (profiles/traffic.csv), per step",
+            "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
+            "phases_ms": {k: round(v, 3) for k, v in prof.items()},
+            "issue": {"warp_instr_per_cell": WARP_INSTR_PER_CELL, "sm_mhz": mhz, "bound_ms": 1e3 * issue_s,
+                      "frac": issue_s / kern_s,
+                      "note": "warp instructions per cell (ncu census, profiles/) x cells / (148 SMs x 4 schedulers x "
+                              "sampled SM clock) over the pair-kernel time"},
+            "canonical_sfu_roofline": {"ops_per_cell": SFU_OPS_PER_CELL, "peak_ops_s": SFU_PEAK,
+                                       "frac": SFU_OPS_PER_CELL * cells / kern_s / SFU_PEAK,
+                                       "note": "north_star's log-space transcendental bound; this path is "
+                                               "linear-space block floating point and issues 1 MUFU per cell"}}
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as td
+    from paper_1512_07437_b200 import inputs, qp
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        td.init_process_group("nccl", device_id=dev)
+
+    prm = inputs.default_params()
+    shard = world > 1 and not args.bulk
+    m = measure(args.config, args.steps, args.warmup, dev, prm, rank, world, shard)
+    fam, all_pairs, pairs, my_cells, total_cells = m["fam"], m["all_pairs"], m["pairs"], m["my_cells"], m["total_cells"]
+    ms_step, clocks = m["ms_step"], m["clocks"]
     value = total_cells / (ms_step * 1e-3)
-    sampler.join(timeout=2)
-    clocks = sampler.summary()
 
     line = None
     if rank == 0:
-        hbm_peak, peak_src = peaks()
-        kern_s = prof["pair_kernels"] * 1e-3
-        achieved = ALGO_BYTES_PER_CELL * my_cells / kern_s / 1e9
-        roofline = {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
-                    "traffic": ncu_traffic(args.config), "peak_source": peak_src,
-                    "kernel": "qp::pair_kernel<float,GP,C,MODE,W>: the 18 class instances of one call (packed C=2..16, split "
-                              "C8/C12/C16 x W4), launched on side streams; duration = fork..join on the caller's stream",
-                    "traffic_note": "dram read+write bytes of those launches from ncu (profiles/traffic.csv), per step",
-                    "kernel_ms": prof["pair_kernels"], "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
-                    "phases_ms": {k: round(v, 3) for k, v in prof.items()},
-                    "canonical_sfu_roofline": {"ops_per_cell": SFU_OPS_PER_CELL, "peak_ops_s": SFU_PEAK,
-                                               "frac": SFU_OPS_PER_CELL * my_cells / kern_s / SFU_PEAK,
-                                               "note": "north_star's log-space transcendental bound; this path is "
-                                                       "linear-space block floating point and issues 1 MUFU per cell"}}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
                 "scaling": "strong" if shard else "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": workload_name(args.config, fam, all_pairs), "cells": total_cells,
-                           "threshold": prm.threshold, "nnz": nnz if world == 1 else None,
-                           "beta": nnz / my_cells, "all_pairs_wall_ms": ms_step,
+                           "threshold": prm.threshold, "nnz": m["nnz"] if world == 1 else None,
+                           "beta": m["nnz"] / my_cells, "all_pairs_wall_ms": ms_step, "refined_pairs": m["refined"],
                            "l2": "per-step scratch traffic (16 B/cell) is far larger than the 126 MB L2",
-                           "parallelism": (f"one family, pairs sharded over {world} GPUs, one distance all-reduce per step"
+                           "parallelism": (f"one family, pairs sharded over {world} GPUs by balanced cells, one NCCL "
+                                           f"all-reduce of the {fam.k} x {fam.k} distance matrix per step"
                                            if shard else f"{world} independent famil{'y' if world == 1 else 'ies'} (bulk mode), "
                                            "one per GPU, no collective")},
-                "roofline": roofline, "clocks": clocks, "gpu_launches": launches_per_step * args.steps}
+                "roofline": roofline_of(args.config, m, clocks), "clocks": clocks,
+                "gpu_launches": m["launches_per_step"] * args.steps,
+                "class_timeline_ms": m["classes"]}
+
+    # ---- the other target / stress configs in the same run (N = 1, default workload only): cheap (10-30 ms a step) ----
+    if rank == 0 and world == 1 and args.config == 3 and not args.no_configs:
+        line["configs"] = {}
+        for cfg in (2, 4):
+            torch.cuda.empty_cache()
+            mc = measure(cfg, max(args.steps, 5), 3, dev, prm, sample_clocks=False)
+            rc = roofline_of(cfg, mc, clocks)
+            line["configs"][str(cfg)] = {
+                "workload": workload_name(cfg, mc["fam"], mc["all_pairs"]), "cells": mc["total_cells"],
+                "value": mc["total_cells"] / (mc["ms_step"] * 1e-3), "unit": UNIT, "ms_per_step": mc["ms_step"],
+                "steps": max(args.steps, 5), "refined_pairs": mc["refined"],
+                "roofline": {k: rc[k] for k in ("bound", "achieved", "peak", "unit", "frac", "kernel_ms", "kernel_frac",
+                                                "phases_ms")}}
+            del mc
 
     # ---- end to end through the public call with HOST buffers (pinned): H2D of the inputs, D2H of every output --
     if world == 1 and not args.no_e2e:
+        torch.cuda.empty_cache()
         e2e = run_e2e(args, fam, pairs, prm, qp, dev, my_cells)
         line["e2e"] = e2e
     elif rank == 0:
@@ -331,8 +395,10 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (0-4)")
-    ap.add_argument("--shard-one-family", action="store_true",
-                    help="N>1: shard ONE family's pair list over the ranks (strong scaling, NCCL all-reduce of distances)")
+    ap.add_argument("--bulk", action="store_true",
+                    help="N>1: one independent family per rank (the paper's bulk mode, weak scaling, no collective) "
+                         "instead of the default: ONE family sharded over the ranks + NCCL all-reduce of the distances")
+    ap.add_argument("--no-configs", action="store_true", help="skip the configs[2] / configs[4] block of the default run")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

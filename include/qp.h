@@ -90,7 +90,8 @@ typedef struct {
     float* dist;             /* [k*k] row-major; (x,y) and (y,x) are written for listed pairs only              */
     float* dense_P;          /* optional: concatenated dense n_p*m_p row-major matrices, pair order (tests)    */
     double* logZ;            /* optional [P][4]: ln Z of hmm fwd, hmm bwd, pf fwd, pf bwd                        */
-    int32_t* status;         /* [4] device status word: {code, pair index or -1, detail, refined pair count}    */
+    int32_t* status;         /* [4] device status word: {code, pair index or -1, detail, pairs whose distance was
+                                re-evaluated in fp64 (predicted near-identical pairs + those found by the fp32 pass)} */
 } qp_output;
 
 /*
@@ -160,9 +161,10 @@ int qp_last_launch_count(void);
  * Phase timing for bench.py's roofline line. qp_set_profile(1) makes later qp_posteriors calls on this thread
  * record CUDA events on the caller's stream at the phase boundaries (no synchronisation is added). After the
  * caller has synchronised the stream, qp_get_profile fills ms[0..3] with the device time of the last call:
- *   ms[0] schedule (a0), ms[1] pair kernels (a1-a7, all stripe classes, fork to join),
- *   ms[2] fp64 distance re-evaluation with the CSR placement (scan + copy) running beside it on a side stream
- *         (QP_FP64 or QP_FLAG_NO_REFINE: the CSR placement alone), ms[3] status word.
+ *   ms[0] schedule (a0, with the near-identical pair prediction), ms[1] pair kernels (a1-a7, all stripe classes, fork
+ *   to join; the early fp64 distance queue runs beside them), ms[2] what is left after their join: the late fp64
+ *   distance queue (pairs the prediction missed) and the CSR placement (scan + copy) beside it, the early queue's
+ *   tail if any, ms[3] status word.
  * Returns QP_OK, or QP_ERR_INVALID_ARG if no profiled call has completed.
  */
 void qp_set_profile(int on);
@@ -172,6 +174,13 @@ int qp_get_profile(float ms[4]);
  * classes that did not run. Same preconditions as qp_get_profile. */
 #define QP_NUM_CLASSES 18
 int qp_get_profile_classes(float start_ms[QP_NUM_CLASSES], float stop_ms[QP_NUM_CLASSES]);
+
+/*
+ * Releases what the library keeps per host thread and device between calls: the side streams and events that fork
+ * and join the per-class kernels (created lazily by the first qp_posteriors call of a thread on a device). Call it
+ * from the thread that made the calls, after its streams have been synchronised. Later calls re-create them.
+ */
+void qp_shutdown(void);
 
 const char* qp_status_string(int status);
 const char* qp_version(void);

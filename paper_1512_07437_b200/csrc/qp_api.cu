@@ -57,7 +57,7 @@ __global__ void k_check_residues(const uint8_t* __restrict__ seqs, const int64_t
 }
 
 __global__ void k_classify(const int64_t* __restrict__ offs, int k, const int32_t* __restrict__ pairs, int64_t P,
-                           uint32_t cmask, int fp64, PairInfo* __restrict__ info, int32_t* __restrict__ rows1,
+                           uint32_t cmask, int fp64, int refine, PairInfo* __restrict__ info, int32_t* __restrict__ rows1,
                            int64_t* __restrict__ cells, SchedHeader* h) {
     const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
     if (p >= P) return;
@@ -85,6 +85,13 @@ __global__ void k_classify(const int64_t* __restrict__ offs, int k, const int32_
             pi.nb = (int16_t)nb;
             pi.bin = bin_of((uint64_t)slot_bytes((int)n, class_C(c, fp64 != 0), nb, fp64 ? 8 : 4));
             atomicAdd(&h->hist[c][pi.bin], 1u);
+            if (refine) {   // the fp64 class the pair would be re-evaluated in, should it turn out near-identical
+                int nbd;
+                const int c64 = choose_class((int)n, (int)m + 1, kMaskRefine, true, &nbd);
+                const unsigned long long sb = (unsigned long long)slot_bytes((int)n, class_C(c64, true), nbd, 8);
+                if (h->rq.poll_slot_bytes[c64] < sb) atomicMax(&h->rq.poll_slot_bytes[c64], sb);
+                if (h->rq.possible[c64] < kPollCtas) atomicAdd(&h->rq.possible[c64], 1);
+            }
         }
     }
     info[p] = pi;
@@ -152,6 +159,8 @@ __global__ void k_slots(const PairInfo* __restrict__ info, const int32_t* __rest
     __shared__ int W[kNumClasses], W0[kNumClasses + 1];
     __shared__ int done, fail;
     const int t = threadIdx.x;
+    const int64_t early = (int64_t)h->poll_bytes;   // head of the slot region: slots of the fp64 pollers
+    avail -= early;
     for (int shift = 0;; ++shift) {
         if (t == 0) {
             int s = 0, all1 = 1;
@@ -181,7 +190,7 @@ __global__ void k_slots(const PairInfo* __restrict__ info, const int32_t* __rest
             for (int q = t * per; q < min(N, (t + 1) * per); ++q) {
                 int c = 0;
                 while (q >= W0[c + 1]) ++c;
-                slot_off[q] = ex;
+                slot_off[q] = early + ex;
                 ex += (int64_t)bin_ub(info[order[h->cls_start[c] + (q - W0[c])]].bin);
             }
             if (t == 0) fail = 0;
@@ -238,36 +247,62 @@ __global__ void k_copy_pool(const int32_t* __restrict__ nnz, const int64_t* __re
 struct MaxW64 {
     int w[kNumClasses];
 };
-__global__ void k_refine_plan(MaxW64 maxw, int64_t avail, SchedHeader* h) {
+// Slot plan of the fp64 re-evaluation queue (RefineQ in qp_internal.h).
+// which = 0, schedule time, before k_slots: the pollers' slots come off the head of the slot region, at most half of
+//   it: up to kPollCtas slots per class that can receive pairs, each sized for the largest pair of the class; classes
+//   are served in ascending slot size and a class that does not fit gets fewer pollers or none (the drainers take
+//   its pairs). What was taken is recorded in poll_bytes; the fp32 slots start behind it.
+// which = 1, after the fp32 classes have joined: the drainers' slots reuse the fp32 slot region; one slot for every
+//   class with pairs left (a misfit is an error), then the rest of the region class by class.
+__global__ void k_refine_plan(int which, MaxW64 maxw, int64_t avail, SchedHeader* h) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
-    // one slot for every class that has pairs, then the rest of the slot region class by class
+    RefineQ& rq = h->rq;
+    if (which == 0) {
+        unsigned long long room = (unsigned long long)avail / 2, used = 0;
+        for (int c = kNumPacked; c < kNumClasses; ++c) {   // slot sizes grow with the class index
+            const unsigned long long sb = (rq.poll_slot_bytes[c] + 255ull) & ~255ull;
+            rq.poll_slot_bytes[c] = sb;
+            int W = 0;
+            if (rq.possible[c] > 0 && sb > 0) W = (int)min((long long)min(rq.possible[c], kPollCtas), (long long)((room - used) / sb));
+            rq.Wpoll[c] = W;
+            rq.poll_slot0[c] = used;
+            used += (unsigned long long)W * sb;
+        }
+        h->poll_bytes = used;
+        return;
+    }
+    const unsigned long long lo = h->poll_bytes, bytes = (unsigned long long)avail - lo;
     unsigned long long base = 0;
-    int total = 0;
-    for (int c = 0; c < kNumClasses; ++c)
-        if (h->refine_count[c] > 0) base += h->refine_slot_bytes[c];
-    const bool fits = base <= (unsigned long long)avail;
-    if (!fits) set_status(h, QP_ERR_WORKSPACE_TOO_SMALL, -1);
-    unsigned long long spare = fits ? (unsigned long long)avail - base : 0, used = 0;
+    int left[kNumClasses];
     for (int c = 0; c < kNumClasses; ++c) {
-        const int cnt = h->refine_count[c];
+        rq.slot_bytes[c] = (rq.slot_bytes[c] + 255ull) & ~255ull;
+        left[c] = max(0, rq.count[c] - min(rq.cursor[c], rq.count[c]));   // the pollers are still pulling: an upper bound
+        if (left[c] > 0) base += rq.slot_bytes[c];
+    }
+    const bool fits = base <= bytes;
+    if (!fits) set_status(h, QP_ERR_WORKSPACE_TOO_SMALL, -1);
+    unsigned long long spare = fits ? bytes - base : 0, used = 0;
+    for (int c = 0; c < kNumClasses; ++c) {
         int W = 0;
-        if (cnt > 0 && fits) {
-            const unsigned long long sb = h->refine_slot_bytes[c];
-            const long long extra = min((long long)min(cnt, maxw.w[c]) - 1, (long long)(spare / sb));
+        if (left[c] > 0 && fits) {
+            const unsigned long long sb = rq.slot_bytes[c];
+            const long long extra = min((long long)min(left[c], maxw.w[c]) - 1, (long long)(spare / sb));
             W = 1 + (int)max(extra, 0ll);
             spare -= (unsigned long long)(W - 1) * sb;
-            h->refine_slot0[c] = used;
+            rq.slot0[c] = lo + used;
             used += (unsigned long long)W * sb;
-            total += cnt;
         }
-        h->refine_W[c] = W;
-        h->refine_cursor[c] = W;
+        rq.W[c] = W;
     }
-    h->status[3] = total;
 }
 
 __global__ void k_finish(const SchedHeader* h, int32_t* status) {
-    if (threadIdx.x < 4) status[threadIdx.x] = h->status[threadIdx.x];
+    if (threadIdx.x < 3) status[threadIdx.x] = h->status[threadIdx.x];
+    if (threadIdx.x == 3) {   // pairs whose distance was re-evaluated in fp64
+        int t = 0;
+        for (int c = 0; c < kNumClasses; ++c) t += h->rq.count[c];
+        status[3] = t;
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -275,47 +310,75 @@ __global__ void k_finish(const SchedHeader* h, int32_t* status) {
 // ------------------------------------------------------------------------------------------------------------
 static thread_local int g_launches = 0;
 static thread_local int g_profile = 0;
-static thread_local bool g_prof_valid = false;
-static thread_local cudaEvent_t g_pev[5];
-static thread_local cudaEvent_t g_cev[2 * kNumClasses];   // per class: start / stop on its side stream
-static thread_local bool g_pev_ok = false;
 
-static void prof_class(int c, int which, cudaStream_t st) {
-    if (g_profile && g_pev_ok) cudaEventRecord(g_cev[2 * c + which], st);
-}
-
-static void prof_mark(int i, cudaStream_t st) {
-    if (!g_profile) return;
-    if (!g_pev_ok) {
-        for (int q = 0; q < 5; ++q) cudaEventCreate(&g_pev[q]);
-        for (int q = 0; q < 2 * kNumClasses; ++q) cudaEventCreate(&g_cev[q]);
-        g_pev_ok = true;
-    }
-    cudaEventRecord(g_pev[i], st);
-    if (i == 4) g_prof_valid = true;
-}
-
-struct Ctx {   // lazily created side streams so that the per-class kernels overlap their tails
+// Per host thread and device: side streams so that the per-class kernels overlap their tails, the events that fork
+// and join them, and the profiling events. Created on the first call on a device, kept until qp_shutdown().
+constexpr int kNumRefine = kNumClasses - kNumPacked;          // split fp64 classes of the re-evaluation queues
+constexpr int kNumStreams = kNumClasses + kNumRefine + 1;     // fp32 / QP_FP64 classes | early fp64 queue | CSR placement
+struct Ctx {
     bool ok = false;
     int dev = -1, sms = kSmAssumed;
-    cudaStream_t st[kNumClasses];
-    cudaEvent_t fork, join[kNumClasses];
+    cudaStream_t st[kNumStreams];
+    cudaEvent_t fork, fork2, join[kNumStreams];
+    cudaEvent_t pev[5];                  // phase boundaries on the caller's stream
+    cudaEvent_t cev[2 * kNumClasses];    // per class: start / stop on its side stream
+    bool prof_valid = false;
 };
-static thread_local Ctx g_ctx;
+constexpr int kMaxDevices = 64;
+static thread_local Ctx* g_ctxs[kMaxDevices] = {nullptr};
+static thread_local Ctx* g_ctx = nullptr;     // context of the last call on this thread
 
-static bool ctx_init() {
-    int dev;
-    if (cudaGetDevice(&dev) != cudaSuccess) return false;
-    if (g_ctx.ok && g_ctx.dev == dev) return true;
-    g_ctx.dev = dev;
-    if (cudaDeviceGetAttribute(&g_ctx.sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return false;
-    for (int c = 0; c < kNumClasses; ++c) {
-        if (cudaStreamCreateWithFlags(&g_ctx.st[c], cudaStreamNonBlocking) != cudaSuccess) return false;
-        if (cudaEventCreateWithFlags(&g_ctx.join[c], cudaEventDisableTiming) != cudaSuccess) return false;
+static void ctx_destroy(Ctx* c) {
+    if (!c) return;
+    int cur = -1;
+    cudaGetDevice(&cur);
+    if (c->dev >= 0) cudaSetDevice(c->dev);
+    if (c->ok) {
+        for (int q = 0; q < kNumStreams; ++q) {
+            cudaStreamDestroy(c->st[q]);
+            cudaEventDestroy(c->join[q]);
+        }
+        cudaEventDestroy(c->fork);
+        cudaEventDestroy(c->fork2);
+        for (int q = 0; q < 5; ++q) cudaEventDestroy(c->pev[q]);
+        for (int q = 0; q < 2 * kNumClasses; ++q) cudaEventDestroy(c->cev[q]);
     }
-    if (cudaEventCreateWithFlags(&g_ctx.fork, cudaEventDisableTiming) != cudaSuccess) return false;
-    g_ctx.ok = true;
-    return true;
+    if (cur >= 0) cudaSetDevice(cur);
+    (void)cudaGetLastError();
+    delete c;
+}
+
+static Ctx* ctx_get() {
+    int dev;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return nullptr;
+    if (g_ctxs[dev] && g_ctxs[dev]->ok) return g_ctx = g_ctxs[dev];
+    Ctx* c = new Ctx();
+    c->dev = dev;
+    bool ok = cudaDeviceGetAttribute(&c->sms, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess;
+    for (int q = 0; q < kNumStreams && ok; ++q)
+        ok = cudaStreamCreateWithFlags(&c->st[q], cudaStreamNonBlocking) == cudaSuccess &&
+             cudaEventCreateWithFlags(&c->join[q], cudaEventDisableTiming) == cudaSuccess;
+    ok = ok && cudaEventCreateWithFlags(&c->fork, cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&c->fork2, cudaEventDisableTiming) == cudaSuccess;
+    for (int q = 0; q < 5 && ok; ++q) ok = cudaEventCreate(&c->pev[q]) == cudaSuccess;
+    for (int q = 0; q < 2 * kNumClasses && ok; ++q) ok = cudaEventCreate(&c->cev[q]) == cudaSuccess;
+    if (!ok) {   // partial creation: nothing is kept
+        (void)cudaGetLastError();
+        delete c;
+        return nullptr;
+    }
+    c->ok = true;
+    g_ctxs[dev] = c;
+    return g_ctx = c;
+}
+
+static void prof_class(Ctx* c, int cls, int which, cudaStream_t st) {
+    if (g_profile) cudaEventRecord(c->cev[2 * cls + which], st);
+}
+static void prof_mark(Ctx* c, int i, cudaStream_t st) {
+    if (!g_profile) return;
+    cudaEventRecord(c->pev[i], st);
+    if (i == 4) c->prof_valid = true;
 }
 
 static inline int64_t align256(int64_t v) { return (v + 255) & ~(int64_t)255; }
@@ -342,7 +405,7 @@ static Layout make_layout(int64_t P, int64_t nnz_cap, bool dense, int64_t max_sl
     L.pool_off = take(P * 8);
     L.dense_off = take(dense ? (P + 1) * 8 : 0);
     L.slot_off = take(max_slots * 8);
-    L.refine_list = take((int64_t)kNumClasses * P * 4);
+    L.refine_list = take((int64_t)kNumRefine * (P + kListPad) * 4);
     L.pool = take(nnz_cap * 8);
     L.slots = o;
     L.fixed = o;
@@ -479,7 +542,8 @@ template <typename R> static void fill_common(KArgs<R>& ka, const uint8_t* d_seq
     ka.slot_off = (const int64_t*)(ws + L.slot_off);
     ka.slots = ws + L.slots;
     ka.refine_list = (int32_t*)(ws + L.refine_list);
-    ka.refine_stride = P;
+    ka.refine_stride = P + kListPad;
+    ka.producers_total = 0;
     ka.refine_cmask = kMaskRefine;
     ka.pair_row_base = out->pair_row_base;
     ka.row_ptr = out->row_ptr;
@@ -506,17 +570,17 @@ extern "C" int qp_last_launch_count(void) { return g_launches; }
 
 extern "C" void qp_set_profile(int on) {
     g_profile = on;
-    if (!on) g_prof_valid = false;
+    if (!on && g_ctx) g_ctx->prof_valid = false;
 }
 
 extern "C" int qp_get_profile_classes(float start_ms[QP_NUM_CLASSES], float stop_ms[QP_NUM_CLASSES]) {
     static_assert(QP_NUM_CLASSES == kNumClasses, "qp.h and qp_internal.h disagree");
-    if (!g_prof_valid || !start_ms || !stop_ms) return QP_ERR_INVALID_ARG;
+    if (!g_ctx || !g_ctx->prof_valid || !start_ms || !stop_ms) return QP_ERR_INVALID_ARG;
     for (int c = 0; c < kNumClasses; ++c) {
         start_ms[c] = stop_ms[c] = -1.0f;
-        if (cudaEventQuery(g_cev[2 * c]) != cudaSuccess) { (void)cudaGetLastError(); continue; }
-        if (cudaEventElapsedTime(&start_ms[c], g_pev[1], g_cev[2 * c]) != cudaSuccess ||
-            cudaEventElapsedTime(&stop_ms[c], g_pev[1], g_cev[2 * c + 1]) != cudaSuccess) {
+        if (cudaEventQuery(g_ctx->cev[2 * c]) != cudaSuccess) { (void)cudaGetLastError(); continue; }
+        if (cudaEventElapsedTime(&start_ms[c], g_ctx->pev[1], g_ctx->cev[2 * c]) != cudaSuccess ||
+            cudaEventElapsedTime(&stop_ms[c], g_ctx->pev[1], g_ctx->cev[2 * c + 1]) != cudaSuccess) {
             (void)cudaGetLastError();
             start_ms[c] = stop_ms[c] = -1.0f;
         }
@@ -525,13 +589,21 @@ extern "C" int qp_get_profile_classes(float start_ms[QP_NUM_CLASSES], float stop
 }
 
 extern "C" int qp_get_profile(float ms[4]) {
-    if (!g_prof_valid || !ms) return QP_ERR_INVALID_ARG;
+    if (!g_ctx || !g_ctx->prof_valid || !ms) return QP_ERR_INVALID_ARG;
     for (int q = 0; q < 4; ++q)
-        if (cudaEventElapsedTime(&ms[q], g_pev[q], g_pev[q + 1]) != cudaSuccess) return QP_ERR_CUDA;
+        if (cudaEventElapsedTime(&ms[q], g_ctx->pev[q], g_ctx->pev[q + 1]) != cudaSuccess) return QP_ERR_CUDA;
     return QP_OK;
 }
 
-extern "C" const char* qp_version(void) { return "qp-b200 0.1 (sm_100a)"; }
+extern "C" void qp_shutdown(void) {
+    for (int d = 0; d < kMaxDevices; ++d) {
+        ctx_destroy(g_ctxs[d]);
+        g_ctxs[d] = nullptr;
+    }
+    g_ctx = nullptr;
+}
+
+extern "C" const char* qp_version(void) { return "qp-b200 0.2 (sm_100a)"; }
 
 extern "C" const char* qp_status_string(int s) {
     switch (s) {
@@ -571,6 +643,7 @@ extern "C" int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int
     const Layout L = make_layout(P, nnz_capacity, want_dense != 0, total_max_slots(sms));
     std::vector<std::vector<uint64_t>> sz(kNumClasses);
     uint64_t sz64[kNumClasses] = {0};   // largest fp64 slot per class among the pairs a refinement pass could see
+    int64_t cnt64[kNumClasses] = {0};   // ... and how many pairs the class could receive
     for (int64_t p = 0; p < P; ++p) {
         const int x = h_pairs[2 * p], y = h_pairs[2 * p + 1];
         if (x < 0 || y < 0 || x >= k || y >= k || x == y) return QP_ERR_BAD_PAIR;
@@ -582,6 +655,7 @@ extern "C" int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int
         if (refine) {
             const int c2 = choose_class((int)n, (int)m + 1, kMaskRefine, true, &nb);
             sz64[c2] = std::max(sz64[c2], (uint64_t)slot_bytes((int)n, class_C(c2, true), nb, 8));
+            ++cnt64[c2];
         }
     }
     uint64_t full = 0, minimum = 0;
@@ -591,7 +665,7 @@ extern "C" int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int
         for (size_t w = 0; w < W; ++w) full += sz[c][w];
         if (!sz[c].empty()) minimum += sz[c][0];
     }
-    // the refinement pass reuses the slot region: every fp64 class must fit its largest slot at least once
+    // the drainers of the fp64 re-evaluation queue reuse the fp32 slots: every fp64 class must fit its largest slot once
     uint64_t ref_min = 0;
     for (uint64_t v : sz64) ref_min += v;
     minimum = std::max(minimum, ref_min);
@@ -599,15 +673,180 @@ extern "C" int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int
     // on the device)
     uint64_t ref_full = 0;
     for (int c = 0; c < kNumClasses; ++c)
-        if ((kMaskRefine >> c) & 1) ref_full += sz64[c] * (uint64_t)std::min<int64_t>(P, max_units(c, true, sms));
+        if ((kMaskRefine >> c) & 1) ref_full += sz64[c] * (uint64_t)std::min<int64_t>(cnt64[c], max_units(c, true, sms));
     full = std::max(full, std::min<uint64_t>(ref_full, 4ull << 30));
-    full = std::max(full, minimum);
+    // the pollers run beside the fp32 classes in a region of their own (at most half of the slot region, k_refine_plan):
+    // kPollCtas slots per class that can receive pairs
+    uint64_t poll_full = 0;
+    for (int c = 0; c < kNumClasses; ++c)
+        if ((kMaskRefine >> c) & 1) poll_full += sz64[c] * (uint64_t)std::min<int64_t>(cnt64[c], kPollCtas);
+    full = std::max(std::max(full + poll_full, 2 * poll_full), minimum);
     const uint64_t need_min = (uint64_t)L.fixed + minimum, need_full = (uint64_t)L.fixed + full;
     if (budget_bytes != 0 && budget_bytes < need_min) {
         *out_bytes = (size_t)need_min;
         return QP_ERR_WORKSPACE_TOO_SMALL;
     }
     *out_bytes = (size_t)((budget_bytes != 0 && budget_bytes < need_full) ? budget_bytes : need_full);
+    return QP_OK;
+}
+
+// the work of qp_posteriors after argument validation; every error after the first enqueue goes through `fail`,
+// which waits for the side streams so that nothing is still writing the caller's buffers when the call returns
+static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, const int32_t* d_pairs,
+                          int64_t P, const qp_params* params, void* d_workspace, size_t workspace_bytes,
+                          const qp_output* out, cudaStream_t st) {
+    const bool fp64 = params->precision == QP_FP64;
+    const bool dense = out->dense_P != nullptr;
+    const int sms = cx->sms;
+    const bool refine = !fp64 && !(params->flags & QP_FLAG_NO_REFINE);
+    const bool full_outputs = out->dense_P != nullptr || out->logZ != nullptr;   // test outputs: separate kernel instances
+    const Layout L = make_layout(P, out->nnz_capacity, dense, total_max_slots(sms));
+    if ((int64_t)workspace_bytes < L.fixed + 256) return QP_ERR_WORKSPACE_TOO_SMALL;
+    char* ws = (char*)d_workspace;
+    SchedHeader* hdr = (SchedHeader*)(ws + L.hdr);
+    const int64_t avail = (int64_t)workspace_bytes - L.slots;
+
+    // ---- host-side preparation of the kernel arguments (can fail: before anything is enqueued) ----------------
+    std::vector<char> buf32(sizeof(KArgs<float>)), buf64(sizeof(KArgs<double>));
+    KArgs<float>* ka32 = new (buf32.data()) KArgs<float>();
+    KArgs<double>* ka64 = new (buf64.data()) KArgs<double>();
+    int r;
+    if (!fp64) {
+        r = fill_kargs<float>(params, *ka32);
+        if (r) return r;
+        fill_common(*ka32, d_seqs, d_pairs, k, ws, L, out, P);
+        ka32->refine_pass = 0;
+        ka32->refine_below = refine ? (float)(params->refine_below > 0.0 ? params->refine_below : 0.25) : -1.0f;
+    }
+    if (fp64 || refine) {
+        r = fill_kargs<double>(params, *ka64);
+        if (r) return r;
+        fill_common(*ka64, d_seqs, d_pairs, k, ws, L, out, P);
+        ka64->refine_pass = 0;
+        ka64->refine_below = -1.0f;
+    }
+
+    bool forked = false;
+    auto fail = [&](int code) {
+        if (forked)
+            for (int q = 0; q < kNumStreams; ++q) cudaStreamSynchronize(cx->st[q]);
+        (void)cudaGetLastError();
+        return code;
+    };
+#define QP_TRY(x)                                          \
+    do {                                                   \
+        if ((x) != cudaSuccess) return fail(QP_ERR_CUDA);  \
+    } while (0)
+
+    QP_TRY(cudaMemsetAsync(hdr, 0, sizeof(SchedHeader), st));
+    prof_mark(cx, 0, st);
+    QP_TRY(cudaMemsetAsync(ws + L.nnz, 0, (size_t)P * 4, st));
+    if (refine) QP_TRY(cudaMemsetAsync(ws + L.refine_list, 0xff, (size_t)kNumRefine * (P + kListPad) * 4, st));   // -1 = empty
+
+    // ---- a0: schedule, entirely on the device --------------------------------------------------------------
+    const uint32_t cmask = fp64 ? kMaskF64 : kMaskF32;
+    const int pb = (int)((P + 255) / 256);
+    k_check_residues<<<2 * sms, 256, 0, st>>>(d_seqs, d_offsets, k, params->hmm.alphabet, hdr);
+    k_classify<<<pb, 256, 0, st>>>(d_offsets, k, d_pairs, P, cmask, fp64 ? 1 : 0, refine ? 1 : 0, (PairInfo*)(ws + L.info),
+                                   (int32_t*)(ws + L.rows1), dense ? (int64_t*)(ws + L.cells) : nullptr, hdr);
+    k_bins<<<1, 32, 0, st>>>(hdr);
+    k_scatter<<<pb, 256, 0, st>>>((const PairInfo*)(ws + L.info), P, (int32_t*)(ws + L.order), hdr);
+    g_launches += 4;
+    MaxW64 mw64;
+    for (int c = 0; c < kNumClasses; ++c) mw64.w[c] = ((kMaskRefine >> c) & 1) ? max_units(c, true, sms) : 0;
+    if (refine) {   // the pollers' slots come off the head of the slot region
+        k_refine_plan<<<1, 32, 0, st>>>(0, mw64, avail, hdr);
+        ++g_launches;
+    }
+    MaxW mw;
+    for (int c = 0; c < kNumClasses; ++c) mw.w[c] = ((cmask >> c) & 1) ? max_units(c, fp64, sms) : 0;
+    k_slots<<<1, 1024, 0, st>>>((const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), mw, avail,
+                                (int64_t*)(ws + L.slot_off), hdr);
+    k_scan<int32_t><<<1, 1024, 0, st>>>((const int32_t*)(ws + L.rows1), P, out->pair_row_base);
+    g_launches += 2;
+    if (dense) {
+        k_scan<int64_t><<<1, 1024, 0, st>>>((const int64_t*)(ws + L.cells), P, (int64_t*)(ws + L.dense_off));
+        ++g_launches;
+    }
+    QP_TRY(cudaGetLastError());
+
+    // ---- a1..a7: one persistent kernel per class, forked onto side streams ----------------------------------
+    if (refine) {   // pollers leave when this many fp32 class warps have exited
+        int total = 0;
+        for (int c = 0; c < kNumClasses; ++c)
+            if ((cmask >> c) & 1) total += class_grid(c, false, sms) * (class_W(c, false) == 1 ? kWarpsPerCta : class_W(c, false));
+        ka32->producers_total = ka64->producers_total = total;
+    }
+    prof_mark(cx, 1, st);
+    QP_TRY(cudaEventRecord(cx->fork, st));
+    forked = true;
+    for (int c = kNumClasses - 1; c >= 0; --c) {   // split classes (long pairs) and wide stripes first
+        if (!((cmask >> c) & 1)) continue;
+        QP_TRY(cudaStreamWaitEvent(cx->st[c], cx->fork, 0));
+        const int grid = class_grid(c, fp64, sms);
+        prof_class(cx, c, 0, cx->st[c]);
+        r = fp64 ? launch_class_f64(false, 2, c, *ka64, grid, cx->st[c])
+                 : launch_class_f32(params->pf.n_ins, full_outputs, c, *ka32, grid, cx->st[c]);
+        if (r) return fail(r);
+        prof_class(cx, c, 1, cx->st[c]);
+        QP_TRY(cudaEventRecord(cx->join[c], cx->st[c]));
+        QP_TRY(cudaStreamWaitEvent(st, cx->join[c], 0));
+    }
+    if (refine) {   // pollers of the fp64 re-evaluation queue, behind the fp32 classes: they fill the room those leave
+        ka64->refine_pass = 1;
+        for (int c = kNumClasses - 1; c >= kNumPacked; --c) {
+            cudaStream_t es = cx->st[kNumClasses + (c - kNumPacked)];
+            QP_TRY(cudaStreamWaitEvent(es, cx->fork, 0));
+            r = launch_class_f64(true, params->pf.n_ins, c, *ka64, kPollCtas, es);
+            if (r) return fail(r);
+            QP_TRY(cudaEventRecord(cx->join[kNumClasses + (c - kNumPacked)], es));
+        }
+    }
+    prof_mark(cx, 2, st);
+
+    // ---- drainers: what the pollers have not taken when the fp32 classes have finished ----------------------------
+    if (refine) {
+        k_refine_plan<<<1, 32, 0, st>>>(1, mw64, avail, hdr);
+        ++g_launches;
+        QP_TRY(cudaEventRecord(cx->fork2, st));
+        ka64->refine_pass = 2;
+        for (int c = kNumPacked; c < kNumClasses; ++c) {
+            QP_TRY(cudaStreamWaitEvent(cx->st[c], cx->fork2, 0));
+            r = launch_class_f64(true, params->pf.n_ins, c, *ka64, class_grid(c, true, sms), cx->st[c]);
+            if (r) return fail(r);
+            QP_TRY(cudaEventRecord(cx->join[c], cx->st[c]));
+        }
+    }
+
+    // ---- CSR placement in pair order; it only needs the fp32 pass, so it runs beside the fp64 kernels ------------
+    cudaStream_t ps = refine ? cx->st[kNumStreams - 1] : st;
+    if (refine) QP_TRY(cudaStreamWaitEvent(ps, cx->fork2, 0));
+    k_scan<int32_t><<<1, 1024, 0, ps>>>((const int32_t*)(ws + L.nnz), P, out->pair_nnz_base);
+    if (out->nnz_capacity > 0)
+        k_copy_pool<<<(int)((P + 3) / 4), 128, 0, ps>>>((const int32_t*)(ws + L.nnz), (const int64_t*)(ws + L.pool_off),
+                                                        out->pair_nnz_base, P, (const float2*)(ws + L.pool), out->nnz_capacity,
+                                                        out->col_idx, out->val);
+    if (refine) {
+        QP_TRY(cudaEventRecord(cx->join[kNumStreams - 1], ps));
+        QP_TRY(cudaStreamWaitEvent(st, cx->join[kNumStreams - 1], 0));
+        for (int c = kNumPacked; c < kNumClasses; ++c) {
+            QP_TRY(cudaStreamWaitEvent(st, cx->join[c], 0));                                  // drainers
+            QP_TRY(cudaStreamWaitEvent(st, cx->join[kNumClasses + (c - kNumPacked)], 0));     // pollers
+        }
+    }
+    prof_mark(cx, 3, st);
+    k_finish<<<1, 32, 0, st>>>(hdr, out->status);
+    g_launches += 3;
+    prof_mark(cx, 4, st);
+    QP_TRY(cudaGetLastError());
+#undef QP_TRY
+
+    if (params->flags & QP_FLAG_SYNC_STATUS) {
+        int32_t hs[4] = {0, 0, 0, 0};
+        QP_CUDA(cudaMemcpyAsync(hs, out->status, sizeof hs, cudaMemcpyDeviceToHost, st));
+        QP_CUDA(cudaStreamSynchronize(st));
+        return hs[0];
+    }
     return QP_OK;
 }
 
@@ -622,11 +861,9 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
     if (P > 0 && (!d_seqs || !d_offsets || !d_pairs || !d_workspace || !out->row_ptr || !out->dist)) return QP_ERR_INVALID_ARG;
     if (out->nnz_capacity < 0 || (out->nnz_capacity > 0 && (!out->col_idx || !out->val))) return QP_ERR_INVALID_ARG;
     if (P > 0 && ((uintptr_t)d_workspace & 255) != 0) return QP_ERR_INVALID_ARG;
-    if (!ctx_init()) return QP_ERR_CUDA;
+    Ctx* cx = ctx_get();
+    if (!cx) return QP_ERR_CUDA;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const bool fp64 = params->precision == QP_FP64;
-    const bool dense = out->dense_P != nullptr;
-    const int sms = g_ctx.sms;
     if (P == 0) {   // nothing to do: empty prefixes, status ok; the workspace is not touched
         QP_CUDA(cudaMemsetAsync(out->pair_row_base, 0, 8, st));
         QP_CUDA(cudaMemsetAsync(out->pair_nnz_base, 0, 8, st));
@@ -634,118 +871,7 @@ extern "C" int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, in
         if (params->flags & QP_FLAG_SYNC_STATUS) QP_CUDA(cudaStreamSynchronize(st));
         return QP_OK;
     }
-    const Layout L = make_layout(P, out->nnz_capacity, dense, total_max_slots(sms));
-    if ((int64_t)workspace_bytes < L.fixed + 256) return QP_ERR_WORKSPACE_TOO_SMALL;
-    char* ws = (char*)d_workspace;
-    SchedHeader* hdr = (SchedHeader*)(ws + L.hdr);
-    const int64_t avail = (int64_t)workspace_bytes - L.slots;
-
-    QP_CUDA(cudaMemsetAsync(hdr, 0, sizeof(SchedHeader), st));
-    prof_mark(0, st);
-    QP_CUDA(cudaMemsetAsync(ws + L.nnz, 0, (size_t)P * 4, st));
-
-    // ---- a0: schedule, entirely on the device --------------------------------------------------------------
-    const uint32_t cmask = fp64 ? kMaskF64 : kMaskF32;
-    const int pb = (int)((P + 255) / 256);
-    k_check_residues<<<2 * sms, 256, 0, st>>>(d_seqs, d_offsets, k, params->hmm.alphabet, hdr);
-    k_classify<<<pb, 256, 0, st>>>(d_offsets, k, d_pairs, P, cmask, fp64 ? 1 : 0, (PairInfo*)(ws + L.info),
-                                   (int32_t*)(ws + L.rows1), dense ? (int64_t*)(ws + L.cells) : nullptr, hdr);
-    k_bins<<<1, 32, 0, st>>>(hdr);
-    k_scatter<<<pb, 256, 0, st>>>((const PairInfo*)(ws + L.info), P, (int32_t*)(ws + L.order), hdr);
-    MaxW mw;
-    for (int c = 0; c < kNumClasses; ++c) mw.w[c] = ((cmask >> c) & 1) ? max_units(c, fp64, sms) : 0;
-    k_slots<<<1, 1024, 0, st>>>((const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), mw, avail,
-                                (int64_t*)(ws + L.slot_off), hdr);
-    k_scan<int32_t><<<1, 1024, 0, st>>>((const int32_t*)(ws + L.rows1), P, out->pair_row_base);
-    g_launches += 6;
-    if (dense) {
-        k_scan<int64_t><<<1, 1024, 0, st>>>((const int64_t*)(ws + L.cells), P, (int64_t*)(ws + L.dense_off));
-        ++g_launches;
-    }
-    QP_CUDA(cudaGetLastError());
-
-    // ---- a1..a7: one persistent kernel per class, forked onto side streams ----------------------------------
-    KArgs<float>* ka32 = nullptr;
-    KArgs<double>* ka64 = nullptr;
-    std::vector<char> buf32(sizeof(KArgs<float>)), buf64(sizeof(KArgs<double>));
-    ka32 = new (buf32.data()) KArgs<float>();
-    ka64 = new (buf64.data()) KArgs<double>();
-    const bool refine = !fp64 && !(params->flags & QP_FLAG_NO_REFINE);
-    const bool full_outputs = out->dense_P != nullptr || out->logZ != nullptr;   // test outputs: separate kernel instances
-    if (!fp64) {
-        r = fill_kargs<float>(params, *ka32);
-        if (r) return r;
-        fill_common(*ka32, d_seqs, d_pairs, k, ws, L, out, P);
-        ka32->refine_pass = 0;
-        ka32->refine_below = refine ? (float)(params->refine_below > 0.0 ? params->refine_below : 0.25) : -1.0f;
-    }
-    if (fp64 || refine) {
-        r = fill_kargs<double>(params, *ka64);
-        if (r) return r;
-        fill_common(*ka64, d_seqs, d_pairs, k, ws, L, out, P);
-        ka64->refine_pass = fp64 ? 0 : 1;
-        ka64->refine_below = -1.0f;
-    }
-    prof_mark(1, st);
-    QP_CUDA(cudaEventRecord(g_ctx.fork, st));
-    for (int c = kNumClasses - 1; c >= 0; --c) {   // split classes (long pairs) and wide stripes first
-        if (!((cmask >> c) & 1)) continue;
-        QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
-        const int grid = class_grid(c, fp64, sms);
-        prof_class(c, 0, g_ctx.st[c]);
-        r = fp64 ? launch_class_f64(false, 2, c, *ka64, grid, g_ctx.st[c])
-                 : launch_class_f32(params->pf.n_ins, full_outputs, c, *ka32, grid, g_ctx.st[c]);
-        if (r) return r;
-        prof_class(c, 1, g_ctx.st[c]);
-        QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
-        QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));
-    }
-
-    prof_mark(2, st);
-
-    // ---- fp64 re-evaluation of the distance of near-identical pairs ----------------
-    if (refine) {
-        MaxW64 mw64;
-        for (int c = 0; c < kNumClasses; ++c) mw64.w[c] = ((kMaskRefine >> c) & 1) ? max_units(c, true, sms) : 0;
-        k_refine_plan<<<1, 32, 0, st>>>(mw64, avail, hdr);
-        ++g_launches;
-        QP_CUDA(cudaEventRecord(g_ctx.fork, st));
-        for (int c = 0; c < kNumClasses; ++c) {
-            if (!((kMaskRefine >> c) & 1)) continue;
-            QP_CUDA(cudaStreamWaitEvent(g_ctx.st[c], g_ctx.fork, 0));
-            r = launch_class_f64(true, params->pf.n_ins, c, *ka64, class_grid(c, true, sms), g_ctx.st[c]);
-            if (r) return r;
-            QP_CUDA(cudaEventRecord(g_ctx.join[c], g_ctx.st[c]));
-        }
-    }
-
-    // ---- CSR placement in pair order; it only needs the fp32 pass, so it runs beside the fp64 kernels ------------
-    cudaStream_t ps = refine ? g_ctx.st[0] : st;
-    if (refine) QP_CUDA(cudaStreamWaitEvent(ps, g_ctx.fork, 0));
-    k_scan<int32_t><<<1, 1024, 0, ps>>>((const int32_t*)(ws + L.nnz), P, out->pair_nnz_base);
-    if (out->nnz_capacity > 0)
-        k_copy_pool<<<(int)((P + 3) / 4), 128, 0, ps>>>((const int32_t*)(ws + L.nnz), (const int64_t*)(ws + L.pool_off),
-                                                        out->pair_nnz_base, P, (const float2*)(ws + L.pool), out->nnz_capacity,
-                                                        out->col_idx, out->val);
-    if (refine) {
-        QP_CUDA(cudaEventRecord(g_ctx.join[0], ps));
-        QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[0], 0));
-        for (int c = 0; c < kNumClasses; ++c)
-            if ((kMaskRefine >> c) & 1) QP_CUDA(cudaStreamWaitEvent(st, g_ctx.join[c], 0));
-    }
-    prof_mark(3, st);
-    k_finish<<<1, 32, 0, st>>>(hdr, out->status);
-    g_launches += 3;
-    prof_mark(4, st);
-    QP_CUDA(cudaGetLastError());
-
-    if (params->flags & QP_FLAG_SYNC_STATUS) {
-        int32_t hs[4] = {0, 0, 0, 0};
-        QP_CUDA(cudaMemcpyAsync(hs, out->status, sizeof hs, cudaMemcpyDeviceToHost, st));
-        QP_CUDA(cudaStreamSynchronize(st));
-        return hs[0];
-    }
-    return QP_OK;
+    return run_posteriors(cx, d_seqs, d_offsets, k, d_pairs, P, params, d_workspace, workspace_bytes, out, st);
 }
 
 extern "C" int qp_posteriors_budgeted(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, const int32_t* d_pairs,

@@ -127,6 +127,30 @@ QP_HD2 uint64_t bin_ub(int b) {
     return (uint64_t)(8 + mant + 1) << (e - 3);
 }
 
+// fp64 distance re-evaluation queue, one list per split fp64 class (kMaskRefine). The fp32
+// pair kernels append the pairs whose fp32 distance is below the limit; two sets of fp64 kernels consume the lists
+// through one cursor per class:
+//   pollers  a few CTAs per class, launched with the fp32 classes (after them, so they take SM room only when the fp32
+//            kernels leave some): they wait for entries to appear, and leave when every fp32 CTA has finished and the
+//            list is drained. Their scratch slots are reserved at schedule time, sized for the largest pair the class
+//            could receive.
+//   drainers full-width kernels launched after the fp32 classes have joined, for what is left; slots from the fp32
+//            slot region, sized for the largest pair actually queued.
+constexpr int kPollCtas = 32;         // pollers per class: 3 x 32 CTAs can never fill the 148 SMs, so the fp32 kernels
+                                      // always find room whatever order the hardware places CTAs in
+constexpr int kListPad = 1024;        // every consumer CTA may pull one index past the end of the list
+struct RefineQ {
+    int32_t count[kNumClasses];                   // pairs queued, per fp64 class
+    int32_t cursor[kNumClasses];                  // next list position to consume
+    int32_t possible[kNumClasses];                // pairs of the call that WOULD go to the class (schedule time)
+    int32_t Wpoll[kNumClasses];                   // pollers granted
+    unsigned long long poll_slot_bytes[kNumClasses];   // largest fp64 scratch slot among all pairs of the class
+    unsigned long long poll_slot0[kNumClasses];
+    int32_t W[kNumClasses];                       // drainers granted
+    unsigned long long slot_bytes[kNumClasses];   // largest fp64 scratch slot among the queued pairs
+    unsigned long long slot0[kNumClasses];        // byte offset of the class's first slot inside the slot region
+};
+
 struct SchedHeader {
     int32_t status[4];                       // mirrors qp_output.status
     unsigned long long pool_cursor;          // CSR staging pool bump pointer (entries)
@@ -135,11 +159,10 @@ struct SchedHeader {
     int32_t cls_W[kNumClasses];              // resident warps (= scratch slots) granted to the class
     int32_t cls_slot0[kNumClasses];          // first entry of the class in slot_off[]
     int32_t cls_cursor[kNumClasses];         // next position in the class's order list
-    int32_t refine_count[kNumClasses];       // pairs queued for fp64 re-evaluation, per fp64 class
-    int32_t refine_cursor[kNumClasses];
-    int32_t refine_W[kNumClasses];
-    unsigned long long refine_slot_bytes[kNumClasses];   // largest fp64 scratch slot among the queued pairs
-    unsigned long long refine_slot0[kNumClasses];        // byte offset of the class's first slot
+    RefineQ rq;
+    unsigned long long poll_bytes;           // head of the slot region, reserved for the pollers' slots
+    int32_t producers_done;                  // fp32 class CTAs that have exited
+    int32_t pad_;
     uint32_t hist[kNumClasses][kNumBins];    // pairs per (class, size bin)
     uint32_t bin_start[kNumClasses][kNumBins];   // position of the bin inside the class, largest bins first
     uint32_t bin_fill[kNumClasses][kNumBins];
@@ -153,7 +176,8 @@ template <typename R> struct KArgs {
     R tau;
     int rescale_mask;            // renormalise every (mask+1) steps
     int32_t k;                   // number of sequences (dist is k x k)
-    int32_t refine_pass;         // 1: process the refine list, write distances only
+    int32_t refine_pass;         // 0: class lists; 1 / 2: poller / drainer of the fp64 re-evaluation queue, distances only
+    int32_t producers_total;     // fp32 class CTAs of the call (pollers leave when all of them have exited); 0: not counted
     float refine_below;          // fp32 pass: queue pairs whose distance is below this (<=0: never)
     double lx_h[kTabDim], lx_p[kTabDim];   // insert log-weights (for the logZ constant)
     const uint8_t* seqs;
@@ -163,7 +187,7 @@ template <typename R> struct KArgs {
     SchedHeader* hdr;
     const int64_t* slot_off;     // byte offset of each slot inside slots
     char* slots;
-    int32_t* refine_list;        // [kNumClasses][refine_stride] pair indices queued for fp64 re-evaluation
+    int32_t* refine_list;        // [3 split classes][refine_stride] pair indices queued for fp64 re-evaluation, -1 = empty
     int64_t refine_stride;
     uint32_t refine_cmask;       // classes of the fp64 distance re-evaluation
     // outputs

@@ -3,6 +3,8 @@
 //   packed classes (W = 1): every warp owns one scratch slot and pulls pairs of its class largest-first;
 //   split classes  (W > 1): every CTA owns one scratch slot, its W warps share each pair it pulls.
 #pragma once
+#include <atomic>
+
 #include "qp_pair.cuh"
 
 namespace qp {
@@ -48,47 +50,82 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
     constexpr int cls = class_index(C, W, sizeof(R) == 8);
     const int unit = W == 1 ? blockIdx.x * kWarpsPerCta + warp : blockIdx.x;   // who owns a scratch slot
     SchedHeader* hdr = ka.hdr;
-    int granted, count;
-    const int32_t* list;
-    char* slot;
-    int* cursor;
-    if (ka.refine_pass) {
-        granted = hdr->refine_W[cls];
-        count = hdr->refine_count[cls];
-        list = ka.refine_list + (int64_t)cls * ka.refine_stride;
-        if (unit >= granted) return;
-        slot = ka.slots + hdr->refine_slot0[cls] + (unsigned long long)unit * hdr->refine_slot_bytes[cls];
-        cursor = &hdr->refine_cursor[cls];
-    } else {
-        granted = hdr->cls_W[cls];
-        count = hdr->cls_count[cls];
-        list = ka.order + hdr->cls_start[cls];
-        if (unit >= granted) return;
-        slot = ka.slots + ka.slot_off[hdr->cls_slot0[cls] + unit];
-        cursor = &hdr->cls_cursor[cls];
-    }
-    int idx = unit;   // the first `granted` pairs of the (largest-first) list go to units 0..granted-1; the rest are pulled
-    while (idx < count) {
-        process_pair<R, GP, C, MODE, W>(ka, smem_u32(tab), list[idx], slot, lane, warp, ring, cs);
-        if constexpr (W == 1) {
-            if (lane == 0) idx = atomicAdd(cursor, 1);
-            idx = __shfl_sync(kFull, idx, 0);
-        } else {
-            cta_sync();   // every warp is done with the slot and with CoopShared
-            if (threadIdx.x == 0) cs->next = atomicAdd(cursor, 1);
+    if constexpr (MODE == kModeDist) {
+        // consumer of the fp64 re-evaluation queue (split classes only): pull list positions through the class cursor;
+        // a poller waits for its position to be filled until every fp32 class CTA has exited
+        static_assert(W > 1, "the distance-only kernels are split-class kernels");
+        RefineQ& q = hdr->rq;
+        const bool poll = ka.refine_pass == 1;
+        if (unit >= (poll ? q.Wpoll[cls] : q.W[cls])) return;
+        char* slot = ka.slots + (poll ? q.poll_slot0[cls] + (unsigned long long)unit * q.poll_slot_bytes[cls]
+                                      : q.slot0[cls] + (unsigned long long)unit * q.slot_bytes[cls]);
+        const int32_t* list = refine_list_of(ka, cls);
+        for (;;) {
+            if (threadIdx.x == 0) {
+                const int pos = atomicAdd(&q.cursor[cls], 1);
+                int v;
+                for (;;) {
+                    v = ld_acquire_gpu(list + pos);
+                    if (v >= 0) break;
+                    if (ld_acquire_gpu(&hdr->producers_done) >= ka.producers_total) {   // nothing more will be queued
+                        v = ld_acquire_gpu(list + pos);
+                        break;
+                    }
+                    __nanosleep(2000);
+                }
+                cs->next = v;
+            }
             cta_sync();
-            idx = cs->next;
+            const int p = cs->next;
+            if (p < 0) return;
+            process_pair<R, GP, C, MODE, W>(ka, smem_u32(tab), p, slot, lane, warp, ring, cs);
+            cta_sync();   // every warp is done with the slot and with CoopShared
+        }
+    } else {
+        struct Leave {   // every fp32 class warp reports its exit, whatever path it leaves by (pollers wait for the total)
+            SchedHeader* h;
+            bool on;
+            __device__ ~Leave() {
+                if (on && (threadIdx.x & 31) == 0) {   // per warp: the warps of a packed-class CTA leave one by one
+                    __threadfence();
+                    atomicAdd(&h->producers_done, 1);
+                }
+            }
+        } leave{hdr, ka.producers_total > 0};
+        const int granted = hdr->cls_W[cls], count = hdr->cls_count[cls];
+        const int32_t* list = ka.order + hdr->cls_start[cls];
+        if (unit >= granted) return;
+        char* slot = ka.slots + ka.slot_off[hdr->cls_slot0[cls] + unit];
+        int* cursor = &hdr->cls_cursor[cls];
+        int idx = unit;   // the first `granted` pairs of the (largest-first) list go to units 0..granted-1; the rest are pulled
+        while (idx < count) {
+            process_pair<R, GP, C, MODE, W>(ka, smem_u32(tab), list[idx], slot, lane, warp, ring, cs);
+            if constexpr (W == 1) {
+                if (lane == 0) idx = atomicAdd(cursor, 1);
+                idx = __shfl_sync(kFull, idx, 0);
+            } else {
+                cta_sync();   // every warp is done with the slot and with CoopShared
+                if (threadIdx.x == 0) cs->next = atomicAdd(cursor, 1);
+                cta_sync();
+                idx = cs->next;
+            }
         }
     }
 }
 
 template <typename R, int GP, int C, int MODE, int W> cudaError_t launch_pair(const KArgs<R>& ka, int grid, cudaStream_t st) {
     constexpr size_t smem = KernelSmem<R, C, W>::template total<GP>();
-    static bool attr_set = false;   // per instantiation; the attribute is sticky per device function
-    if (!attr_set) {
-        cudaError_t e = cudaFuncSetAttribute(pair_kernel<R, GP, C, MODE, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    // the opt-in to more than 48 KB of dynamic shared memory is per device function AND per device: remember it as
+    // one bit per device ordinal (per instantiation), set atomically so that host threads may share the library
+    static std::atomic<unsigned long long> attr_devs{0};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const unsigned long long bit = 1ull << (dev & 63);
+    if (dev >= 64 || !(attr_devs.load(std::memory_order_acquire) & bit)) {
+        e = cudaFuncSetAttribute(pair_kernel<R, GP, C, MODE, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
-        attr_set = true;
+        if (dev < 64) attr_devs.fetch_or(bit, std::memory_order_release);
     }
     pair_kernel<R, GP, C, MODE, W><<<grid, KernelSmem<R, C, W>::kWarps * 32, smem, st>>>(ka);
     return cudaGetLastError();

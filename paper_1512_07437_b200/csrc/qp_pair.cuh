@@ -253,6 +253,19 @@ __device__ __forceinline__ void cta_sync() { __syncthreads(); }
 // travels with the wavefront by shuffle; only the entering lane (lane 0 forward, lane 31 backward) takes a new
 // code, from a 32-row chunk that the warp loads (coalesced) one chunk ahead of its use.
 
+// re-evaluation list of split fp64 class cls (kNumPacked..kNumClasses-1)
+template <typename R> __host__ __device__ __forceinline__ int32_t* refine_list_of(const KArgs<R>& ka, int cls) {
+    return ka.refine_list + (int64_t)(cls - kNumPacked) * ka.refine_stride;
+}
+__device__ __forceinline__ void st_release_gpu(int32_t* p, int32_t v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ int32_t ld_acquire_gpu(const int32_t* p) {
+    int32_t v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // ---------------------------------------------------------------------------------------------------------
 // the pair pipeline
 // ---------------------------------------------------------------------------------------------------------
@@ -285,7 +298,9 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
     char* bnd0 = slot + (int64_t)nb * blk_bytes;
     char* bnd1 = bnd0 + (int64_t)(n + 1) * bnd_rec_bytes(RB);
     int range_flag = 0;
-    auto xcode_at = [&](int i) -> int { return (i >= 1 && i <= n) ? (int)__ldg(xs + i - 1) : kSentinel; };
+    // residue bytes index the 32 x 32 emission table in shared memory: clamp them so that an invalid code (>= 32; the
+    // call then ends with QP_ERR_BAD_RESIDUE, k_check_residues) can never address outside the table
+    auto xcode_at = [&](int i) -> int { return (i >= 1 && i <= n) ? min((int)__ldg(xs + i - 1), kSentinel) : kSentinel; };
 
     // =========================================== forward ===================================================
     R zcap_h = R(0), zcap_p = R(0);
@@ -304,7 +319,7 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
 #pragma unroll
         for (int k = 0; k < C; ++k) {
             int j = b * 32 * C + lane * C + k;
-            ycode[k] = ((j >= 1 && j <= m) ? (int)ys[j - 1] : kSentinel) * kEm;
+            ycode[k] = ((j >= 1 && j <= m) ? min((int)ys[j - 1], kSentinel) : kSentinel) * kEm;
         }
         const bool last = (b == nb - 1);
         const int tend = n + (last ? lz : 31);
@@ -500,7 +515,7 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
         for (int k = 0; k < C; ++k) {
             An[k] = 0;
             int j = b * 32 * C + lane * C + k;
-            ycode[k] = ((j >= 1 && j <= m) ? (int)ys[j - 1] : kSentinel) * kEm;
+            ycode[k] = ((j >= 1 && j <= m) ? min((int)ys[j - 1], kSentinel) : kSentinel) * kEm;
         }
         Acc Adin = 0, exA = 0;
         bool rare_h = false, rare_p = false;   // warp-uniform, see the forward loop
@@ -726,10 +741,11 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
         if (MODE != kModeDist && sizeof(R) == 4 && (float)dist < lim) {
             int nbd;
             const int c64 = choose_class(n, m + 1, ka.refine_cmask, true, &nbd);
-            const int pos = atomicAdd(&ka.hdr->refine_count[c64], 1);
-            ka.refine_list[(int64_t)c64 * ka.refine_stride + pos] = p;
-            atomicMax(&ka.hdr->refine_slot_bytes[c64],
-                      (unsigned long long)slot_bytes(n, class_C(c64, true), nbd, 8));
+            RefineQ& q = ka.hdr->rq;
+            const int pos = atomicAdd(&q.count[c64], 1);
+            atomicMax(&q.slot_bytes[c64], (unsigned long long)slot_bytes(n, class_C(c64, true), nbd, 8));
+            // publish: the fp64 kernel that picks the entry up overwrites the distance written above
+            st_release_gpu(refine_list_of(ka, c64) + pos, p);
         }
     }
 
@@ -737,8 +753,8 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
     if constexpr (MODE == kModeFull) {
         if (ka.logZ != nullptr && warp == 0) {
             double ch = 0.0, cp = 0.0;
-            for (int q = lane; q < n; q += 32) { ch += ka.lx_h[xs[q]]; cp += ka.lx_p[xs[q]]; }
-            for (int q = lane; q < m; q += 32) { ch += ka.lx_h[ys[q]]; cp += ka.lx_p[ys[q]]; }
+            for (int q = lane; q < n; q += 32) { ch += ka.lx_h[xs[q] & 31]; cp += ka.lx_p[xs[q] & 31]; }
+            for (int q = lane; q < m; q += 32) { ch += ka.lx_h[ys[q] & 31]; cp += ka.lx_p[ys[q] & 31]; }
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) {
                 ch += __shfl_xor_sync(kFull, ch, o);

@@ -23,7 +23,7 @@ FLAG_SYNC_STATUS, FLAG_NO_REFINE = 1, 2
 NUM_CLASSES = 18
 
 EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_posteriors_budgeted", "qp_guide_tree", "qp_guide_tree_workspace_bytes", "qp_last_launch_count", "qp_status_string", "qp_version",
-           "qp_set_profile", "qp_get_profile", "qp_get_profile_classes"]
+           "qp_set_profile", "qp_get_profile", "qp_get_profile_classes", "qp_shutdown"]
 
 
 class QpError(RuntimeError):
@@ -78,6 +78,7 @@ def _load():
     L.qp_get_profile.argtypes = [C.POINTER(C.c_float)]
     L.qp_get_profile_classes.restype = C.c_int
     L.qp_get_profile_classes.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]
+    L.qp_shutdown.restype = None
     return L
 
 
@@ -94,6 +95,11 @@ def version() -> str:
 
 def last_launch_count() -> int:
     return int(_lib.qp_last_launch_count())
+
+
+def shutdown() -> None:
+    """qp_shutdown: release the calling thread's side streams and events (synchronise your streams first)."""
+    _lib.qp_shutdown()
 
 
 def set_profile(on: bool) -> None:

@@ -41,7 +41,6 @@ def _compare(fam, pairs, params, res, run, dense=True, logZ=True, p_atol=parity.
                               dense=d, logZ=lz[p] if logZ else None, p_atol=p_atol, d_rtol=d_rtol,
                               logz_rtol=logz_rtol)
         worst = (max(worst[0], e[0]), max(worst[1], e[1]))
-    assert nb[-1] == sum(run.nnz) or True
     return worst
 
 
@@ -152,6 +151,67 @@ def test_generic_models_g1_hmm_g2_pf():
         _compare(fam, pairs, prm, res, run, **tol)
 
 
+def _pf_two_gap_states():
+    """The default partition function with a second, long-gap insert-state pair (G = 2): dearer to open, cheaper to
+    extend. Parameter values only (inputs), scaled by the default temperature 3."""
+    pf, T = inputs.default_pf(), 3.0
+    return inputs.Model(n_ins=2, alphabet=pf.alphabet, log_match=pf.log_match, log_ins=pf.log_ins, t_MM=0.0,
+                        t_MI=(pf.t_MI[0], -16.0 / T), t_II=(pf.t_II[0], -0.4 / T), t_IM=(0.0, 0.0), init_M=0.0,
+                        init_I=(pf.init_I[0], -16.0 / T), end_M=0.0, end_I=(0.0, 0.0))
+
+
+def test_g2_partition_function_split_classes_and_distance_pass(default_params):
+    """A partition function with TWO insert-state pairs through the fp32 SPLIT classes (launch_pair<float,2,C,*,4>,
+    C = 8, 12, 16: columns 700 / 1300 / 2000, and 2600 = more blocks than warps), once with the test outputs
+    (kModeFull) and once as the production instances (kModeCsr: no dense_P, no logZ), plus a near-identical pair so
+    that the fp64 distance-only kernels run with GP = 2 (launch_pair<double,2,C,kModeDist,8>)."""
+    qp = _qp()
+    rng = np.random.default_rng(11)
+    q = inputs.background()
+    prm = inputs.Params(hmm=default_params.hmm, pf=_pf_two_gap_states(), threshold=0.01)
+    seqs = [rng.choice(20, size=L, p=q).astype(np.uint8) for L in (700, 1300, 2000, 2600, 45)]
+    a = rng.choice(20, size=800, p=q).astype(np.uint8)
+    b = a.copy()
+    hit = rng.random(800) < 0.04
+    b[hit] = rng.choice(20, size=int(hit.sum()), p=q)
+    seqs += [a, np.delete(b, slice(400, 403))]
+    c = seqs[1].copy()                       # a diverged copy of the 1300-residue sequence: real structure in a wide pair
+    hit = rng.random(1300) < 0.5
+    c[hit] = rng.choice(20, size=int(hit.sum()), p=q)
+    seqs.append(c)
+    fam = inputs.pack(seqs)
+    pairs = np.array([[4, 0], [0, 4], [0, 1], [1, 2], [4, 3], [3, 4], [2, 0], [5, 6], [6, 5], [7, 1], [1, 7], [0, 3]],
+                     dtype=np.int32)
+    run = orc.Run(prm, fam, pairs, keep_dense=True)
+    assert float(run.dist.min()) < 0.25
+    full = qp.run_family(fam, pairs, prm, precision="fp32", want_dense=True, want_logZ=True)
+    _compare(fam, pairs, prm, full, run)
+    prod = qp.run_family(fam, pairs, prm, precision="fp32")
+    _compare(fam, pairs, prm, prod, run, dense=False, logZ=False)
+    assert int(full.status[3].item()) >= 2 and int(prod.status[3].item()) >= 2   # the fp64 distance pass ran (GP = 2)
+
+
+def test_g2_partition_function_production_instances_packed(default_params):
+    """launch_pair<float,2,C,kModeCsr,1> for every packed stripe width C = 2..16: column counts 40, 72, ... , 488 (one
+    per width), G = 2 partition function, production outputs only (CSR + distance) against the oracle's dense matrix."""
+    qp = _qp()
+    rng = np.random.default_rng(12)
+    q = inputs.background()
+    prm = inputs.Params(hmm=default_params.hmm, pf=_pf_two_gap_states(), threshold=0.01)
+    root = rng.choice(20, size=520, p=q).astype(np.uint8)
+    seqs = [root[:260].copy()]
+    for C in range(2, 17):                   # m + 1 <= 32 C and > 32 (C - 1): the narrowest class that holds it is C
+        s = root[: 32 * C - 24].copy()
+        hit = rng.random(len(s)) < 0.35
+        s[hit] = rng.choice(20, size=int(hit.sum()), p=q)
+        seqs.append(s)
+    fam = inputs.pack(seqs)
+    pairs = np.array([[0, j] for j in range(1, 16)] + [[j, j + 1] for j in range(1, 15)], dtype=np.int32)
+    run = orc.Run(prm, fam, pairs, keep_dense=True)
+    res = qp.run_family(fam, pairs, prm, precision="fp32")
+    _compare(fam, pairs, prm, res, run, dense=False, logZ=False)
+
+
 def test_nucleotide_mode_alphabet_4():
     """PAPER.md:69 nucleotide mode: alphabet 4 through the same kernels (synthetic 4-letter model, the HOXD/GTR
     tables are not in the container). Related sequences (12 % substitutions, a few indels), lengths 150-600."""
@@ -200,6 +260,18 @@ def test_error_paths(default_params):
     with pytest.raises(qp.QpError) as ei:
         qp.run_family(bad, pairs, default_params)
     assert ei.value.code == qp.ERR["BAD_RESIDUE"]
+    # bytes far outside the 32 x 32 emission table (255, and ASCII letters passed by mistake): the documented error,
+    # no out-of-range shared-memory access (the context stays usable: the next call below succeeds)
+    for junk in (255, None):
+        bad = inputs.Family(seqs=fam.seqs.copy(), offsets=fam.offsets.copy())
+        if junk is None:
+            bad.seqs[:] = np.frombuffer(b"ACDEFGHIKLMNPQRSTVWY", dtype=np.uint8)[bad.seqs % 20]
+        else:
+            bad.seqs[7] = junk
+        with pytest.raises(qp.QpError) as ei:
+            qp.run_family(bad, pairs, default_params)
+        assert ei.value.code == qp.ERR["BAD_RESIDUE"]
+        torch.cuda.synchronize()
     # empty pair list is fine
     res = qp.run_family(fam, np.zeros((0, 2), np.int32), default_params)
     assert res.code == 0 and int(res.pair_nnz_base[0].item()) == 0
