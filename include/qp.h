@@ -154,6 +154,66 @@ size_t qp_guide_tree_workspace_bytes(int32_t k);
 int qp_guide_tree(const float* d_dist, int32_t k, int32_t* d_merge, float* d_height, int32_t* d_leaves,
                   int32_t* d_parent, int32_t* d_treedist, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
 
+/*
+ * Stage III: selective consistency transformation of the sparse posterior matrices.
+ * "consistency relies on the relaxation of posterior probability matrices by other sequences";
+ * PAPER.md:55, :63 (Figure 2): "posterior matrix S_xy is relaxed over sequence z if assumed function f(d_xz, d_yz)
+ * fulfills given condition", d = the tree-guided distance, thresholded deterministically: f(d_xz, d_yz) <= T
+ * (best setting: maximum, T ~ 200); S_xy is amplified by h_xy, which "varies from 1
+ * when no relaxations of S_xy are performed, to h when maximum number of relaxations ... is done (200 in our case)",
+ * best h = 3; PAPER.md:59 footnote: the matrices are sparse. The paper prints no formula; the reading
+ * (the oracle oracle/qp_consistency.py follows the same):
+ *     sel(x,y) = { z != x, y : both pairs {x,z}, {z,y} are in the input and f(treedist[x][z], treedist[y][z]) <= T }
+ *     h_xy     = 1 + (h - 1) * min(|sel|, max_relax) / max_relax
+ *     S'_xy    = ( 2 h_xy S_xy + sum_{z in sel(x,y)} S_xz S_zy ) / ( 2 h_xy + |sel(x,y)| ),  S_zx = S_xz^T,
+ *                evaluated on the cells stored in S_xy only; values below `threshold` are dropped.
+ * Every relaxed matrix is computed from the INPUT matrices (one transformation = one call; 2 calls for
+ * k < 50, 1 otherwise -- qp_consistency_passes). Arithmetic: fp32, fixed summation order (reproducible).
+ *   in       the per-pair CSR that qp_posteriors wrote (same d_offsets / d_pairs); an unordered pair should be
+ *            listed once
+ *   nnz      HOST value: entries of the input, in->pair_nnz_base[P]
+ *   out      pair_nnz_base [P+1], row_ptr [sum(n_p+1)] (same row layout as the input: in->pair_row_base serves both),
+ *            col_idx / val [nnz_capacity]; nnz_capacity >= nnz always suffices (the pattern only shrinks);
+ *            relaxations: optional [P], |sel| of every pair; status [4] device status word {code, pair or -1, 0, 0}
+ * Errors: QP_ERR_INVALID_ARG; device-detected in out->status: QP_ERR_BAD_PAIR, QP_ERR_EMPTY_SEQUENCE,
+ * QP_ERR_WORKSPACE_TOO_SMALL, QP_ERR_NNZ_CAPACITY. Work is enqueued on the stream, nothing is synchronised. All
+ * device buffers are caller-owned; the workspace (qp_consistency_workspace_bytes, a host-only query on host copies
+ * of the offsets and pairs) holds the pair lookup table, interleaved copies of every matrix and of its transpose,
+ * and the staging area of the relaxed entries.
+ */
+enum { QP_SEL_MAX = 0, QP_SEL_MIN = 1, QP_SEL_SUM = 2 };
+typedef struct {
+    int32_t T;               /* selection threshold on f(treedist[x][z], treedist[y][z])                        */
+    int32_t f;               /* QP_SEL_MAX (the paper's best), QP_SEL_MIN or QP_SEL_SUM                          */
+    double h;                /* amplification of the original signal at max_relax relaxations, >= 1 (paper: 3)   */
+    int32_t max_relax;       /* relaxations at which h_xy reaches h (paper: 200)                                 */
+    int32_t reserved;
+    double threshold;        /* relaxed values below it are dropped (stage I's tau)                              */
+} qp_consistency_params;
+typedef struct {             /* per-pair CSR matrices, device, layout of qp_output                               */
+    const int64_t* pair_row_base;
+    const int64_t* pair_nnz_base;
+    const int32_t* row_ptr;
+    const int32_t* col_idx;
+    const float* val;
+} qp_csr;
+typedef struct {
+    int64_t* pair_nnz_base;
+    int32_t* row_ptr;
+    int32_t* col_idx;
+    float* val;
+    int64_t nnz_capacity;
+    int32_t* relaxations;    /* optional */
+    int32_t* status;
+} qp_csr_out;
+int qp_consistency_workspace_bytes(const int64_t* h_offsets, int32_t k, const int32_t* h_pairs, int64_t P, int64_t nnz,
+                                   size_t* out_bytes);
+int qp_consistency(const int64_t* d_offsets, int32_t k, const int32_t* d_pairs, int64_t P, const qp_csr* in, int64_t nnz,
+                   const int32_t* d_treedist, const qp_consistency_params* params, void* d_workspace,
+                   size_t workspace_bytes, const qp_csr_out* out, void* cuda_stream);
+/* "the number of transformations is adjusted to the number of sequences (2 for k < 50, 1 otherwise)". */
+int qp_consistency_passes(int32_t k);
+
 /* Number of kernels the last qp_posteriors call on this thread launched (bench.py's gpu_launches). */
 int qp_last_launch_count(void);
 

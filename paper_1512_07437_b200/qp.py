@@ -23,7 +23,8 @@ FLAG_SYNC_STATUS, FLAG_NO_REFINE = 1, 2
 NUM_CLASSES = 18
 
 EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_posteriors_budgeted", "qp_guide_tree", "qp_guide_tree_workspace_bytes", "qp_last_launch_count", "qp_status_string", "qp_version",
-           "qp_set_profile", "qp_get_profile", "qp_get_profile_classes", "qp_shutdown"]
+           "qp_set_profile", "qp_get_profile", "qp_get_profile_classes", "qp_shutdown",
+           "qp_consistency", "qp_consistency_workspace_bytes", "qp_consistency_passes"]
 
 
 class QpError(RuntimeError):
@@ -48,6 +49,24 @@ class _Output(C.Structure):
     _fields_ = [("pair_row_base", C.c_void_p), ("pair_nnz_base", C.c_void_p), ("row_ptr", C.c_void_p),
                 ("col_idx", C.c_void_p), ("val", C.c_void_p), ("nnz_capacity", C.c_int64), ("dist", C.c_void_p),
                 ("dense_P", C.c_void_p), ("logZ", C.c_void_p), ("status", C.c_void_p)]
+
+
+class _Csr(C.Structure):
+    _fields_ = [("pair_row_base", C.c_void_p), ("pair_nnz_base", C.c_void_p), ("row_ptr", C.c_void_p),
+                ("col_idx", C.c_void_p), ("val", C.c_void_p)]
+
+
+class _CsrOut(C.Structure):
+    _fields_ = [("pair_nnz_base", C.c_void_p), ("row_ptr", C.c_void_p), ("col_idx", C.c_void_p), ("val", C.c_void_p),
+                ("nnz_capacity", C.c_int64), ("relaxations", C.c_void_p), ("status", C.c_void_p)]
+
+
+class _ConsParams(C.Structure):
+    _fields_ = [("T", C.c_int32), ("f", C.c_int32), ("h", C.c_double), ("max_relax", C.c_int32), ("reserved", C.c_int32),
+                ("threshold", C.c_double)]
+
+
+SEL = {"max": 0, "min": 1, "sum": 2}
 
 
 def _load():
@@ -79,6 +98,13 @@ def _load():
     L.qp_get_profile_classes.restype = C.c_int
     L.qp_get_profile_classes.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]
     L.qp_shutdown.restype = None
+    L.qp_consistency_workspace_bytes.restype = C.c_int
+    L.qp_consistency_workspace_bytes.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.c_int64, C.POINTER(C.c_size_t)]
+    L.qp_consistency.restype = C.c_int
+    L.qp_consistency.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.POINTER(_Csr), C.c_int64, C.c_void_p,
+                                 C.POINTER(_ConsParams), C.c_void_p, C.c_size_t, C.POINTER(_CsrOut), C.c_void_p]
+    L.qp_consistency_passes.restype = C.c_int
+    L.qp_consistency_passes.argtypes = [C.c_int32]
     return L
 
 
@@ -323,3 +349,54 @@ def guide_tree(dist, want_treedist=True, stream=None, workspace=None) -> GuideTr
         raise QpError(code)
     t._ws = ws   # keep the workspace alive until the stream has run
     return t
+
+
+def consistency_passes(k: int) -> int:
+    """qp_consistency_passes: the paper's rule, 2 transformations for k < 50, 1 otherwise."""
+    return int(_lib.qp_consistency_passes(int(k)))
+
+
+def consistency(d_offsets, k, d_pairs, csr, treedist, *, h_offsets, h_pairs, nnz=None, T=200, f="max", h=3.0,
+                max_relax=200, threshold=0.01, stream=None, workspace=None, check=True) -> Result:
+    """qp_consistency (stage III, selective consistency) on torch CUDA tensors. `csr` = anything with the members
+    pair_row_base / pair_nnz_base / row_ptr / col_idx / val (a Result of `posteriors` or of a previous call);
+    `treedist` = int32 k x k (GuideTree.treedist). Marshalling only. Returns a Result whose pair_row_base is the
+    input's (rows do not change), with `.relaxations` (int32 [P]) attached. Synchronises once to read the status
+    (and, if `nnz` is not given, once to read the input's entry count)."""
+    import torch
+    dev = d_pairs.device
+    P = int(d_pairs.shape[0])
+    if nnz is None:
+        nnz = int(csr.pair_nnz_base[P].item()) if P else 0
+    h_offsets = np.ascontiguousarray(h_offsets, dtype=np.int64)
+    h_pairs = np.ascontiguousarray(h_pairs, dtype=np.int32).reshape(-1, 2)
+    need = C.c_size_t(0)
+    r = _lib.qp_consistency_workspace_bytes(h_offsets.ctypes.data, int(k), h_pairs.ctypes.data, P, int(nnz), C.byref(need))
+    if r != QP_OK:
+        raise QpError(r)
+    ws = workspace if workspace is not None else torch.empty(max(int(need.value), 256), dtype=torch.uint8, device=dev)
+    i64, i32, f32 = torch.int64, torch.int32, torch.float32
+    rows_total = int(csr.row_ptr.numel())
+    out = Result(pair_row_base=csr.pair_row_base, pair_nnz_base=torch.empty(P + 1, dtype=i64, device=dev),
+                 row_ptr=torch.empty(max(rows_total, 1), dtype=i32, device=dev),
+                 col_idx=torch.empty(max(int(nnz), 1), dtype=i32, device=dev),
+                 val=torch.empty(max(int(nnz), 1), dtype=f32, device=dev), dist=None, dense_P=None, dense_off=None,
+                 logZ=None, status=torch.zeros(4, dtype=i32, device=dev), code=0, launches=9)
+    out.relaxations = torch.zeros(max(P, 1), dtype=i32, device=dev)
+    ci = _Csr(csr.pair_row_base.data_ptr(), csr.pair_nnz_base.data_ptr(), csr.row_ptr.data_ptr(), csr.col_idx.data_ptr(),
+              csr.val.data_ptr())
+    co = _CsrOut(out.pair_nnz_base.data_ptr(), out.row_ptr.data_ptr(), out.col_idx.data_ptr(), out.val.data_ptr(), int(nnz),
+                 out.relaxations.data_ptr(), out.status.data_ptr())
+    prm = _ConsParams(int(T), SEL[f] if isinstance(f, str) else int(f), float(h), int(max_relax), 0, float(threshold))
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    with torch.cuda.device(dev):
+        code = _lib.qp_consistency(d_offsets.data_ptr(), int(k), d_pairs.data_ptr(), P, C.byref(ci), int(nnz),
+                                   treedist.data_ptr(), C.byref(prm), ws.data_ptr(), ws.numel(), C.byref(co),
+                                   C.c_void_p(st.cuda_stream))
+    out._ws = ws
+    if code == QP_OK and check:
+        code = int(out.status[0].item())      # synchronises
+    out.code = int(code)
+    if check and code != QP_OK:
+        raise QpError(code)
+    return out
