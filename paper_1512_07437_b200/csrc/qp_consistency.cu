@@ -12,11 +12,13 @@
 //   k_cs_index      pair lookup table pair_of[k][k] -> (pair, orientation); per-pair column counts
 //   k_cs_transpose  per pair: an interleaved (value, column) copy of the matrix and its transpose (value, row), so
 //                   that EVERY oriented matrix S_ab (rows = residues of a) is a row-compressed list of 8-byte entries
-//   k_cs_relax      one CTA per pair, one warp per row i of S_xy, lane q owns the q-th stored cell (i, c_q) of the row:
+//   k_cs_relax      one CTA per pair; for every selected z (outer loop) the warps take the rows i of S_xy, lane q owns
+//                   the q-th stored cell (i, c_q) of the row:
 //                   S_xz S_zy (i, c_q) = sum_k S_xz(i,k) S_yz(c_q,k) = <row i of S_xz , row c_q of S_yz>. The warp
 //                   spreads row i of S_xz into a dense window over k in shared memory; every lane walks its own row
 //                   of S_yz and gathers from the window: no atomics, no search, a fixed summation order (z ascending,
-//                   k ascending), so the result is reproducible bit for bit.
+//                   k ascending), so the result is reproducible bit for bit. With z outermost the two factor
+//                   matrices stream through L1 once per (pair, z); the accumulators sit in shared memory.
 //   k_scan / k_cs_place   kept entries -> the caller's CSR in pair order.
 #include <cuda_runtime.h>
 
@@ -29,8 +31,9 @@ namespace qp {
 
 constexpr int kCsThreads = 256;
 constexpr int kCsWarps = kCsThreads / 32;
-constexpr int kCsWin = 128;          // dense window over k (floats per warp)
-constexpr int kCsList = 512;         // selected sequences held in shared memory at a time
+constexpr int kCsWin = 128;          // generic routine: dense window over k (floats per warp)
+constexpr int kCsList = kCsThreads;  // selected sequences held in shared memory at a time: one block of candidates
+constexpr int kCsAcc = 8192;         // accumulators (cells of S_xy) held in shared memory; larger pairs use the staging area
 constexpr unsigned kAll = 0xffffffffu;
 
 struct CsHeader {
@@ -138,6 +141,9 @@ __global__ void __launch_bounds__(kCsThreads) k_cs_transpose(CsArgs a) {
         if (p == 0 && threadIdx.x == 0) cs_status(a.hdr, QP_ERR_WORKSPACE_TOO_SMALL, -1);
         return;
     }
+    // S_xz is a factor of some relaxation only if f(d_xz, .) <= T is possible: for max and sum that needs d_xz <= T
+    // (distances are >= 0). Copies of the other pairs are never read.
+    if (a.f != QP_SEL_MIN && a.treedist[(int64_t)x * a.k + y] > a.T) return;
     const int32_t* rp = a.row_ptr + a.row_base[p];
     const int64_t base = a.nnz_base[p];
     const int cnt = rp[n];
@@ -199,29 +205,95 @@ __device__ __forceinline__ bool cs_oriented(const CsArgs& a, int ra, int rb, con
     return true;
 }
 
+// ---- the inner routine of the relaxation ----------------------------------------------------------------------------
+// Adds, for one selected z, <row i of S_xz, row c of S_yz> to the accumulator of the stored cells (i, c) of row i of
+// S_xy, cells [lo, hi), 32 at a time (one per lane). Any row lengths, any spread of k: row i of S_xz is spread into a
+// dense window over k in shared memory, kCsWin wide, as many windows as its spread needs (normally one); every lane
+// walks its own row of S_yz and gathers from the window. `w` is the warp's window, all zero between uses.
+template <typename AccT>
+__device__ __forceinline__ void cs_row_generic(const CsZ& Z, int i, int lo, int hi, const int32_t* __restrict__ colxy,
+                                               AccT accum, float* w, int lane) {
+    const int a0 = Z.rpA[i], a1 = Z.rpA[i + 1];
+    if (a0 == a1) return;                                  // warp-uniform: x_i has no partner in z
+    for (int qb = lo; qb < hi; qb += 32) {
+        const int e = qb + lane;
+        const bool have = e < hi;
+        int b0 = 0, b1 = 0;
+        if (have) {
+            const int cq = __ldg(colxy + e);
+            b0 = Z.rpB[cq];
+            b1 = Z.rpB[cq + 1];
+        }
+        float accv = 0.f;
+        for (int ab = a0; ab < a1; ab += 32) {             // row i of S_xz, 32 entries at a time
+            const bool ha = ab + lane < a1;
+            float av = 0.f;
+            int ak = 0;
+            if (ha) {
+                const float2 t = __ldg(Z.entA + ab + lane);
+                av = t.x;
+                ak = __float_as_int(t.y);
+            }
+            const int na = min(32, a1 - ab);
+            const int kmin = __shfl_sync(kAll, ak, 0), kmax = __shfl_sync(kAll, ak, na - 1);
+            for (int wb = kmin; wb <= kmax; wb += kCsWin) {   // dense window over k (normally one)
+                const bool inw = ha && (unsigned)(ak - wb) < (unsigned)kCsWin;
+                if (inw) w[ak - wb] = av;
+                __syncwarp();
+                // row c_q of S_yz against the window, four entries per round of loads; entries outside the window
+                // meet zeros or fail the range test
+                for (int b = b0; b < b1; b += 4) {
+                    float2 t[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u)
+                        t[u] = b + u < b1 ? __ldg(Z.entB + b + u) : make_float2(0.f, __int_as_float(-(1 << 30)));
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int d = __float_as_int(t[u].y) - wb;
+                        if ((unsigned)d < (unsigned)kCsWin) accv = fmaf(w[d], t[u].x, accv);
+                    }
+                }
+                __syncwarp();
+                if (inw) w[ak - wb] = 0.f;
+            }
+        }
+        if (have) accum(e, accv);
+    }
+}
+
+// One CTA per pair (x, y). The selected sequences are taken a block of candidates at a time, in ascending order; for
+// every selected z (outer loop, the whole CTA on the same z so that its two matrices stream through L1 once) the
+// warps take the rows of S_xy (inner loop) and add <row i of S_xz, row c of S_yz> to the accumulator of every stored
+// cell (i, c). Pairs with at most kCsAcc cells keep the accumulators in shared memory, larger ones in the staging area.
 __global__ void __launch_bounds__(kCsThreads) k_cs_relax(CsArgs a) {
     __shared__ CsZ zl[kCsList];
     __shared__ float win[kCsWarps][kCsWin];
+    __shared__ float acc_s[kCsAcc];                                  // accumulators of S_xy's stored cells
     __shared__ int32_t sh[kCsThreads];
     __shared__ int wcnt[kCsWarps];
-    __shared__ int fill, rtot;
+    __shared__ int rtot;
     const int64_t p = blockIdx.x;
     if (a.hdr->status[0] != 0) return;
     const int x = a.pairs[2 * p], y = a.pairs[2 * p + 1];
     const int n = (int)(a.offs[x + 1] - a.offs[x]);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int32_t* rp = a.row_ptr + a.row_base[p];
+    const int32_t* __restrict__ rp = a.row_ptr + a.row_base[p];
     const int64_t base = a.nnz_base[p];
-    const float2* exy = a.ent + base;
+    const int cnt = rp[n];
+    const int32_t* __restrict__ colxy = a.col_idx + base;
+    const float* __restrict__ valxy = a.val + base;
     float2* tmp = a.tmp + base;
     int32_t* orp = a.out_row_ptr + a.row_base[p];
     const int32_t* tdx = a.treedist + (int64_t)x * a.k;
     const int32_t* tdy = a.treedist + (int64_t)y * a.k;
-    if (tid == 0) fill = rtot = 0;
+    const bool cached = cnt <= kCsAcc;                   // CTA-uniform: the accumulators live in shared memory
+    float* w = win[warp];
+    for (int u = lane; u < kCsWin; u += 32) w[u] = 0.f;   // the window is all zero between uses
+    if (tid == 0) rtot = 0;
     __syncthreads();
-    bool first = true;
-    for (int z0 = 0; z0 < a.k || first; z0 += kCsThreads) {
-        // ---- selection: candidates z0 .. z0+255, appended to the list in ascending order -------------
+    bool touched = false;
+    for (int z0 = 0; z0 < a.k; z0 += kCsThreads) {
+        // ---- selection: candidates z0 .. z0+255, listed in ascending order ---------------------------
         const int z = z0 + tid;
         CsZ mine;
         bool sel = false;
@@ -233,106 +305,84 @@ __global__ void __launch_bounds__(kCsThreads) k_cs_relax(CsArgs a) {
         const unsigned bal = __ballot_sync(kAll, sel);
         if (lane == 0) wcnt[warp] = __popc(bal);
         __syncthreads();
-        int off = fill;
-        for (int w = 0; w < warp; ++w) off += wcnt[w];
+        int off = 0, nz = 0;
+        for (int q = 0; q < kCsWarps; ++q) {
+            if (q < warp) off += wcnt[q];
+            nz += wcnt[q];
+        }
         if (sel) zl[off + __popc(bal & ((1u << lane) - 1))] = mine;
-        __syncthreads();
-        if (tid == 0) {
-            int c = 0;
-            for (int w = 0; w < kCsWarps; ++w) c += wcnt[w];
-            fill += c;
-            rtot += c;
+        if (tid == 0) rtot += nz;
+        if (nz > 0 && !touched) {   // CTA-uniform: the first selected sequences of this pair
+            if (cached) for (int e = tid; e < cnt; e += kCsThreads) acc_s[e] = 0.f;
+            else for (int e = tid; e < cnt; e += kCsThreads) tmp[e].x = 0.f;
+            touched = true;
         }
         __syncthreads();
-        const bool last = z0 + kCsThreads >= a.k;
-        if (!last && fill + kCsThreads <= kCsList) continue;   // room for another block of candidates
-        // ---- relax every row over the listed sequences -------------------------------------------------------------
-        const int nz = fill, r = rtot;
-        const float hxy = 1.f + (a.h - 1.f) * (float)min(r, a.max_relax) / (float)a.max_relax;
-        const float w2 = 2.f * hxy, inv = 1.f / (w2 + (float)r);
-        float* w = win[warp];
-        for (int i = warp; i < n; i += kCsWarps) {
-            const int s0 = rp[i], s1 = rp[i + 1];
-            int kept = 0;
-            for (int qb = s0; qb < s1; qb += 32) {
-                const int e = qb + lane;
-                const bool have = e < s1;
-                float sxy = 0.f;
-                int cq = 0;
-                if (have) {
-                    const float2 t = exy[e];
-                    sxy = t.x;
-                    cq = __float_as_int(t.y);
-                }
-                float acc = (have && !first) ? tmp[e].x : 0.f;
-                for (int q = 0; q < nz; ++q) {
-                    const CsZ Z = zl[q];
-                    const int a0 = Z.rpA[i], a1 = Z.rpA[i + 1];
-                    if (a0 == a1) continue;                    // warp-uniform: x_i has no partner in z
-                    int b0 = 0, b1 = 0;
-                    if (have) {
-                        b0 = Z.rpB[cq];
-                        b1 = Z.rpB[cq + 1];
-                    }
-                    for (int ab = a0; ab < a1; ab += 32) {     // row i of S_xz, 32 entries at a time
-                        const bool ha = ab + lane < a1;
-                        float av = 0.f;
-                        int ak = 0;
-                        if (ha) {
-                            const float2 t = Z.entA[ab + lane];
-                            av = t.x;
-                            ak = __float_as_int(t.y);
-                        }
-                        const int na = min(32, a1 - ab);
-                        const int kmin = __shfl_sync(kAll, ak, 0), kmax = __shfl_sync(kAll, ak, na - 1);
-                        for (int wb = kmin; wb <= kmax; wb += kCsWin) {   // dense window over k
-                            __syncwarp();
-                            for (int u = lane; u < kCsWin; u += 32) w[u] = 0.f;
-                            __syncwarp();
-                            if (ha && (unsigned)(ak - wb) < (unsigned)kCsWin) w[ak - wb] = av;
-                            __syncwarp();
-                            const int whi = min(kmax, wb + kCsWin - 1);
-                            // row c_q of S_yz: entries ascending in k; skip those before the window, stop after it
-                            while (b0 < b1) {
-                                const float2 t = Z.entB[b0];
-                                const int bk = __float_as_int(t.y);
-                                if (bk > whi) break;
-                                if (bk >= wb) acc = fmaf(w[bk - wb], t.x, acc);
-                                ++b0;
-                            }
-                        }
-                    }
-                }
-                if (!last) {
-                    if (have) tmp[e].x = acc;
-                } else {
-                    // ---- amplify, normalise, threshold; kept entries are packed at the start of the row --------
-                    const float v = fmaf(w2, sxy, acc) * inv;
-                    const bool keep = have && v >= a.tau;
-                    const unsigned kb = __ballot_sync(kAll, keep);
-                    __syncwarp();
-                    if (keep) tmp[s0 + kept + __popc(kb & ((1u << lane) - 1))] = make_float2(v, __int_as_float(cq));
-                    kept += __popc(kb);
-                }
+        // ---- relax over the listed sequences ------------------------------------------------------------------------
+        for (int q = 0; q < nz; ++q) {
+            const CsZ Z = zl[q];
+            if (cached) {
+                auto add_s = [&](int e, float v) { acc_s[e] += v; };
+                for (int i = warp; i < n; i += kCsWarps) cs_row_generic(Z, i, rp[i], rp[i + 1], colxy, add_s, w, lane);
+            } else {
+                auto add_g = [&](int e, float v) { tmp[e].x += v; };
+                for (int i = warp; i < n; i += kCsWarps) cs_row_generic(Z, i, rp[i], rp[i + 1], colxy, add_g, w, lane);
             }
-            if (last && lane == 0) orp[i] = kept;
         }
-        first = false;
-        __syncthreads();
-        if (tid == 0) fill = 0;
-        __syncthreads();
-        if (last) break;
+        __syncthreads();   // the list is rebuilt by the next block of candidates
     }
+    // ---- amplify, normalise, threshold; kept entries are packed at the start of their row ------------
+    const int r = rtot;
+    if (!touched) {   // nothing selected: S' = S, the placement copies the input entries themselves
+        for (int i = tid; i <= n; i += kCsThreads) orp[i] = rp[i];
+        if (tid == 0) {
+            a.nnz_pair[p] = -cnt - 1;                          // negative: "copy from the input"
+            if (a.relaxations) a.relaxations[p] = 0;
+        }
+        return;
+    }
+    const float hxy = 1.f + (a.h - 1.f) * (float)min(r, a.max_relax) / (float)a.max_relax;
+    const float w2 = 2.f * hxy, inv = 1.f / (w2 + (float)r);
+    for (int i = warp; i < n; i += kCsWarps) {
+        const int s0 = rp[i], s1 = rp[i + 1];
+        int kept = 0;
+        for (int qb = s0; qb < s1; qb += 32) {
+            const int e = qb + lane;
+            const bool have = e < s1;
+            float v = 0.f;
+            int cq = 0;
+            if (have) {
+                cq = colxy[e];
+                v = fmaf(w2, valxy[e], cached ? acc_s[e] : tmp[e].x) * inv;
+            }
+            const bool keep = have && v >= a.tau;
+            const unsigned kb = __ballot_sync(kAll, keep);
+            if (keep) tmp[s0 + kept + __popc(kb & ((1u << lane) - 1))] = make_float2(v, __int_as_float(cq));
+            kept += __popc(kb);
+        }
+        if (lane == 0) orp[i] = kept;
+    }
+    __syncthreads();
     // ---- row counts -> row pointer of the relaxed pair ---------------------------------------------------------------
     const int total = block_scan_inplace(orp, n, sh);
     if (tid == 0) {
         orp[n] = total;
         a.nnz_pair[p] = total;
-        if (a.relaxations) a.relaxations[p] = rtot;
+        if (a.relaxations) a.relaxations[p] = r;
     }
 }
 
-__global__ void __launch_bounds__(kCsThreads) k_cs_place(CsArgs a) {
+// nnz_pair holds -(count) - 1 for the pairs that were not relaxed: make it the count and keep the sign as a flag
+// for the placement
+__global__ void k_cs_counts(CsArgs a, int32_t* flags) {
+    const int64_t p = blockIdx.x * (int64_t)blockDim.x + threadIdx.x;
+    if (p >= a.P) return;
+    const int v = a.nnz_pair[p];
+    flags[p] = v < 0;
+    if (v < 0) a.nnz_pair[p] = -v - 1;
+}
+
+__global__ void __launch_bounds__(kCsThreads) k_cs_place(CsArgs a, const int32_t* __restrict__ flags) {
     const int64_t p = blockIdx.x;
     if (a.hdr->status[0] != 0) return;
     const int x = a.pairs[2 * p];
@@ -340,14 +390,20 @@ __global__ void __launch_bounds__(kCsThreads) k_cs_place(CsArgs a) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int32_t* rp = a.row_ptr + a.row_base[p];
     const int32_t* orp = a.out_row_ptr + a.row_base[p];
-    const float2* tmp = a.tmp + a.nnz_base[p];
-    const int64_t ob = a.out_nnz_base[p];
+    const int64_t ib = a.nnz_base[p], ob = a.out_nnz_base[p];
     if (ob + orp[n] > a.out_cap) {
-        if (threadIdx.x == 0) {
-            cs_status(a.hdr, QP_ERR_NNZ_CAPACITY, (int)p);
+        if (threadIdx.x == 0) cs_status(a.hdr, QP_ERR_NNZ_CAPACITY, (int)p);
+        return;
+    }
+    if (flags[p]) {   // not relaxed: the input entries, unchanged
+        const int c = orp[n];
+        for (int e = threadIdx.x; e < c; e += kCsThreads) {
+            a.out_val[ob + e] = a.val[ib + e];
+            a.out_col[ob + e] = a.col_idx[ib + e];
         }
         return;
     }
+    const float2* tmp = a.tmp + ib;
     for (int i = warp; i < n; i += kCsWarps) {
         const int s0 = rp[i], d0 = orp[i], c = orp[i + 1] - d0;
         for (int q = lane; q < c; q += 32) {
@@ -365,7 +421,7 @@ __global__ void k_cs_finish(const CsHeader* h, int32_t* status) {
 static inline int64_t al256(int64_t v) { return (v + 255) & ~(int64_t)255; }
 
 struct CsLayout {
-    int64_t hdr, pair_of, cols1, col_base, ent, tmp, nnz_pair, rpT, curT, total;
+    int64_t hdr, pair_of, cols1, col_base, ent, tmp, nnz_pair, flags, rpT, curT, total;
 };
 static CsLayout cs_layout(int32_t k, int64_t P, int64_t nnz, int64_t cols_total) {
     CsLayout L;
@@ -382,6 +438,7 @@ static CsLayout cs_layout(int32_t k, int64_t P, int64_t nnz, int64_t cols_total)
     L.ent = take(2 * nnz * 8);
     L.tmp = take(nnz * 8);
     L.nnz_pair = take(P * 4);
+    L.flags = take(P * 4);
     L.rpT = take(cols_total * 4);     // the two arrays sized by sum(m_p + 1) come last: the device checks the sum
     L.curT = take(cols_total * 4);
     L.total = o;
@@ -475,8 +532,10 @@ extern "C" int qp_consistency(const int64_t* d_offsets, int32_t k, const int32_t
     k_scan<int32_t><<<1, 1024, 0, st>>>(a.cols1, P, a.col_base);
     k_cs_transpose<<<(int)P, kCsThreads, 0, st>>>(a);
     k_cs_relax<<<(int)P, kCsThreads, 0, st>>>(a);
+    int32_t* flags = (int32_t*)(ws + L.flags);
+    k_cs_counts<<<(int)((P + 255) / 256), 256, 0, st>>>(a, flags);
     k_scan<int32_t><<<1, 1024, 0, st>>>(a.nnz_pair, P, a.out_nnz_base);
-    k_cs_place<<<(int)P, kCsThreads, 0, st>>>(a);
+    k_cs_place<<<(int)P, kCsThreads, 0, st>>>(a, flags);
     k_cs_finish<<<1, 32, 0, st>>>(a.hdr, out->status);
     QP_CS(cudaGetLastError());
 #undef QP_CS
