@@ -161,8 +161,8 @@ def measure(cfg, steps, warmup, dev, prm, rank=0, world=1, shard=False, sample_c
         fam = inputs.config_family(cfg)
     all_pairs = inputs.all_pairs(fam.k)
     L = fam.lengths
-    mine = multi.shard_pairs(all_pairs, L, world, rank) if shard else np.arange(len(all_pairs))
-    pairs = np.ascontiguousarray(all_pairs[mine])
+    sharded = multi.ShardedFamily(L, all_pairs, world, rank) if shard else None
+    pairs = sharded.pairs if shard else all_pairs
     n, m = L[pairs[:, 0]].astype(np.int64), L[pairs[:, 1]].astype(np.int64)
     my_cells, rows_total = int((n * m).sum()), int((n + 1).sum())
     total_cells = my_cells
@@ -199,15 +199,19 @@ def measure(cfg, steps, warmup, dev, prm, rank=0, world=1, shard=False, sample_c
     state = {"res": None}
     xbuf = torch.empty_like(dist) if shard else None
 
-    def step():
+    def run_shard(_pairs=None):
         r = qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp_async, ws, reuse=state["res"], **out_kw)
         state["res"] = r
+        return r.dist
+
+    def step():
         if shard:
             # the one exchange of the path: every rank's distance entries (disjoint supports) summed over NCCL
-            # (on a copy: the next step rewrites this rank's own entries of `dist` in place)
-            xbuf.copy_(r.dist)
-            multi.exchange_distances(xbuf)
-        return r
+            # (in a second buffer: the next step rewrites this rank's own entries of `dist` in place)
+            sharded.step(run_shard, exchange_buffer=xbuf)
+        else:
+            run_shard()
+        return state["res"]
 
     for _ in range(max(warmup, 3)):
         res = step()
@@ -283,6 +287,74 @@ def roofline_of(cfg, m, clocks):
                                                "linear-space block floating point and issues 1 MUFU per cell"}}
 
 
+def measure_stage3(cfg, dev, prm, T=200, steps=3):
+    """Stage II (qp_guide_tree) + stage III (qp_consistency, the paper's best setting: maximum, T = 200, h = 3) on the
+    device-resident stage-I output of configs[cfg]. Reports relaxations/s and the algorithmic traffic of the relaxation:
+    every relaxation (x, y, z) reads S_xz and S_yz once, 8 bytes per stored entry."""
+    import torch
+    from paper_1512_07437_b200 import inputs, qp
+    fam = inputs.config_family(cfg)
+    pairs = inputs.all_pairs(fam.k)
+    res = qp.run_family(fam, pairs, prm, beta_guess=0.05)
+    d_offs = torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev)
+    d_pairs = torch.from_numpy(pairs).to(dev)
+    nnz = int(res.pair_nnz_base[-1].item())
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    t_tree, t_cons = [], []
+    for it in range(steps + 1):
+        e0.record()
+        tree = qp.guide_tree(res.dist)
+        e1.record()
+        r3 = qp.consistency(d_offs, fam.k, d_pairs, res, tree.treedist, h_offsets=fam.offsets, h_pairs=pairs, nnz=nnz, T=T,
+                            threshold=prm.threshold, check=False)
+        e2.record()
+        torch.cuda.synchronize()
+        assert int(r3.status[0].item()) == 0
+        if it:                                   # the first round is the warm-up
+            t_tree.append(e0.elapsed_time(e1))
+            t_cons.append(e1.elapsed_time(e2))
+    rel = r3.relaxations[: len(pairs)].to(torch.int64)
+    td_ = tree.treedist.cpu().numpy()
+    A = td_ <= T
+    np.fill_diagonal(A, False)
+    N = np.zeros((fam.k, fam.k))
+    d = np.diff(res.pair_nnz_base.cpu().numpy())
+    N[pairs[:, 0], pairs[:, 1]] = d
+    N[pairs[:, 1], pairs[:, 0]] = d
+    algo_bytes = 8.0 * float(((A * N).sum(0) * (A.sum(0) - 1)).sum())
+    ms = float(np.median(t_cons))
+    hbm_peak, peak_src = peaks()
+    return {"workload": f"configs[{cfg}] stage-I output: {len(pairs)} sparse matrices, {nnz} entries", "T": T, "f": "max", "h": 3.0,
+            "guide_tree_ms": float(np.median(t_tree)), "consistency_ms": ms, "relaxations": int(rel.sum().item()),
+            "pairs_relaxed": int((rel > 0).sum().item()), "max_relaxations": int(rel.max().item()),
+            "relaxations_per_s": float(rel.sum().item()) / (ms * 1e-3), "nnz_out": int(r3.pair_nnz_base[-1].item()),
+            "roofline": {"bound": "hbm", "achieved": algo_bytes / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                         "frac": algo_bytes / (ms * 1e-3) / 1e9 / hbm_peak, "algorithmic_bytes": algo_bytes,
+                         "note": "algorithmic bytes = 8 B x (nnz(S_xz) + nnz(S_yz)) summed over every relaxation (no reuse "
+                                 "assumed); the kernel is instruction-bound, not bandwidth-bound (profiles/r02_stage3.md)"}}
+
+
+def beta_vs_tau(cfg, dev, prm):
+    """PAPER.md:73 memory-limited mode: the sparsity coefficient beta = nnz / cells as a function of the threshold,
+    read off the histogram that qp_posteriors_budgeted builds in its first pass."""
+    import torch
+    from paper_1512_07437_b200 import inputs, qp
+    fam = inputs.config_family(cfg)
+    pairs = inputs.all_pairs(fam.k)
+    L = fam.lengths
+    cells = int((L[pairs[:, 0]].astype(np.int64) * L[pairs[:, 1]]).sum())
+    cap = int(0.06 * cells) + 4096
+    cp = qp.CParams(prm)
+    ws = torch.empty(qp.workspace_bytes(fam.offsets, fam.k, pairs, cp, cap), dtype=torch.uint8, device=dev)
+    args = (torch.from_numpy(fam.seqs).to(dev), torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev), fam.k,
+            torch.from_numpy(pairs).to(dev), cp, ws)
+    res = qp.posteriors(*args, nnz_capacity=cap, h_rows_total=int((L[pairs[:, 0]] + 1).sum()), budget_passes=2)
+    tau, cnt = qp.last_tau_curve()
+    pick = [b for b in range(0, len(tau), 8) if tau[b] <= 0.9]                     # every half octave
+    return {"cells": cells, "passes": res.passes, "tau": [float(tau[b]) for b in pick],
+            "beta": [float(cnt[b]) / cells for b in pick]}
+
+
 def run_ours(args):
     import torch
     import torch.distributed as td
@@ -336,6 +408,13 @@ def run_ours(args):
                 "roofline": {k: rc[k] for k in ("bound", "achieved", "peak", "unit", "frac", "kernel_ms", "kernel_frac",
                                                 "phases_ms")}}
             del mc
+
+    # ---- the NEXT rows of SURVEY.md 8(f) in the same run: stage II + III on configs[2]'s stage-I output, and the
+    # beta-vs-tau curve of the memory-limited mode ---------------------------------------------------------------------
+    if rank == 0 and world == 1 and args.config == 3 and not args.no_configs:
+        torch.cuda.empty_cache()
+        line["stage3"] = measure_stage3(2, dev, prm)
+        line["beta_vs_tau"] = {str(c): beta_vs_tau(c, dev, prm) for c in (1, 2)}
 
     # ---- end to end through the public call with HOST buffers (pinned): H2D of the inputs, D2H of every output --
     if world == 1 and not args.no_e2e:

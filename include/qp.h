@@ -120,19 +120,28 @@ int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, co
                   void* cuda_stream);
 
 /*
- * Memory-limited mode ("a memory-limited mode ... by decreasing sparsity coefficient"; PAPER.md:192:
- * memory for the posterior matrices is the limit on the set size). The caller's CSR capacity out->nnz_capacity is the
- * budget (8 bytes per entry); if the CSR at params->threshold does not fit, the threshold is raised and the pass is
- * repeated, at most max_passes times in all: tau <- tau * max(1.25, (required / capacity)^1.5) with `required` the
- * entry count the failed pass reported. On success *tau_used is the threshold the returned CSR was cut at and
- * *passes the number of passes run; every output is exactly what qp_posteriors returns for that threshold.
- * Synchronises the stream after every pass (it has to read the status). Returns QP_ERR_NNZ_CAPACITY if max_passes
- * did not suffice (pair_nnz_base[P] = entries required at the last threshold, *tau_used = that threshold), any other
- * error of qp_posteriors unchanged. tau_used and passes are HOST pointers (may be NULL).
+ * Memory-limited mode ("fit analysis in user-specified amount of RAM by decreasing sparsity coefficient in
+ * posterior matrices"; memory for the posterior matrices limits the set size). The caller's CSR capacity
+ * out->nnz_capacity is the budget (8 bytes per entry). At most TWO passes of the stage:
+ *   pass 1  qp_posteriors at params->threshold; on the way every kept value is counted into threshold bins (16 per
+ *           octave above the threshold). If the CSR fits, that is the result (*passes = 1).
+ *   pass 2  otherwise the smallest bin edge tau' whose count of values >= tau' fits the capacity is taken from the
+ *           histogram -- exactly, since the second pass recomputes the very same values -- and the stage is run again
+ *           at tau' (*passes = 2).
+ * On success *tau_used is the threshold the returned CSR was cut at; every output is exactly what qp_posteriors
+ * returns for that threshold. Synchronises the stream after every pass. Returns QP_ERR_NNZ_CAPACITY if max_passes is 1
+ * and the CSR does not fit, or if not even the top bin fits (pair_nnz_base[P] = entries required at the last threshold
+ * tried, *tau_used = that threshold); any other error of qp_posteriors unchanged. tau_used and passes are HOST
+ * pointers (may be NULL).
+ * qp_last_tau_curve: the histogram of the last qp_posteriors_budgeted call of this thread as a curve: tau[b] = lower
+ * edge of bin b (tau[0] = the requested threshold), count[b] = kept values >= tau[b] (so count[b] / cells is the
+ * sparsity coefficient beta at threshold tau[b]). Returns the number of bins written (<= max_bins, 128
+ * in all) or QP_ERR_INVALID_ARG if there is no histogram. HOST pointers.
  */
 int qp_posteriors_budgeted(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, const int32_t* d_pairs, int64_t P,
                            const qp_params* params, void* d_workspace, size_t workspace_bytes, const qp_output* out,
                            void* cuda_stream, int max_passes, double* tau_used, int* passes);
+int qp_last_tau_curve(double* tau, int64_t* count, int max_bins);
 
 /*
  * Stage II ("pairwise distances ... are given as an input for weighted UPGMA

@@ -277,6 +277,10 @@ __global__ void k_finish(const SchedHeader* h, int32_t* status) {
 // ------------------------------------------------------------------------------------------------------------
 static thread_local int g_launches = 0;
 static thread_local int g_profile = 0;
+static thread_local bool g_want_hist = false;                      // set by qp_posteriors_budgeted around its passes
+static thread_local unsigned long long g_tau_hist[kTauBins];      // host copy of the last budgeted call's histogram
+static thread_local float g_tau0 = 0.f;
+static thread_local bool g_tau_hist_valid = false;
 
 // Per host thread and device: side streams so that the per-class kernels overlap their tails, the events that fork
 // and join them, and the profiling events. Created on the first call on a device, kept until qp_shutdown().
@@ -351,7 +355,7 @@ static void prof_mark(Ctx* c, int i, cudaStream_t st) {
 static inline int64_t align256(int64_t v) { return (v + 255) & ~(int64_t)255; }
 
 struct Layout {   // byte offsets inside the workspace
-    int64_t hdr, info, order, rows1, cells, nnz, pool_off, dense_off, slot_off, refine_list, pool, slots;
+    int64_t hdr, info, order, rows1, cells, nnz, pool_off, dense_off, slot_off, refine_list, tau_hist, pool, slots;
     int64_t fixed;   // everything before the slots
 };
 
@@ -373,6 +377,7 @@ static Layout make_layout(int64_t P, int64_t nnz_cap, bool dense, int64_t max_sl
     L.dense_off = take(dense ? (P + 1) * 8 : 0);
     L.slot_off = take(max_slots * 8);
     L.refine_list = take((int64_t)kNumRefine * (P + kListPad) * 4);
+    L.tau_hist = take((int64_t)kTauBins * 8);
     L.pool = take(nnz_cap * 8);
     L.slots = o;
     L.fixed = o;
@@ -511,6 +516,8 @@ template <typename R> static void fill_common(KArgs<R>& ka, const uint8_t* d_seq
     ka.refine_list = (int32_t*)(ws + L.refine_list);
     ka.refine_stride = P + kListPad;
     ka.producers_total = 0;
+    ka.tau_hist = nullptr;
+    ka.tau_bits0 = 0;
     ka.refine_cmask = kMaskRefine;
     ka.pair_row_base = out->pair_row_base;
     ka.row_ptr = out->row_ptr;
@@ -693,6 +700,13 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
         ka64->refine_below = -1.0f;
     }
 
+    if (g_want_hist) {   // memory-limited mode: histogram of the kept values over threshold bins (qp_posteriors_budgeted)
+        float t0 = (float)params->threshold;
+        int32_t bits;
+        memcpy(&bits, &t0, 4);
+        ka32->tau_hist = ka64->tau_hist = (unsigned long long*)(ws + L.tau_hist);
+        ka32->tau_bits0 = ka64->tau_bits0 = bits;
+    }
     bool forked = false;
     auto fail = [&](int code) {
         if (forked)
@@ -709,6 +723,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     prof_mark(cx, 0, st);
     QP_TRY(cudaMemsetAsync(ws + L.nnz, 0, (size_t)P * 4, st));
     if (refine) QP_TRY(cudaMemsetAsync(ws + L.refine_list, 0xff, (size_t)kNumRefine * (P + kListPad) * 4, st));   // -1 = empty
+    if (g_want_hist) QP_TRY(cudaMemsetAsync(ws + L.tau_hist, 0, (size_t)kTauBins * 8, st));
 
     // ---- a0: schedule, entirely on the device --------------------------------------------------------------
     const uint32_t cmask = fp64 ? kMaskF64 : kMaskF32;
@@ -846,26 +861,63 @@ extern "C" int qp_posteriors_budgeted(const uint8_t* d_seqs, const int64_t* d_of
                                       const qp_output* out, void* cuda_stream, int max_passes, double* tau_used,
                                       int* passes) {
     if (!params || !out || max_passes < 1) return QP_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
     qp_params prm = *params;
     prm.flags |= QP_FLAG_SYNC_STATUS;
-    int r = QP_OK, launches = 0, done = 0;
-    for (int pass = 0; pass < max_passes; ++pass) {
-        r = qp_posteriors(d_seqs, d_offsets, k, d_pairs, P, &prm, d_workspace, workspace_bytes, out, cuda_stream);
-        launches += g_launches;
-        done = pass + 1;
-        if (r != QP_ERR_NNZ_CAPACITY || pass + 1 == max_passes) break;
-        int64_t required = 0;   // the failed pass left the entry count it needs in pair_nnz_base[P]
-        if (cudaMemcpyAsync(&required, out->pair_nnz_base + P, sizeof required, cudaMemcpyDeviceToHost,
-                            (cudaStream_t)cuda_stream) != cudaSuccess ||
-            cudaStreamSynchronize((cudaStream_t)cuda_stream) != cudaSuccess) {
-            r = QP_ERR_CUDA;
-            break;
+    // pass 1: the stage at the requested threshold, with every kept value counted into threshold bins on the way
+    g_want_hist = true;
+    g_tau_hist_valid = false;
+    int r = qp_posteriors(d_seqs, d_offsets, k, d_pairs, P, &prm, d_workspace, workspace_bytes, out, st);
+    g_want_hist = false;
+    int launches = g_launches, done = 1;
+    if ((r == QP_OK || r == QP_ERR_NNZ_CAPACITY) && P > 0) {
+        Ctx* cx = ctx_get();
+        const Layout L = make_layout(P, out->nnz_capacity, out->dense_P != nullptr, total_max_slots(cx ? cx->sms : kSmAssumed));
+        if (cudaMemcpyAsync(g_tau_hist, (char*)d_workspace + L.tau_hist, sizeof g_tau_hist, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess)
+            return QP_ERR_CUDA;
+        g_tau0 = (float)prm.threshold;
+        g_tau_hist_valid = true;
+    }
+    if (r == QP_ERR_NNZ_CAPACITY && max_passes >= 2 && g_tau_hist_valid) {
+        // the smallest bin edge whose tail of the histogram fits the capacity: exact, the second pass recomputes the
+        // very same values
+        int32_t bits0;
+        memcpy(&bits0, &g_tau0, 4);
+        unsigned long long tail = 0;
+        int b = kTauBins;              // first bin NOT taken when walking down from the top
+        while (b > 0 && tail + g_tau_hist[b - 1] <= (unsigned long long)out->nnz_capacity) tail += g_tau_hist[--b];
+        if (b < kTauBins && b > 0) {   // b == 0 cannot happen (the whole histogram did not fit); b == kTauBins: nothing fits
+            const int32_t bits = bits0 + (b << kTauShift);
+            float tb;
+            memcpy(&tb, &bits, 4);
+            prm.threshold = (double)tb;
+            r = qp_posteriors(d_seqs, d_offsets, k, d_pairs, P, &prm, d_workspace, workspace_bytes, out, st);
+            launches += g_launches;
+            done = 2;
         }
-        const double ratio = (double)required / (double)std::max<int64_t>(out->nnz_capacity, 1);
-        prm.threshold = std::min(1.0, prm.threshold * std::max(1.25, std::pow(ratio, 1.5)));
     }
     g_launches = launches;
     if (tau_used) *tau_used = prm.threshold;
     if (passes) *passes = done;
     return r;
+}
+
+extern "C" int qp_last_tau_curve(double* tau, int64_t* count, int max_bins) {
+    if (!g_tau_hist_valid || !tau || !count || max_bins < 1) return QP_ERR_INVALID_ARG;
+    int32_t bits0;
+    memcpy(&bits0, &g_tau0, 4);
+    unsigned long long tail = 0;
+    const int nb = max_bins < kTauBins ? max_bins : kTauBins;
+    for (int b = kTauBins - 1; b >= 0; --b) {
+        tail += g_tau_hist[b];
+        if (b < nb) {
+            const int32_t bits = bits0 + (b << kTauShift);
+            float tb;
+            memcpy(&tb, &bits, 4);
+            tau[b] = (double)tb;
+            count[b] = (int64_t)tail;
+        }
+    }
+    return nb;
 }

@@ -201,6 +201,14 @@ template <typename R> struct KArgs {
     float* dense_P;
     const int64_t* dense_off;
     double* logZ;
+    // memory-limited mode (qp_posteriors_budgeted): histogram of the kept posterior values over threshold bins
+    unsigned long long* tau_hist;   // [kTauBins] or nullptr
+    int32_t tau_bits0;              // bit pattern of the threshold as a float: bin = (bits(P) - tau_bits0) >> kTauShift
 };
+
+// threshold bins of the memory-limited mode: 16 per octave above the requested threshold (positive floats order like
+// their bit patterns, so a bin is a range of bit patterns); the last bin is open-ended
+constexpr int kTauBins = 128;
+constexpr int kTauShift = 19;
 
 }  // namespace qp

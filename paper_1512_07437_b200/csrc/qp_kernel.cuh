@@ -16,9 +16,9 @@ template <typename R, int C, int W> struct KernelSmem {
     static constexpr size_t mbars = 256;   // kWarps * kStages mbarriers
     static constexpr size_t rings = (size_t)kWarps * RingBytes<R, C>::v + RingBytes<R, C>::stage;   // + one zeroed stage
     static_assert(kWarps * kStages * 8 <= (int)mbars, "mbarrier area");
-    template <int GP> static constexpr size_t total() {
-        return tab + mbars + rings + (W > 1 ? ((sizeof(CoopShared<R, GP, W>) + 127) & ~(size_t)127) : 0);
-    }
+    static constexpr size_t hist = (size_t)kWarps * kTauBins * 4;   // per-warp threshold histogram (memory-limited mode)
+    template <int GP> static constexpr size_t coop() { return W > 1 ? ((sizeof(CoopShared<R, GP, W>) + 127) & ~(size_t)127) : 0; }
+    template <int GP> static constexpr size_t total() { return tab + mbars + rings + coop<GP>() + hist; }
 };
 
 template <typename R, int GP, int C, int MODE, int W>
@@ -33,6 +33,10 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
     uint64_t* mbars = (uint64_t*)(smem_raw + SM::tab);
     unsigned char* rings = smem_raw + SM::tab + SM::mbars;
     CoopShared<R, GP, W>* cs = (CoopShared<R, GP, W>*)(rings + SM::rings);   // only touched when W > 1
+    constexpr size_t kCoop = W > 1 ? ((sizeof(CoopShared<R, GP, W>) + 127) & ~(size_t)127) : 0;
+    uint32_t* hist_s = (uint32_t*)(rings + SM::rings + kCoop) + (threadIdx.x >> 5) * kTauBins;
+    if (ka.tau_hist != nullptr)
+        for (int q = threadIdx.x & 31; q < kTauBins; q += 32) hist_s[q] = 0u;
     for (int q = threadIdx.x; q < kTabDim * kTabDim; q += blockDim.x) tab[q] = ka.tab[q];
     for (int q = threadIdx.x; q < (int)(SM::rings / 16); q += blockDim.x) ((float4*)rings)[q] = make_float4(0.f, 0.f, 0.f, 0.f);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -78,7 +82,7 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
             cta_sync();
             const int p = cs->next;
             if (p < 0) return;
-            process_pair<R, GP, C, MODE, W>(ka, smem_u32(tab), p, slot, lane, warp, ring, cs);
+            process_pair<R, GP, C, MODE, W>(ka, smem_u32(tab), p, slot, lane, warp, ring, cs, hist_s);
             cta_sync();   // every warp is done with the slot and with CoopShared
         }
     } else {
@@ -99,7 +103,7 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
         int* cursor = &hdr->cls_cursor[cls];
         int idx = unit;   // the first `granted` pairs of the (largest-first) list go to units 0..granted-1; the rest are pulled
         while (idx < count) {
-            process_pair<R, GP, C, MODE, W>(ka, smem_u32(tab), list[idx], slot, lane, warp, ring, cs);
+            process_pair<R, GP, C, MODE, W>(ka, smem_u32(tab), list[idx], slot, lane, warp, ring, cs, hist_s);
             if constexpr (W == 1) {
                 if (lane == 0) idx = atomicAdd(cursor, 1);
                 idx = __shfl_sync(kFull, idx, 0);
@@ -109,6 +113,11 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
                 cta_sync();
                 idx = cs->next;
             }
+        }
+        if (ka.tau_hist != nullptr) {   // memory-limited mode: this warp's histogram joins the call's
+            __syncwarp();
+            for (int q = lane; q < kTauBins; q += 32)
+                if (hist_s[q]) atomicAdd(&ka.tau_hist[q], (unsigned long long)hist_s[q]);
         }
     }
 }

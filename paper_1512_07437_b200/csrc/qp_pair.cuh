@@ -271,7 +271,8 @@ __device__ __forceinline__ int32_t ld_acquire_gpu(const int32_t* p) {
 // ---------------------------------------------------------------------------------------------------------
 template <typename R, int GP, int C, int MODE, int W>
 __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared address of the emission table*/, int p,
-                             char* slot, int lane, int warp, FRing& ring, CoopShared<R, GP, W>* cs) {
+                             char* slot, int lane, int warp, FRing& ring, CoopShared<R, GP, W>* cs,
+                             uint32_t* hist_s /*this warp's threshold histogram in shared memory*/) {
     using V2 = typename Traits<R>::vec2;
     using Acc = typename Traits<R>::acc_t;
     using SL = Slot<R>;
@@ -891,6 +892,23 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             rp[n] = running;
             ka.nnz[p] = nnz;
             ka.pool_off[p] = (int64_t)poff;
+        }
+    }
+
+    // ---- memory-limited mode only: histogram of the kept values over the threshold bins -------------
+    // A second walk over the entry buffers, so that the emission above stays as it is for every other call.
+    if constexpr (kCsr) {
+        if (ka.tau_hist != nullptr) {   // warp-uniform
+            const int32_t* rowcnt = (const int32_t*)(slot + rowcnt_offset(n, C, nb, RB));
+            for (int i = 1 + 32 * warp + lane; i <= n; i += 32 * W)
+                for (int b = 0; b < nb; ++b) {
+                    const int cb = __ldcg(rowcnt + (int64_t)b * (n + 1) + i);
+                    const float2* buf = (const float2*)(slot + (int64_t)b * blk_bytes + (int64_t)(i + 32) * stride);
+                    for (int e = 0; e < cb; ++e) {
+                        const int bin = (__float_as_int(__ldcg(&buf[e].x)) - ka.tau_bits0) >> kTauShift;
+                        atomicAdd(&hist_s[min(max(bin, 0), kTauBins - 1)], 1u);
+                    }
+                }
         }
     }
 }

@@ -34,3 +34,24 @@ def exchange_distances(dist, group=None):
     if td.is_available() and td.is_initialized() and td.get_world_size(group) > 1:
         td.all_reduce(dist, op=td.ReduceOp.SUM, group=group)
     return dist
+
+
+class ShardedFamily:
+    """One family over `world` ranks: this rank's slice of the pair list, and one step of the path =
+    run the posterior stage on the slice (a callback: qp_posteriors on a GPU, anything that fills this rank's entries
+    of the k x k matrix elsewhere) followed by the one exchange. bench.py and tests/test_multi_gloo.py both go
+    through this class."""
+
+    def __init__(self, lengths, all_pairs, world, rank):
+        self.world, self.rank = int(world), int(rank)
+        self.all_pairs = np.ascontiguousarray(all_pairs, dtype=np.int32).reshape(-1, 2)
+        self.mine = shard_pairs(self.all_pairs, np.asarray(lengths), self.world, self.rank)
+        self.pairs = np.ascontiguousarray(self.all_pairs[self.mine])
+
+    def step(self, run_shard, exchange_buffer=None, group=None):
+        """run_shard(pairs) -> k x k torch tensor holding this rank's distances (zeros elsewhere). Returns the full
+        matrix (summed over ranks). `exchange_buffer`: optional tensor of the same shape to reduce in (the result of
+        run_shard is left untouched, e.g. because the next step rewrites it in place)."""
+        d = run_shard(self.pairs)
+        buf = d.clone() if exchange_buffer is None else exchange_buffer.copy_(d)
+        return exchange_distances(buf, group)

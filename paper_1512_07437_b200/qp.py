@@ -24,7 +24,7 @@ NUM_CLASSES = 18
 
 EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_posteriors_budgeted", "qp_guide_tree", "qp_guide_tree_workspace_bytes", "qp_last_launch_count", "qp_status_string", "qp_version",
            "qp_set_profile", "qp_get_profile", "qp_get_profile_classes", "qp_shutdown",
-           "qp_consistency", "qp_consistency_workspace_bytes", "qp_consistency_passes"]
+           "qp_consistency", "qp_consistency_workspace_bytes", "qp_consistency_passes", "qp_last_tau_curve"]
 
 
 class QpError(RuntimeError):
@@ -103,6 +103,8 @@ def _load():
     L.qp_consistency.restype = C.c_int
     L.qp_consistency.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.POINTER(_Csr), C.c_int64, C.c_void_p,
                                  C.POINTER(_ConsParams), C.c_void_p, C.c_size_t, C.POINTER(_CsrOut), C.c_void_p]
+    L.qp_last_tau_curve.restype = C.c_int
+    L.qp_last_tau_curve.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), C.c_int]
     L.qp_consistency_passes.restype = C.c_int
     L.qp_consistency_passes.argtypes = [C.c_int32]
     return L
@@ -349,6 +351,15 @@ def guide_tree(dist, want_treedist=True, stream=None, workspace=None) -> GuideTr
         raise QpError(code)
     t._ws = ws   # keep the workspace alive until the stream has run
     return t
+
+
+def last_tau_curve(max_bins: int = 128):
+    """qp_last_tau_curve: (tau[b], count of kept values >= tau[b]) of the last memory-limited call, numpy arrays."""
+    tau, cnt = (C.c_double * max_bins)(), (C.c_int64 * max_bins)()
+    n = _lib.qp_last_tau_curve(tau, cnt, int(max_bins))
+    if n < 0:
+        raise QpError(n)
+    return np.array(tau[:n]), np.array(cnt[:n], dtype=np.int64)
 
 
 def consistency_passes(k: int) -> int:

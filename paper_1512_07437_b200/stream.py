@@ -70,24 +70,38 @@ class HostStreamer:
         self.h_pairs = torch.from_numpy(self.pairs).pin_memory()
         self.dist = torch.empty((family.k, family.k), dtype=f32).pin_memory()
         self.d_dist = torch.zeros((family.k, family.k), dtype=f32, device=self.dev)
-        wsb = max((qp.workspace_bytes(family.offsets, family.k, self.pairs[bounds[b]:bounds[b + 1]], self.cp, self.cap)
-                   for b in range(nb)), default=256)
+        self.max_pairs, self.max_rows = max_pairs, max_rows
         self.slots = []
         for _ in range(2):   # two batches in flight
-            self.slots.append(dict(
+            sl = dict(
                 stream=torch.cuda.Stream(self.dev),
-                ws=torch.empty(wsb, dtype=torch.uint8, device=self.dev),
                 d_pairs=torch.empty((max_pairs, 2), dtype=i32, device=self.dev),
-                res=qp.alloc_outputs(self.dev, max_pairs, max_rows, self.cap, family.k, dist=self.d_dist),
-                h_col=torch.empty(self.cap, dtype=i32).pin_memory(), h_val=torch.empty(self.cap, dtype=f32).pin_memory(),
                 h_rp=torch.empty(max_rows, dtype=i32).pin_memory(),
                 h_rb=torch.empty(max_pairs + 1, dtype=i64).pin_memory(),
                 h_nb=torch.empty(max_pairs + 1, dtype=i64).pin_memory(),
                 h_status=torch.empty(4, dtype=i32).pin_memory(),
                 sized=torch.cuda.Event(), done=torch.cuda.Event(),
-            ))
+            )
+            self._size_slot(sl, self.cap)
+            self.slots.append(sl)
         self.h2d_bytes = self.d2h_bytes = 0
         self.launches = 0
+        self.retries = 0
+
+    def _size_slot(self, sl, cap):
+        """(Re)allocate what depends on the CSR capacity of a slot: workspace (it holds the staging pool), device CSR,
+        pinned CSR."""
+        torch = self.torch
+        nb = len(self.bounds) - 1
+        wsb = max((qp.workspace_bytes(self.fam.offsets, self.fam.k, self.pairs[self.bounds[b]:self.bounds[b + 1]], self.cp, cap)
+                   for b in range(nb)), default=256)
+        for key in ("ws", "res", "h_col", "h_val"):
+            sl.pop(key, None)
+        sl["cap"] = int(cap)
+        sl["ws"] = torch.empty(wsb, dtype=torch.uint8, device=self.dev)
+        sl["res"] = qp.alloc_outputs(self.dev, self.max_pairs, self.max_rows, cap, self.fam.k, dist=self.d_dist)
+        sl["h_col"] = torch.empty(cap, dtype=torch.int32).pin_memory()
+        sl["h_val"] = torch.empty(cap, dtype=torch.float32).pin_memory()
 
     def _enqueue(self, b, d_seqs, d_offs):
         """H2D of the batch's pairs, the call, D2H of the small arrays (sizes, status); all on the slot's stream."""
@@ -96,7 +110,7 @@ class HostStreamer:
         lo, hi = self.bounds[b], self.bounds[b + 1]
         with torch.cuda.stream(s["stream"]):
             s["d_pairs"][: hi - lo].copy_(self.h_pairs[lo:hi], non_blocking=True)
-            r = qp.posteriors(d_seqs, d_offs, self.fam.k, s["d_pairs"][: hi - lo], self.cp, s["ws"], nnz_capacity=self.cap,
+            r = qp.posteriors(d_seqs, d_offs, self.fam.k, s["d_pairs"][: hi - lo], self.cp, s["ws"], nnz_capacity=s["cap"],
                               h_rows_total=self.rows[b], stream=s["stream"], check=True, reuse=s["res"])
             res = s["res"]
             s["h_nb"][: hi - lo + 1].copy_(res.pair_nnz_base[: hi - lo + 1], non_blocking=True)
@@ -107,13 +121,22 @@ class HostStreamer:
         self.launches += r.launches
         self.h2d_bytes += 8 * (hi - lo)
 
-    def _collect(self, b):
-        """Wait for the batch's sizes, then D2H of exactly nnz entries of col/val on the slot's stream."""
+    def _collect(self, b, d_seqs, d_offs):
+        """Wait for the batch's sizes, then D2H of exactly nnz entries of col/val on the slot's stream. A batch whose
+        CSR did not fit the slot's capacity (denser than beta_guess) is run again, once, in a slot grown to the entry
+        count the failed call reported; the batches already handed out are not affected."""
         torch = self.torch
         s = self.slots[b % 2]
         lo, hi = self.bounds[b], self.bounds[b + 1]
         s["sized"].synchronize()
         code = int(s["h_status"][0].item())
+        if code == qp.ERR["NNZ_CAPACITY"]:
+            need = int(s["h_nb"][hi - lo].item())          # pair_nnz_base[P] = entries required
+            self._size_slot(s, need + need // 16 + 4096)
+            self.retries += 1
+            self._enqueue(b, d_seqs, d_offs)
+            s["sized"].synchronize()
+            code = int(s["h_status"][0].item())
         if code != qp.QP_OK:
             raise qp.QpError(code, f"(batch {b}, pairs {lo}..{hi})")
         nz = int(s["h_nb"][hi - lo].item())
@@ -143,7 +166,7 @@ class HostStreamer:
             # has come back for more, so that slot is free: start batch b+1 in it before waiting for batch b.
             if b + 1 < nb:
                 self._enqueue(b + 1, d_seqs, d_offs)
-            nz = self._collect(b)          # D2H of batch b's CSR overlaps batch b+1's kernels
+            nz = self._collect(b, d_seqs, d_offs)   # D2H of batch b's CSR overlaps batch b+1's kernels
             s = self.slots[b % 2]
             lo, hi = self.bounds[b], self.bounds[b + 1]
             s["done"].synchronize()

@@ -311,6 +311,13 @@ def test_host_streamer_matches_single_call(default_params):
             assert np.array_equal(b.col.numpy(), col[n0:n1]) and np.array_equal(b.val.numpy(), val[n0:n1])
         assert seen == len(pairs)
         assert torch.equal(hs.dist, ref.dist.cpu())
+    # a capacity guess that is far too small: the overflowing batches are re-run in a grown slot, same result
+    hs = stream.HostStreamer(fam, pairs, default_params, batch_cells=2.0e7, beta_guess=0.004)
+    got = [(b.lo, b.hi, b.col.numpy().copy(), b.val.numpy().copy()) for b in hs.run()]
+    assert hs.retries >= 1
+    for lo, hi, c, v in got:
+        assert np.array_equal(c, col[nb[lo]:nb[hi]]) and np.array_equal(v, val[nb[lo]:nb[hi]])
+    assert torch.equal(hs.dist, ref.dist.cpu())
 
 
 def test_fuzz_random_pairs_models_thresholds():
@@ -370,9 +377,14 @@ def test_memory_limited_mode_raises_threshold(default_params):
     args = (torch.from_numpy(fam.seqs).to(dev), torch.from_numpy(fam.offsets).to(dev), fam.k, torch.from_numpy(pairs).to(dev), cp, ws)
     kw = dict(nnz_capacity=cap, h_rows_total=int((L[pairs[:, 0]] + 1).sum()))
     res = qp.posteriors(*args, budget_passes=8, **kw)
-    assert res.code == 0 and res.passes >= 2 and res.tau_used > default_params.threshold
+    assert res.code == 0 and res.passes == 2 and res.tau_used > default_params.threshold      # never more than two passes
     nnz = int(res.pair_nnz_base[-1].item())
     assert nnz <= cap
+    # the threshold comes off the histogram of the first pass: a bin edge, the smallest one that fits, exactly
+    tau, cnt = qp.last_tau_curve()
+    assert tau[0] == np.float32(default_params.threshold) and cnt[0] == nnz_full and (np.diff(cnt) <= 0).all()
+    b = int(np.nonzero(tau == res.tau_used)[0][0])
+    assert cnt[b] == nnz and cnt[b - 1] > cap
     print(f"budget {cap} entries of {nnz_full}: tau {default_params.threshold} -> {res.tau_used:.4f} in {res.passes} passes, nnz {nnz}")
     prm = inputs.Params(hmm=default_params.hmm, pf=default_params.pf, threshold=res.tau_used)
     run = orc.Run(prm, fam, pairs, keep_dense=True)

@@ -39,15 +39,20 @@ def _worker(rank, world, port, out):
     from oracle import qp_oracle as orc
     prm = inputs.default_params()
     fam = inputs.config_family(0)
-    pairs = inputs.all_pairs(fam.k)
-    mine = multi.shard_pairs(pairs, fam.lengths, world, rank)
-    run = orc.Run(prm, fam, pairs[mine], threads=1)
-    D = torch.zeros((fam.k, fam.k), dtype=torch.float64)
-    D[pairs[mine, 0], pairs[mine, 1]] = torch.from_numpy(run.dist)
-    D[pairs[mine, 1], pairs[mine, 0]] = torch.from_numpy(run.dist)
-    multi.exchange_distances(D)
+    sh = multi.ShardedFamily(fam.lengths, inputs.all_pairs(fam.k), world, rank)   # the class bench.py --gpus N uses
+
+    def run_shard(pairs):     # stands in for qp_posteriors on this rank's GPU
+        run = orc.Run(prm, fam, pairs, threads=1)
+        D = torch.zeros((fam.k, fam.k), dtype=torch.float64)
+        D[pairs[:, 0], pairs[:, 1]] = torch.from_numpy(run.dist)
+        D[pairs[:, 1], pairs[:, 0]] = torch.from_numpy(run.dist)
+        return D
+
+    full = sh.step(run_shard)
+    again = sh.step(run_shard, exchange_buffer=torch.empty_like(full))             # reusable, with a caller's buffer
+    assert torch.equal(full, again)
     if rank == 0:
-        np.save(out, D.numpy())
+        np.save(out, full.numpy())
     td.destroy_process_group()
 
 
