@@ -34,7 +34,7 @@ METRIC = "posterior DP cells/sec (fwd+bwd, both models, combine+sparsify+MEA)"
 UNIT = "cells/s"
 ALGO_BYTES_PER_CELL = 16.0     # fp32 F_M of both models written in forward, read back in backward
 SFU_OPS_PER_CELL = 43.0        # canonical log-space transcendental count (context only)
-SFU_PEAK = 148 * 16 * 1.965e9  # SURVEY.md 8(d) nominal MUFU rate
+SFU_PEAK = 148 * 16 * 1.965e9  # SURVEY.md 8(d) nominal MUFU rate (the measured one is in roofline.alu_peaks_measured)
 
 
 def peaks():
@@ -256,7 +256,18 @@ def measure(cfg, steps, warmup, dev, prm, rank=0, world=1, shard=False, sample_c
                 clocks=clocks, shard=shard)
 
 
-def roofline_of(cfg, m, clocks):
+_ALU = {}
+
+
+def alu_peaks(dev):
+    """Measured FFMA / FFMA2 / MUFU rates of this device (qp_measure_peaks), once per process."""
+    if "v" not in _ALU:
+        from paper_1512_07437_b200 import qp
+        _ALU["v"] = qp.measure_peaks(str(dev))
+    return _ALU["v"]
+
+
+def roofline_of(cfg, m, clocks, dev=None):
     """HBM roofline of the hot path: algorithmic bytes (16 B/cell) over the WHOLE step's device time
     (`frac`) and over the pair kernels alone (`kernel_frac`: fork..join of the class kernels, the dominant kernels),
     with the issue bound of the pair kernels beside it."""
@@ -267,7 +278,9 @@ def roofline_of(cfg, m, clocks):
     achieved = ALGO_BYTES_PER_CELL * cells / step_s / 1e9
     kernel_achieved = ALGO_BYTES_PER_CELL * cells / kern_s / 1e9
     mhz = (clocks or {}).get("sm_mhz") or 1965
-    issue_s = WARP_INSTR_PER_CELL * cells / (N_SMS * 4 * mhz * 1e6)
+    alu = alu_peaks(dev) if dev is not None else None
+    issue_rate = alu["warp_instr_per_s"] if alu else N_SMS * 4 * mhz * 1e6
+    issue_s = WARP_INSTR_PER_CELL * cells / issue_rate
     return {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
             "traffic": ncu_traffic(cfg), "peak_source": peak_src,
             "frac_note": "whole step (schedule + pair kernels + fp64 distance queues + CSR placement) over the HBM peak",
@@ -277,10 +290,11 @@ def roofline_of(cfg, m, clocks):
             "traffic_note": "dram read+write bytes of those launches from ncu (profiles/traffic.csv), per step",
             "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
             "phases_ms": {k: round(v, 3) for k, v in prof.items()},
-            "issue": {"warp_instr_per_cell": WARP_INSTR_PER_CELL, "sm_mhz": mhz, "bound_ms": 1e3 * issue_s,
-                      "frac": issue_s / kern_s,
-                      "note": "warp instructions per cell (ncu census, profiles/) x cells / (148 SMs x 4 schedulers x "
-                              "sampled SM clock) over the pair-kernel time"},
+            "issue": {"warp_instr_per_cell": WARP_INSTR_PER_CELL, "sm_mhz": mhz, "warp_instr_per_s": issue_rate,
+                      "bound_ms": 1e3 * issue_s, "frac": issue_s / kern_s,
+                      "note": "warp instructions per cell (ncu census, profiles/) x cells / the MEASURED issue rate "
+                              "(qp_measure_peaks: scalar FFMA lane-ops per second / 32) over the pair-kernel time"},
+            "alu_peaks_measured": alu,
             "canonical_sfu_roofline": {"ops_per_cell": SFU_OPS_PER_CELL, "peak_ops_s": SFU_PEAK,
                                        "frac": SFU_OPS_PER_CELL * cells / kern_s / SFU_PEAK,
                                        "note": "north_star's log-space transcendental bound; this path is "
@@ -390,7 +404,7 @@ def run_ours(args):
                                            f"all-reduce of the {fam.k} x {fam.k} distance matrix per step"
                                            if shard else f"{world} independent famil{'y' if world == 1 else 'ies'} (bulk mode), "
                                            "one per GPU, no collective")},
-                "roofline": roofline_of(args.config, m, clocks), "clocks": clocks,
+                "roofline": roofline_of(args.config, m, clocks, dev), "clocks": clocks,
                 "gpu_launches": m["launches_per_step"] * args.steps,
                 "class_timeline_ms": m["classes"]}
 
@@ -400,7 +414,7 @@ def run_ours(args):
         for cfg in (2, 4):
             torch.cuda.empty_cache()
             mc = measure(cfg, max(args.steps, 5), 3, dev, prm, sample_clocks=False)
-            rc = roofline_of(cfg, mc, clocks)
+            rc = roofline_of(cfg, mc, clocks, dev)
             line["configs"][str(cfg)] = {
                 "workload": workload_name(cfg, mc["fam"], mc["all_pairs"]), "cells": mc["total_cells"],
                 "value": mc["total_cells"] / (mc["ms_step"] * 1e-3), "unit": UNIT, "ms_per_step": mc["ms_step"],
@@ -437,34 +451,26 @@ def run_ours(args):
 
 
 def run_e2e(args, fam, pairs, prm, qp, dev, my_cells):
-    """Same metric through the package's host-buffer front end (paper_1512_07437_b200.stream.HostStreamer over
-    qp_posteriors): every step copies sequences/offsets/pairs from pinned host memory, runs the call batch by batch
-    (BASELINE.json configs[3]: "memory-budgeted by streaming pair batches"), and copies the distance matrix and the
-    WHOLE CSR back to pinned host memory; batch b's copies overlap batch b+1's kernels."""
+    """Same metric end to end through ONE C-ABI call with HOST buffers, qp_posteriors_host: every step copies
+    sequences / offsets / pairs from pinned host memory, runs the stage batch by batch (BASELINE.json configs[3]:
+    "memory-budgeted by streaming pair batches") and copies the distance matrix and the WHOLE CSR back to pinned host
+    memory; batch b's copies overlap batch b+1's kernels (csrc/qp_host.cu)."""
     import torch
-    from paper_1512_07437_b200 import stream
-    hs = stream.HostStreamer(fam, pairs, prm, device=str(dev))
-
-    def one_step():
-        nnz = 0
-        for batch in hs.run():          # a consumer would read batch.col / batch.val here
-            nnz += int(batch.col.numel())
-        return nnz
-
-    one_step()   # warm-up
+    hc = qp.HostCall(fam, pairs, prm, device=str(dev))
+    hc.run()   # warm-up
     torch.cuda.synchronize()
-    hs.h2d_bytes = hs.d2h_bytes = 0
     steps = max(1, min(args.steps, 3))
     t0 = time.perf_counter()
     for _ in range(steps):
-        nnz = one_step()
+        hc.run()
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
-    return {"value": my_cells * steps / wall, "unit": UNIT, "h2d_bytes_per_step": hs.h2d_bytes // steps,
-            "d2h_bytes_per_step": hs.d2h_bytes // steps, "ms_per_step": 1e3 * wall / steps, "steps": steps,
-            "batches": len(hs.bounds) - 1, "nnz": nnz,
-            "note": "host wall clock around stream.HostStreamer.run(): H2D of the inputs, qp_posteriors per pair batch, "
-                    "D2H of distances and the full CSR (two batches in flight: copies overlap the next batch's kernels)"}
+    return {"value": my_cells * steps / wall, "unit": UNIT, "h2d_bytes_per_step": hc.h2d_bytes,
+            "d2h_bytes_per_step": hc.d2h_bytes, "ms_per_step": 1e3 * wall / steps, "steps": steps,
+            "batches": hc.batches, "nnz": hc.nnz,
+            "note": "host wall clock around qp_posteriors_host (one C-ABI call per step, pinned host buffers): H2D of the "
+                    "inputs, qp_posteriors per pair batch, D2H of distances and the full CSR (two batches in flight: "
+                    "copies overlap the next batch's kernels)"}
 
 
 def main():

@@ -48,7 +48,11 @@ enum { QP_FP32 = 0, QP_FP64 = 1 };
 
 enum {
     QP_FLAG_SYNC_STATUS = 1,        /* synchronise the stream at the end and return the device status          */
-    QP_FLAG_NO_REFINE = 2           /* QP_FP32 only: skip the fp64 re-evaluation of near-identical pairs        */
+    QP_FLAG_NO_REFINE = 2,          /* QP_FP32 only: skip the fp64 re-evaluation of near-identical pairs        */
+    QP_FLAG_NO_POLLERS = 4          /* QP_FP32 only: do not start the fp64 re-evaluation beside the fp32 kernels, only
+                                       after them. For callers that keep several calls in flight on different streams
+                                       (qp_posteriors_host): the waiting kernels of one call would sit in front of the
+                                       next call's kernels in the hardware queues they share                      */
 };
 
 /*
@@ -118,6 +122,44 @@ int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int32_t* h_pai
 int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, const int32_t* d_pairs, int64_t P,
                   const qp_params* params, void* d_workspace, size_t workspace_bytes, const qp_output* out,
                   void* cuda_stream);
+
+/*
+ * The posterior stage on HOST buffers (BASELINE.json configs[3]: "memory-budgeted by streaming pair batches"): inputs
+ * and outputs live in host memory (pin them -- cudaHostAlloc / cudaHostRegister -- or the copies will not overlap
+ * anything). The pair list is cut into batches of about a quarter of the family (4e8 .. 6e9 cells), shrunk until two
+ * batches fit d_workspace; every batch goes through qp_posteriors; two batches are in flight, so that the CSR of one
+ * travels back over PCIe while the kernels of the next run. A batch that turns out denser than beta_guess is split in
+ * two and run again. The call returns when every output is in host memory (it synchronises).
+ *   h_seqs / h_offsets / h_pairs   as d_seqs / d_offsets / d_pairs of qp_posteriors, in host memory
+ *   d_workspace                    DEVICE memory, 256-byte aligned, caller-owned; holds the device copies of the inputs,
+ *                                  the k x k distance matrix, and per batch in flight the outputs and the workspace of
+ *                                  qp_posteriors. qp_posteriors_host_workspace_bytes gives the size at which no batch has
+ *                                  to be shrunk; less works down to one pair per batch
+ *   out                            host arrays laid out like qp_output -- pair order, global prefixes; beta_guess: expected
+ *                                  nnz / cells (<= 0: 0.05) sizes the per-batch device CSR; the call fills status,
+ *                                  h2d_bytes / d2h_bytes (bytes it copied) and batches
+ * Returns QP_OK or an error of qp_posteriors; QP_ERR_NNZ_CAPACITY if out->nnz_capacity is too small (pair_nnz_base[P] =
+ * entries required). params->flags: QP_FLAG_NO_REFINE is honoured, the others are set by the call.
+ */
+typedef struct {
+    int64_t* pair_row_base;  /* [P+1] */
+    int64_t* pair_nnz_base;  /* [P+1] */
+    int32_t* row_ptr;        /* [sum(n_p+1)] */
+    int32_t* col_idx;        /* [nnz_capacity] */
+    float* val;              /* [nnz_capacity] */
+    int64_t nnz_capacity;
+    float* dist;             /* [k*k] */
+    double beta_guess;       /* in */
+    int32_t status[4];       /* out: {code, pair index or -1, detail, pairs re-evaluated in fp64} */
+    int32_t batches;         /* out */
+    int32_t reserved;
+    int64_t h2d_bytes, d2h_bytes;   /* out */
+} qp_host_output;
+int qp_posteriors_host_workspace_bytes(const int64_t* h_offsets, int32_t k, const int32_t* h_pairs, int64_t P,
+                                       const qp_params* params, double beta_guess, size_t* out_bytes);
+int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offsets, int32_t k, const int32_t* h_pairs, int64_t P,
+                       const qp_params* params, void* d_workspace, size_t workspace_bytes, qp_host_output* out,
+                       void* cuda_stream);
 
 /*
  * Memory-limited mode ("fit analysis in user-specified amount of RAM by decreasing sparsity coefficient in
@@ -250,6 +292,25 @@ int qp_get_profile_classes(float start_ms[QP_NUM_CLASSES], float stop_ms[QP_NUM_
  * from the thread that made the calls, after its streams have been synchronised. Later calls re-create them.
  */
 void qp_shutdown(void);
+
+/*
+ * Measured arithmetic peaks of the current device, for the roofline lines of bench.py ("measure it
+ * with a ... micro-benchmark at the sustained clock"; "report the FP32-pipe bound beside it"). Three micro-kernels of
+ * independent dependency chains, 32 warps per SM, a few ms each, best of two timed repetitions:
+ *   ffma_per_s        scalar fp32 FMA lane-operations per second (FFMA);  / 32 = warp instructions per second when
+ *                     nothing but the issue slots limits a kernel (warp_instr_per_s)
+ *   ffma2_fma_per_s   scalar-equivalent FMAs per second through the packed instruction (fma.rn.f32x2 -> FFMA2), the
+ *                     one the pair kernels use for the two automata side by side
+ *   mufu_per_s        sqrt.approx per second (MUFU pipe; the pair kernels issue one per cell)
+ * d_scratch: at least sms * 4096 bytes of device memory (caller-owned). Synchronises the stream. Errors:
+ * QP_ERR_INVALID_ARG, QP_ERR_WORKSPACE_TOO_SMALL, QP_ERR_CUDA.
+ */
+typedef struct {
+    int32_t sms;
+    int32_t reserved;
+    double ffma_per_s, ffma2_fma_per_s, mufu_per_s, warp_instr_per_s;
+} qp_peaks;
+int qp_measure_peaks(qp_peaks* out, void* d_scratch, size_t scratch_bytes, void* cuda_stream);
 
 const char* qp_status_string(int status);
 const char* qp_version(void);

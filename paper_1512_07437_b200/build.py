@@ -19,7 +19,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libqp.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-I" + INC, "-I" + CSRC]
+              "-Xcompiler", "-fPIC", "-I" + INC, "-I" + CSRC] + os.environ.get("QP_EXTRA_NVCC_FLAGS", "").split()
 
 
 def _newer(target, deps):

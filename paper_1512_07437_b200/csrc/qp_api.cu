@@ -673,6 +673,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     const bool dense = out->dense_P != nullptr;
     const int sms = cx->sms;
     const bool refine = !fp64 && !(params->flags & QP_FLAG_NO_REFINE);
+    const bool pollers = refine && !(params->flags & QP_FLAG_NO_POLLERS);
     const bool full_outputs = out->dense_P != nullptr || out->logZ != nullptr;   // test outputs: separate kernel instances
     const Layout L = make_layout(P, out->nnz_capacity, dense, total_max_slots(sms));
     if ((int64_t)workspace_bytes < L.fixed + 256) return QP_ERR_WORKSPACE_TOO_SMALL;
@@ -736,7 +737,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     g_launches += 4;
     MaxW64 mw64;
     for (int c = 0; c < kNumClasses; ++c) mw64.w[c] = ((kMaskRefine >> c) & 1) ? max_units(c, true, sms) : 0;
-    if (refine) {   // the pollers' slots come off the head of the slot region
+    if (pollers) {   // the pollers' slots come off the head of the slot region
         k_refine_plan<<<1, 32, 0, st>>>(0, mw64, avail, hdr);
         ++g_launches;
     }
@@ -753,7 +754,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     QP_TRY(cudaGetLastError());
 
     // ---- a1..a7: one persistent kernel per class, forked onto side streams ----------------------------------
-    if (refine) {   // pollers leave when this many fp32 class warps have exited
+    if (pollers) {   // pollers leave when this many fp32 class warps have exited
         int total = 0;
         for (int c = 0; c < kNumClasses; ++c)
             if ((cmask >> c) & 1) total += class_grid(c, false, sms) * (class_W(c, false) == 1 ? kWarpsPerCta : class_W(c, false));
@@ -774,7 +775,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
         QP_TRY(cudaEventRecord(cx->join[c], cx->st[c]));
         QP_TRY(cudaStreamWaitEvent(st, cx->join[c], 0));
     }
-    if (refine) {   // pollers of the fp64 re-evaluation queue, behind the fp32 classes: they fill the room those leave
+    if (pollers) {   // pollers of the fp64 re-evaluation queue, behind the fp32 classes: they fill the room those leave
         ka64->refine_pass = 1;
         for (int c = kNumClasses - 1; c >= kNumPacked; --c) {
             cudaStream_t es = cx->st[kNumClasses + (c - kNumPacked)];
@@ -812,8 +813,8 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
         QP_TRY(cudaEventRecord(cx->join[kNumStreams - 1], ps));
         QP_TRY(cudaStreamWaitEvent(st, cx->join[kNumStreams - 1], 0));
         for (int c = kNumPacked; c < kNumClasses; ++c) {
-            QP_TRY(cudaStreamWaitEvent(st, cx->join[c], 0));                                  // drainers
-            QP_TRY(cudaStreamWaitEvent(st, cx->join[kNumClasses + (c - kNumPacked)], 0));     // pollers
+            QP_TRY(cudaStreamWaitEvent(st, cx->join[c], 0));                                               // drainers
+            if (pollers) QP_TRY(cudaStreamWaitEvent(st, cx->join[kNumClasses + (c - kNumPacked)], 0));     // pollers
         }
     }
     prof_mark(cx, 3, st);

@@ -1,0 +1,386 @@
+// qp_host.cu -- qp_posteriors_host: the posterior stage on HOST buffers (include/qp.h).
+//
+// BASELINE.json configs[3]: "memory-budgeted by streaming pair batches". The caller's data lives in host memory;
+// the pair list is cut into batches that fit the device workspace twice, and two batches are in flight: while batch
+// b's CSR travels back over PCIe on one stream, batch b+1's kernels run on the other, so the wall time of a family
+// is max(compute, copy) instead of their sum. Every step of the computation runs inside qp_posteriors (this file
+// only plans batches, moves buffers and orders streams; it is written against the public C ABI).
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+#include "qp.h"
+
+namespace {
+
+inline int64_t al256(int64_t v) { return (v + 255) & ~(int64_t)255; }
+
+struct Batch {
+    int64_t lo, hi;        // pairs [lo, hi)
+    int64_t cells, rows;   // sum n*m, sum (n+1)
+};
+
+struct Slot {              // device buffers of one batch in flight + its stream
+    cudaStream_t st = nullptr;
+    cudaEvent_t sized = nullptr, done = nullptr;
+    char* base = nullptr;
+    int32_t* pairs = nullptr;
+    int64_t *row_base = nullptr, *nnz_base = nullptr;
+    int32_t *row_ptr = nullptr, *col = nullptr, *status = nullptr;
+    float* val = nullptr;
+    char* ws = nullptr;
+    int64_t ws_bytes = 0, cap = 0;
+    // pinned staging of the small per-batch results (sizes and status), owned by the call
+    int64_t* h_last = nullptr;   // [1] nnz of the batch
+    int32_t* h_status = nullptr; // [4]
+    Batch cur{0, 0, 0, 0};
+    int64_t out_nnz0 = 0;        // where the batch's entries go in the caller's col_idx / val
+};
+
+struct SlotPlan {
+    int64_t max_pairs, max_rows, cap, ws_bytes, total;
+};
+
+// bytes of one slot for batches of at most these sizes
+SlotPlan plan_slot(int64_t max_pairs, int64_t max_rows, int64_t cap, int64_t ws_bytes) {
+    SlotPlan p{max_pairs, max_rows, cap, ws_bytes, 0};
+    p.total = al256(max_pairs * 8) + 2 * al256((max_pairs + 1) * 8) + al256(max_rows * 4) + 2 * al256(cap * 4) + 256 +
+              al256(ws_bytes);
+    return p;
+}
+
+}  // namespace
+
+extern "C" int qp_posteriors_host_workspace_bytes(const int64_t* h_offsets, int32_t k, const int32_t* h_pairs, int64_t P,
+                                                  const qp_params* params, double beta_guess, size_t* out_bytes) {
+    if (!h_offsets || (!h_pairs && P > 0) || !params || !out_bytes || k < 0 || P < 0) return QP_ERR_INVALID_ARG;
+    const double beta = beta_guess > 0.0 ? beta_guess : 0.05;
+    int64_t total_cells = 0;
+    std::vector<int64_t> cells(P), rows(P);
+    for (int64_t p = 0; p < P; ++p) {
+        const int x = h_pairs[2 * p], y = h_pairs[2 * p + 1];
+        if (x < 0 || y < 0 || x >= k || y >= k || x == y) return QP_ERR_BAD_PAIR;
+        const int64_t n = h_offsets[x + 1] - h_offsets[x], m = h_offsets[y + 1] - h_offsets[y];
+        if (n < 1 || m < 1 || n > QP_MAX_LEN || m > QP_MAX_LEN) return QP_ERR_EMPTY_SEQUENCE;
+        cells[p] = n * m;
+        rows[p] = n + 1;
+        total_cells += cells[p];
+    }
+    // the batch size qp_posteriors_host aims at first: a quarter of the family, between 4e8 and 6e9 cells
+    const double target = std::min(6.0e9, std::max(4.0e8, (double)total_cells / 4.0));
+    int64_t max_pairs = 0, max_rows = 0, max_cells = 0, lo = 0, c = 0, r = 0;
+    size_t worst = 0;
+    qp_params prm = *params;
+    std::vector<std::pair<int64_t, int64_t>> bounds;
+    for (int64_t p = 0; p < P; ++p) {
+        c += cells[p];
+        r += rows[p];
+        if ((double)c >= target || p + 1 == P) {
+            bounds.push_back({lo, p + 1});
+            max_pairs = std::max(max_pairs, p + 1 - lo);
+            max_rows = std::max(max_rows, r);
+            max_cells = std::max(max_cells, c);
+            lo = p + 1;
+            c = r = 0;
+        }
+    }
+    const int64_t cap = (int64_t)(beta * (double)max_cells) + 4096;
+    for (auto& b : bounds) {
+        size_t wsb = 0;
+        const int rr = qp_workspace_bytes(h_offsets, k, h_pairs + 2 * b.first, b.second - b.first, &prm, cap, 0, 0, &wsb);
+        if (rr != QP_OK) return rr;
+        worst = std::max(worst, wsb);
+    }
+    const int64_t seq_bytes = h_offsets[k] - h_offsets[0];
+    const int64_t common = al256(seq_bytes) + al256((int64_t)(k + 1) * 8) + al256((int64_t)k * k * 4);
+    *out_bytes = (size_t)(common + 2 * plan_slot(max_pairs, max_rows, cap, (int64_t)worst).total);
+    return QP_OK;
+}
+
+extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offsets, int32_t k, const int32_t* h_pairs,
+                                  int64_t P, const qp_params* params, void* d_workspace, size_t workspace_bytes,
+                                  qp_host_output* out, void* cuda_stream) {
+    if (!out || !params || !h_offsets || k < 0 || P < 0 || (P > 0 && (!h_seqs || !h_pairs || !d_workspace))) return QP_ERR_INVALID_ARG;
+    if (!out->pair_row_base || !out->pair_nnz_base || (P > 0 && (!out->row_ptr || !out->dist))) return QP_ERR_INVALID_ARG;
+    if (out->nnz_capacity < 0 || (out->nnz_capacity > 0 && (!out->col_idx || !out->val))) return QP_ERR_INVALID_ARG;
+    if (((uintptr_t)d_workspace & 255) != 0) return QP_ERR_INVALID_ARG;
+    out->h2d_bytes = out->d2h_bytes = 0;
+    out->batches = 0;
+    out->status[0] = out->status[1] = out->status[2] = out->status[3] = 0;
+    out->pair_row_base[0] = out->pair_nnz_base[0] = 0;
+    if (P == 0) return QP_OK;
+    cudaStream_t main = (cudaStream_t)cuda_stream;
+    const double beta = out->beta_guess > 0.0 ? out->beta_guess : 0.05;
+
+    // ---- host-side plan: per-pair sizes, prefix of rows, batches ---------------------------------------------------
+    std::vector<int64_t> cells(P);
+    int64_t total_cells = 0;
+    for (int64_t p = 0; p < P; ++p) {
+        const int x = h_pairs[2 * p], y = h_pairs[2 * p + 1];
+        if (x < 0 || y < 0 || x >= k || y >= k || x == y) {
+            out->status[0] = QP_ERR_BAD_PAIR;
+            out->status[1] = (int32_t)p;
+            return QP_ERR_BAD_PAIR;
+        }
+        const int64_t n = h_offsets[x + 1] - h_offsets[x], m = h_offsets[y + 1] - h_offsets[y];
+        if (n < 1 || m < 1 || n > QP_MAX_LEN || m > QP_MAX_LEN) {
+            out->status[0] = QP_ERR_EMPTY_SEQUENCE;
+            out->status[1] = (int32_t)p;
+            return QP_ERR_EMPTY_SEQUENCE;
+        }
+        cells[p] = n * m;
+        total_cells += cells[p];
+        out->pair_row_base[p + 1] = out->pair_row_base[p] + n + 1;
+    }
+    const int64_t seq_bytes = h_offsets[k] - h_offsets[0];
+    const int64_t common = al256(seq_bytes) + al256((int64_t)(k + 1) * 8) + al256((int64_t)k * k * 4);
+    qp_params prm = *params;
+    prm.flags = (prm.flags & ~QP_FLAG_SYNC_STATUS) | QP_FLAG_NO_POLLERS;   // several calls in flight: see qp.h
+
+    std::vector<Batch> batches;
+    SlotPlan sp{0, 0, 0, 0, 0};
+    // at least four batches when the family is large (so that copies overlap kernels), at most ~6e9 cells each;
+    // shrink until two slots fit the workspace
+    double target = std::min(6.0e9, std::max(4.0e8, (double)total_cells / 4.0));
+    for (int attempt = 0; attempt < 40; ++attempt) {
+        batches.clear();
+        Batch b{0, 0, 0, 0};
+        for (int64_t p = 0; p < P; ++p) {
+            b.cells += cells[p];
+            b.rows += out->pair_row_base[p + 1] - out->pair_row_base[p];
+            b.hi = p + 1;
+            if ((double)b.cells >= target) {
+                batches.push_back(b);
+                b = Batch{p + 1, p + 1, 0, 0};
+            }
+        }
+        if (b.hi > b.lo) batches.push_back(b);
+        int64_t max_pairs = 0, max_rows = 0, max_cells = 0;
+        for (const Batch& q : batches) {
+            max_pairs = std::max(max_pairs, q.hi - q.lo);
+            max_rows = std::max(max_rows, q.rows);
+            max_cells = std::max(max_cells, q.cells);
+        }
+        const int64_t cap = (int64_t)(beta * (double)max_cells) + 4096;
+        size_t wsb = 0, worst = 0;
+        int r = QP_OK;
+        for (const Batch& q : batches) {
+            r = qp_workspace_bytes(h_offsets, k, h_pairs + 2 * q.lo, q.hi - q.lo, &prm, cap, 0, 0, &wsb);
+            if (r != QP_OK) return r;
+            worst = std::max(worst, wsb);
+        }
+        sp = plan_slot(max_pairs, max_rows, cap, (int64_t)worst);
+        if (common + 2 * sp.total <= (int64_t)workspace_bytes) break;
+        if (batches.size() >= (size_t)P) {
+            // one pair per batch and still too large: let qp_posteriors run with fewer scratch slots
+            const int64_t spare = ((int64_t)workspace_bytes - common) / 2 - (sp.total - al256(sp.ws_bytes));
+            size_t minimum = 0;
+            for (const Batch& q : batches) {
+                size_t mb = 0;
+                const int rr = qp_workspace_bytes(h_offsets, k, h_pairs + 2 * q.lo, q.hi - q.lo, &prm, cap, 0, 1, &mb);
+                if (rr != QP_ERR_WORKSPACE_TOO_SMALL && rr != QP_OK) return rr;
+                minimum = std::max(minimum, mb);
+            }
+            if (spare < (int64_t)minimum) return QP_ERR_WORKSPACE_TOO_SMALL;
+            sp = plan_slot(max_pairs, max_rows, cap, spare & ~(int64_t)255);
+            break;
+        }
+        target *= 0.6;
+        sp.total = 0;
+    }
+    if (sp.total == 0 || common + 2 * sp.total > (int64_t)workspace_bytes) return QP_ERR_WORKSPACE_TOO_SMALL;
+
+    // ---- carve the device workspace ------------------------------------------------------------------------------------
+    char* w = (char*)d_workspace;
+    uint8_t* d_seqs = (uint8_t*)w;
+    int64_t* d_offs = (int64_t*)(w + al256(seq_bytes));
+    float* d_dist = (float*)(w + al256(seq_bytes) + al256((int64_t)(k + 1) * 8));
+    Slot sl[2];
+    int rc = QP_OK;
+    int64_t* h_small = nullptr;   // pinned: per slot [1] nnz + [4] status
+    auto cleanup = [&]() {
+        for (Slot& s : sl) {
+            if (s.st) cudaStreamSynchronize(s.st);
+            if (s.sized) cudaEventDestroy(s.sized);
+            if (s.done) cudaEventDestroy(s.done);
+            if (s.st) cudaStreamDestroy(s.st);
+        }
+        if (h_small) cudaFreeHost(h_small);
+        (void)cudaGetLastError();
+    };
+#define QP_H(x)                     \
+    do {                            \
+        if ((x) != cudaSuccess) {   \
+            cleanup();              \
+            return QP_ERR_CUDA;     \
+        }                           \
+    } while (0)
+    QP_H(cudaMallocHost((void**)&h_small, 2 * 64));
+    for (int q = 0; q < 2; ++q) {
+        Slot& s = sl[q];
+        QP_H(cudaStreamCreateWithFlags(&s.st, cudaStreamNonBlocking));
+        QP_H(cudaEventCreateWithFlags(&s.sized, cudaEventDisableTiming));
+        QP_H(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+        char* o = w + common + q * sp.total;
+        s.base = o;
+        s.pairs = (int32_t*)o;
+        o += al256(sp.max_pairs * 8);
+        s.row_base = (int64_t*)o;
+        o += al256((sp.max_pairs + 1) * 8);
+        s.nnz_base = (int64_t*)o;
+        o += al256((sp.max_pairs + 1) * 8);
+        s.row_ptr = (int32_t*)o;
+        o += al256(sp.max_rows * 4);
+        s.col = (int32_t*)o;
+        o += al256(sp.cap * 4);
+        s.val = (float*)o;
+        o += al256(sp.cap * 4);
+        s.status = (int32_t*)o;
+        o += 256;
+        s.ws = o;
+        s.ws_bytes = al256(sp.ws_bytes);
+        s.cap = sp.cap;
+        s.h_last = h_small + q * 8;
+        s.h_status = (int32_t*)(h_small + q * 8 + 1);
+    }
+
+    // ---- inputs host -> device, once ---------------------------------------------------------------------------------
+    cudaEvent_t up;
+    QP_H(cudaEventCreateWithFlags(&up, cudaEventDisableTiming));
+    cudaMemcpyAsync(d_seqs, h_seqs + h_offsets[0], (size_t)seq_bytes, cudaMemcpyHostToDevice, main);
+    if (h_offsets[0] == 0) {
+        cudaMemcpyAsync(d_offs, h_offsets, (size_t)(k + 1) * 8, cudaMemcpyHostToDevice, main);
+    } else {   // the device copy of the sequences starts at 0
+        std::vector<int64_t> sh(k + 1);
+        for (int q = 0; q <= k; ++q) sh[q] = h_offsets[q] - h_offsets[0];
+        cudaMemcpy(d_offs, sh.data(), (size_t)(k + 1) * 8, cudaMemcpyHostToDevice);
+    }
+    cudaMemsetAsync(d_dist, 0, (size_t)k * k * 4, main);
+    cudaEventRecord(up, main);
+    out->h2d_bytes += seq_bytes + (int64_t)(k + 1) * 8;
+    for (Slot& s : sl) cudaStreamWaitEvent(s.st, up, 0);
+
+    // enqueue one batch on a slot: pairs up, the stage, sizes and status down
+    auto enqueue = [&](Slot& s, const Batch& b) -> int {
+        s.cur = b;
+        const int64_t nb = b.hi - b.lo;
+        cudaMemcpyAsync(s.pairs, h_pairs + 2 * b.lo, (size_t)nb * 8, cudaMemcpyHostToDevice, s.st);
+        out->h2d_bytes += nb * 8;
+        qp_output o;
+        o.pair_row_base = s.row_base;
+        o.pair_nnz_base = s.nnz_base;
+        o.row_ptr = s.row_ptr;
+        o.col_idx = s.col;
+        o.val = s.val;
+        o.nnz_capacity = s.cap;
+        o.dist = d_dist;
+        o.dense_P = nullptr;
+        o.logZ = nullptr;
+        o.status = s.status;
+        const int r = qp_posteriors(d_seqs, d_offs, k, s.pairs, nb, &prm, s.ws, (size_t)s.ws_bytes, &o, s.st);
+        if (r != QP_OK) return r;
+        cudaMemcpyAsync(s.h_last, s.nnz_base + nb, 8, cudaMemcpyDeviceToHost, s.st);
+        cudaMemcpyAsync(s.h_status, s.status, 16, cudaMemcpyDeviceToHost, s.st);
+        // row pointers do not depend on the CSR size: straight to their place in the caller's array
+        cudaMemcpyAsync(out->row_ptr + out->pair_row_base[b.lo], s.row_ptr, (size_t)b.rows * 4, cudaMemcpyDeviceToHost, s.st);
+        cudaMemcpyAsync(out->pair_nnz_base + b.lo + 1, s.nnz_base + 1, (size_t)nb * 8, cudaMemcpyDeviceToHost, s.st);
+        cudaEventRecord(s.sized, s.st);
+        out->d2h_bytes += 24 + b.rows * 4 + nb * 8;
+        return cudaGetLastError() == cudaSuccess ? QP_OK : QP_ERR_CUDA;
+    };
+
+    // ---- the pipeline ---------------------------------------------------------------------------------------------------
+    // work list: batches in order; a batch whose CSR does not fit its slot is split in two and taken again
+    std::vector<Batch> work(batches.rbegin(), batches.rend());   // stack: next batch at the back
+    int64_t nnz_running = 0;     // entries of the batches collected so far
+    int64_t required = 0;        // entries needed in all (keeps counting past the caller's capacity)
+    bool host_overflow = false;
+    std::vector<int> inflight;   // slots in enqueue order
+    int next_slot = 0;
+    auto collect = [&](int q) -> int {   // sizes known -> CSR down -> fix the prefix; returns QP_OK, an error, or 1 = "split"
+        Slot& s = sl[q];
+        if (cudaEventSynchronize(s.sized) != cudaSuccess) return QP_ERR_CUDA;
+        const int code = s.h_status[0];
+        const Batch b = s.cur;
+        const int64_t nb = b.hi - b.lo;
+        if (code == QP_ERR_NNZ_CAPACITY && nb > 1) return 1;
+        if (code != QP_OK) {
+            out->status[0] = code;
+            out->status[1] = s.h_status[1] >= 0 ? (int32_t)(b.lo + s.h_status[1]) : -1;
+            return code;
+        }
+        const int64_t nz = *s.h_last;
+        out->status[3] += s.h_status[3];
+        required += nz;
+        if (nnz_running + nz > out->nnz_capacity) {
+            host_overflow = true;
+        } else {
+            cudaMemcpyAsync(out->col_idx + nnz_running, s.col, (size_t)nz * 4, cudaMemcpyDeviceToHost, s.st);
+            cudaMemcpyAsync(out->val + nnz_running, s.val, (size_t)nz * 4, cudaMemcpyDeviceToHost, s.st);
+            out->d2h_bytes += nz * 8;
+        }
+        cudaEventRecord(s.done, s.st);
+        // the batch's pair_nnz_base arrived as local offsets (copied before `sized`): make them global
+        for (int64_t p = b.lo + 1; p <= b.hi; ++p) out->pair_nnz_base[p] += nnz_running;
+        nnz_running += nz;
+        ++out->batches;
+        return QP_OK;
+    };
+    while (rc == QP_OK && (!work.empty() || !inflight.empty())) {
+        // keep two batches in flight
+        while (rc == QP_OK && !work.empty() && inflight.size() < 2) {
+            Slot& s = sl[next_slot];
+            cudaEventSynchronize(s.done);            // the slot's previous CSR has left the device
+            rc = enqueue(s, work.back());
+            work.pop_back();
+            inflight.push_back(next_slot);
+            next_slot ^= 1;
+        }
+        if (rc != QP_OK) break;
+        const int q = inflight.front();
+        const int r = collect(q);
+        if (r == 1) {
+            // denser than beta_guess: everything enqueued after this batch is abandoned (its results are simply
+            // computed again), the batch goes back as two halves
+            for (int other : inflight) cudaStreamSynchronize(sl[other].st);
+            for (size_t u = inflight.size(); u-- > 1;) work.push_back(sl[inflight[u]].cur);
+            const Batch b = sl[q].cur;
+            int64_t mid = b.lo, acc = 0;
+            while (mid < b.hi - 1 && acc + cells[mid] <= b.cells / 2) acc += cells[mid++];
+            if (mid == b.lo) mid = b.lo + 1;
+            Batch hi_half{mid, b.hi, 0, 0}, lo_half{b.lo, mid, 0, 0};
+            for (int64_t p = b.lo; p < b.hi; ++p) {
+                Batch& t = p < mid ? lo_half : hi_half;
+                t.cells += cells[p];
+                t.rows += out->pair_row_base[p + 1] - out->pair_row_base[p];
+            }
+            work.push_back(hi_half);
+            work.push_back(lo_half);
+            inflight.clear();
+            next_slot = 0;
+            cudaEventRecord(sl[0].done, sl[0].st);
+            cudaEventRecord(sl[1].done, sl[1].st);
+            continue;
+        }
+        rc = r;
+        inflight.erase(inflight.begin());
+    }
+    for (Slot& s : sl) cudaStreamSynchronize(s.st);
+    if (rc == QP_OK) {
+        cudaMemcpyAsync(out->dist, d_dist, (size_t)k * k * 4, cudaMemcpyDeviceToHost, main);
+        out->d2h_bytes += (int64_t)k * k * 4;
+        if (cudaStreamSynchronize(main) != cudaSuccess) rc = QP_ERR_CUDA;
+    }
+    cudaEventDestroy(up);
+    cleanup();
+#undef QP_H
+    if (rc == QP_OK && host_overflow) {
+        rc = QP_ERR_NNZ_CAPACITY;
+        out->pair_nnz_base[P] = required;
+    }
+    if (rc != QP_OK && out->status[0] == 0) out->status[0] = rc;
+    return rc;
+}

@@ -208,7 +208,8 @@ __device__ __forceinline__ void lds16(double2& v, uint32_t addr) {
 }
 
 // append a kept posterior to its row's entry buffer and advance the buffer pointer: predicated 8-byte store and
-// predicated 64-bit add, no branch
+// predicated 64-bit add, no branch. (A 32-bit entry count + mad.wide address under the predicate is three instructions
+// instead of seven in SASS, but needs one more live register and the C = 8..12 kernels then spill: measured +20 %.)
 __device__ __forceinline__ void st_entry_adv(char*& ptr, float val, int col, bool keep) {
     asm volatile(
         "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %3, 0;\n\t@p st.global.v2.b32 [%0], {%1, %2};\n\t@p add.s64 %0, %0, 8;\n\t}"
@@ -544,6 +545,8 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
         auto issue = [&](int tt) {   // bulk-copy the F area of step tt
             const uint32_t st = ring.issued % kStages;
             if (lane == 0) {   // one lane issues: the copy instruction takes uniform operands
+                // (copying only the on-grid lanes' share of every unit row on the ramp steps -- kUnits small copies
+                // instead of one -- saves ~4 % of the reads and was measured no faster: round 2)
                 const uint32_t mb = ring.mbar + st * 8;
                 mbar_expect_tx(mb, kUnits * 512);
                 bulk_g2s(ring.data + st * (kUnits * 512), blk0 + (int64_t)tt * stride, kUnits * 512, mb);

@@ -19,12 +19,13 @@ QP_OK = 0
 ERR = {"INVALID_ARG": -1, "BAD_RESIDUE": -2, "EMPTY_SEQUENCE": -3, "BAD_PAIR": -4, "WORKSPACE_TOO_SMALL": -5,
        "NNZ_CAPACITY": -6, "CUDA": -7, "RANGE": -8}
 QP_FP32, QP_FP64 = 0, 1
-FLAG_SYNC_STATUS, FLAG_NO_REFINE = 1, 2
+FLAG_SYNC_STATUS, FLAG_NO_REFINE, FLAG_NO_POLLERS = 1, 2, 4
 NUM_CLASSES = 18
 
 EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_posteriors_budgeted", "qp_guide_tree", "qp_guide_tree_workspace_bytes", "qp_last_launch_count", "qp_status_string", "qp_version",
            "qp_set_profile", "qp_get_profile", "qp_get_profile_classes", "qp_shutdown",
-           "qp_consistency", "qp_consistency_workspace_bytes", "qp_consistency_passes", "qp_last_tau_curve"]
+           "qp_consistency", "qp_consistency_workspace_bytes", "qp_consistency_passes", "qp_last_tau_curve", "qp_measure_peaks",
+           "qp_posteriors_host", "qp_posteriors_host_workspace_bytes"]
 
 
 class QpError(RuntimeError):
@@ -66,6 +67,18 @@ class _ConsParams(C.Structure):
                 ("threshold", C.c_double)]
 
 
+class _HostOutput(C.Structure):
+    _fields_ = [("pair_row_base", C.c_void_p), ("pair_nnz_base", C.c_void_p), ("row_ptr", C.c_void_p),
+                ("col_idx", C.c_void_p), ("val", C.c_void_p), ("nnz_capacity", C.c_int64), ("dist", C.c_void_p),
+                ("beta_guess", C.c_double), ("status", C.c_int32 * 4), ("batches", C.c_int32), ("reserved", C.c_int32),
+                ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64)]
+
+
+class _Peaks(C.Structure):
+    _fields_ = [("sms", C.c_int32), ("reserved", C.c_int32), ("ffma_per_s", C.c_double), ("ffma2_fma_per_s", C.c_double),
+                ("mufu_per_s", C.c_double), ("warp_instr_per_s", C.c_double)]
+
+
 SEL = {"max": 0, "min": 1, "sum": 2}
 
 
@@ -103,6 +116,14 @@ def _load():
     L.qp_consistency.restype = C.c_int
     L.qp_consistency.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.POINTER(_Csr), C.c_int64, C.c_void_p,
                                  C.POINTER(_ConsParams), C.c_void_p, C.c_size_t, C.POINTER(_CsrOut), C.c_void_p]
+    L.qp_posteriors_host_workspace_bytes.restype = C.c_int
+    L.qp_posteriors_host_workspace_bytes.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.POINTER(_Params), C.c_double,
+                                                     C.POINTER(C.c_size_t)]
+    L.qp_posteriors_host.restype = C.c_int
+    L.qp_posteriors_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_void_p, C.c_int64, C.POINTER(_Params), C.c_void_p,
+                                     C.c_size_t, C.POINTER(_HostOutput), C.c_void_p]
+    L.qp_measure_peaks.restype = C.c_int
+    L.qp_measure_peaks.argtypes = [C.POINTER(_Peaks), C.c_void_p, C.c_size_t, C.c_void_p]
     L.qp_last_tau_curve.restype = C.c_int
     L.qp_last_tau_curve.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_int64), C.c_int]
     L.qp_consistency_passes.restype = C.c_int
@@ -362,6 +383,20 @@ def last_tau_curve(max_bins: int = 128):
     return np.array(tau[:n]), np.array(cnt[:n], dtype=np.int64)
 
 
+def measure_peaks(device="cuda:0") -> dict:
+    """qp_measure_peaks: measured FFMA / FFMA2 / MUFU rates and the warp-instruction issue rate of the device."""
+    import torch
+    dev = torch.device(device)
+    scratch = torch.empty(1 << 20, dtype=torch.uint8, device=dev)
+    pk = _Peaks()
+    with torch.cuda.device(dev):
+        r = _lib.qp_measure_peaks(C.byref(pk), scratch.data_ptr(), scratch.numel(), C.c_void_p(torch.cuda.current_stream(dev).cuda_stream))
+    if r != QP_OK:
+        raise QpError(r)
+    return dict(sms=pk.sms, ffma_per_s=pk.ffma_per_s, ffma2_fma_per_s=pk.ffma2_fma_per_s, mufu_per_s=pk.mufu_per_s,
+                warp_instr_per_s=pk.warp_instr_per_s)
+
+
 def consistency_passes(k: int) -> int:
     """qp_consistency_passes: the paper's rule, 2 transformations for k < 50, 1 otherwise."""
     return int(_lib.qp_consistency_passes(int(k)))
@@ -411,3 +446,57 @@ def consistency(d_offsets, k, d_pairs, csr, treedist, *, h_offsets, h_pairs, nnz
     if check and code != QP_OK:
         raise QpError(code)
     return out
+
+
+class HostCall:
+    """qp_posteriors_host: the posterior stage on HOST buffers (pinned torch CPU tensors), one C call per family.
+    Allocates the pinned inputs / outputs and the device workspace once; `run()` may be called again and again.
+    Marshalling only: batching, copies and stream ordering happen inside libqp.so (csrc/qp_host.cu)."""
+
+    def __init__(self, family, pairs, params, *, device="cuda:0", beta_guess=0.05, nnz_capacity=None, workspace_bytes=None,
+                 precision="fp32", flags=0):
+        import torch
+        self.torch = torch
+        self.dev = torch.device(device)
+        self.k = int(family.k)
+        pairs = np.ascontiguousarray(pairs, dtype=np.int32).reshape(-1, 2)
+        self.P = len(pairs)
+        L = family.lengths
+        n, m = L[pairs[:, 0]].astype(np.int64), L[pairs[:, 1]].astype(np.int64)
+        self.cells = int((n * m).sum())
+        rows_total = int((n + 1).sum())
+        self.cp = CParams(params, precision=precision, flags=flags)
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        self.h_seqs, self.h_offs, self.h_pairs = pin(family.seqs), pin(family.offsets.astype(np.int64)), pin(pairs)
+        cap = int(nnz_capacity) if nnz_capacity is not None else int(1.2 * beta_guess * self.cells) + 4096
+        e = lambda size, dt: torch.empty(max(int(size), 1), dtype=dt).pin_memory()
+        self.pair_row_base, self.pair_nnz_base = e(self.P + 1, torch.int64), e(self.P + 1, torch.int64)
+        self.row_ptr, self.col_idx, self.val = e(rows_total, torch.int32), e(cap, torch.int32), e(cap, torch.float32)
+        self.dist = torch.empty((self.k, self.k), dtype=torch.float32).pin_memory()
+        self.cap, self.beta_guess = cap, float(beta_guess)
+        need = C.c_size_t(0)
+        r = _lib.qp_posteriors_host_workspace_bytes(self.h_offs.data_ptr(), self.k, self.h_pairs.data_ptr(), self.P, self.cp.ref,
+                                                    self.beta_guess, C.byref(need))
+        if r != QP_OK:
+            raise QpError(r)
+        self.ws = torch.empty(int(workspace_bytes) if workspace_bytes else max(int(need.value), 256), dtype=torch.uint8, device=self.dev)
+        self.out = _HostOutput()
+
+    def run(self, stream=None, check=True):
+        """One call. Returns self (pinned tensors pair_row_base, pair_nnz_base, row_ptr, col_idx, val, dist are filled;
+        .nnz, .batches, .h2d_bytes, .d2h_bytes, .code, .refined are set)."""
+        torch = self.torch
+        o = self.out
+        o.pair_row_base, o.pair_nnz_base, o.row_ptr = self.pair_row_base.data_ptr(), self.pair_nnz_base.data_ptr(), self.row_ptr.data_ptr()
+        o.col_idx, o.val, o.nnz_capacity, o.dist = self.col_idx.data_ptr(), self.val.data_ptr(), self.cap, self.dist.data_ptr()
+        o.beta_guess = self.beta_guess
+        st = stream if stream is not None else torch.cuda.current_stream(self.dev)
+        with torch.cuda.device(self.dev):
+            code = _lib.qp_posteriors_host(self.h_seqs.data_ptr(), self.h_offs.data_ptr(), self.k, self.h_pairs.data_ptr(), self.P,
+                                           self.cp.ref, self.ws.data_ptr(), self.ws.numel(), C.byref(o), C.c_void_p(st.cuda_stream))
+        self.code, self.batches = int(code), int(o.batches)
+        self.h2d_bytes, self.d2h_bytes, self.refined = int(o.h2d_bytes), int(o.d2h_bytes), int(o.status[3])
+        self.nnz = int(self.pair_nnz_base[self.P].item()) if self.P else 0
+        if check and code != QP_OK:
+            raise QpError(code, f"(pair {o.status[1]})")
+        return self

@@ -63,7 +63,8 @@ class HostStreamer:
         max_rows = max(self.rows) if nb else 1
         max_pairs = max(bounds[b + 1] - bounds[b] for b in range(nb)) if nb else 1
         self.cap = int(beta_guess * max_cells) + 4096
-        self.cp = qp.CParams(params, precision=precision, flags=0)   # no sync inside the call: status is read with the CSR sizes
+        # no sync inside the call (status is read with the CSR sizes); two calls are in flight: no pollers (qp.h)
+        self.cp = qp.CParams(params, precision=precision, flags=qp.FLAG_NO_POLLERS)
         i64, i32, f32 = torch.int64, torch.int32, torch.float32
         self.h_seqs = torch.from_numpy(np.ascontiguousarray(family.seqs)).pin_memory()
         self.h_offs = torch.from_numpy(np.ascontiguousarray(family.offsets, dtype=np.int64)).pin_memory()

@@ -320,6 +320,42 @@ def test_host_streamer_matches_single_call(default_params):
     assert torch.equal(hs.dist, ref.dist.cpu())
 
 
+def test_host_call_matches_single_call(default_params):
+    """qp_posteriors_host (host buffers in, host buffers out, batching inside the C library) returns the same CSR and
+    distances as one device-resident call: default workspace, a workspace so small that batches must shrink, and a
+    density guess so low that batches overflow and are split."""
+    qp = _qp()
+    import torch
+    fam = inputs.config_family(1)
+    pairs = inputs.all_pairs(fam.k)
+    ref = qp.run_family(fam, pairs, default_params)
+    nz = int(ref.pair_nnz_base[-1].item())
+    want = dict(rb=ref.pair_row_base.cpu(), nb=ref.pair_nnz_base.cpu(), rp=ref.row_ptr.cpu(), col=ref.col_idx[:nz].cpu(),
+                val=ref.val[:nz].cpu(), dist=ref.dist.cpu())
+
+    def same(hc):
+        assert hc.code == 0 and hc.nnz == nz
+        assert torch.equal(hc.pair_row_base, want["rb"]) and torch.equal(hc.pair_nnz_base, want["nb"])
+        assert torch.equal(hc.row_ptr[: len(want["rp"])], want["rp"])
+        assert torch.equal(hc.col_idx[:nz], want["col"]) and torch.equal(hc.val[:nz], want["val"])
+        assert torch.equal(hc.dist, want["dist"])
+        assert hc.refined == int(ref.status[3].item())
+        assert hc.d2h_bytes >= 8 * nz and hc.h2d_bytes >= fam.seqs.nbytes
+
+    hc = qp.HostCall(fam, pairs, default_params)
+    same(hc.run())
+    same(hc.run())                                             # reusable
+    small = qp.HostCall(fam, pairs, default_params, workspace_bytes=hc.ws.numel() // 6)
+    same(small.run())
+    assert small.batches > hc.batches
+    dense = qp.HostCall(fam, pairs, default_params, beta_guess=0.004, nnz_capacity=nz + 16)
+    same(dense.run())
+    assert dense.batches > hc.batches                          # overflowing batches were split
+    tight = qp.HostCall(fam, pairs, default_params, nnz_capacity=nz // 2)
+    tight.run(check=False)
+    assert tight.code == qp.ERR["NNZ_CAPACITY"] and int(tight.pair_nnz_base[len(pairs)].item()) == nz
+
+
 def test_fuzz_random_pairs_models_thresholds():
     """Seeded fuzz: random lengths (1..400, incl. very skewed pairs), random symmetric models with G in {1,2} for
     either automaton, alphabets 4 / 12 / 20 / 31, thresholds 0.001 .. 0.2, both precisions."""
