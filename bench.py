@@ -484,10 +484,16 @@ def main():
                     help="N>1: one independent family per rank (the paper's bulk mode, weak scaling, no collective) "
                          "instead of the default: ONE family sharded over the ranks + NCCL all-reduce of the distances")
     ap.add_argument("--no-configs", action="store_true", help="skip the configs[2] / configs[4] block of the default run")
+    ap.add_argument("--stage3", type=int, default=None, metavar="CFG",
+                    help="only the stage II + III measurement (qp_guide_tree + qp_consistency) on configs[CFG]; prints its block")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.stage3 is not None:
+        import torch
+        from paper_1512_07437_b200 import inputs
+        print(json.dumps({"stage3": measure_stage3(args.stage3, torch.device("cuda", 0), inputs.default_params())}), flush=True)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
