@@ -235,3 +235,41 @@ def test_chain_stage1_tree_consistency_on_the_gpu(default_params):
     rows = np.repeat(np.arange(len(rp) - 1), np.diff(rp))
     both = Rd[rows, col] > 0
     assert both.mean() > 0.99 and np.abs(val[both] - Rd[rows[both], col[both]]).max() <= 1e-4
+
+
+def test_error_paths_and_empty_input(default_params):
+    """qp_consistency argument and device-detected errors: bad pair, undersized workspace, undersized output, an empty
+    pair list; and qp_shutdown between calls (the library re-creates its streams)."""
+    import torch
+    qp = _qp()
+    dev = torch.device("cuda:0")
+    fam = inputs.config_family(0)
+    pairs = inputs.all_pairs(fam.k)
+    S, td = _oracle_stage1(fam, pairs, default_params)
+    d_offs = torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev)
+    d_pairs = torch.from_numpy(pairs).to(dev)
+    d_td = torch.from_numpy(np.ascontiguousarray(td, dtype=np.int32)).to(dev)
+    csr, nnz = _upload(S, pairs, fam, dev)
+    kw = dict(h_offsets=fam.offsets, h_pairs=pairs, nnz=nnz, T=9, threshold=default_params.threshold)
+    ok = qp.consistency(d_offs, fam.k, d_pairs, csr, d_td, **kw)
+    assert ok.code == 0
+    qp.shutdown()                                           # streams and events of this thread are released ...
+    again = qp.consistency(d_offs, fam.k, d_pairs, csr, d_td, **kw)
+    assert torch.equal(ok.val[:int(ok.pair_nnz_base[-1])], again.val[:int(again.pair_nnz_base[-1])])
+    res1 = qp.run_family(fam, pairs, default_params)        # ... and re-created by the next stage-I call
+    assert res1.code == 0
+    # a pair that lists a sequence with itself: host query and device check
+    bad = pairs.copy()
+    bad[3] = (2, 2)
+    with pytest.raises(qp.QpError) as ei:
+        qp.consistency(d_offs, fam.k, torch.from_numpy(bad).to(dev), csr, d_td, **dict(kw, h_pairs=bad))
+    assert ei.value.code == qp.ERR["BAD_PAIR"]
+    # workspace too small
+    small = torch.empty(1 << 16, dtype=torch.uint8, device=dev)
+    with pytest.raises(qp.QpError) as ei:
+        qp.consistency(d_offs, fam.k, d_pairs, csr, d_td, workspace=small, **kw)
+    assert ei.value.code == qp.ERR["WORKSPACE_TOO_SMALL"]
+    # empty pair list
+    none = np.zeros((0, 2), np.int32)
+    r0 = qp.consistency(d_offs, fam.k, torch.from_numpy(none).to(dev), csr, d_td, **dict(kw, h_pairs=none, nnz=0))
+    assert r0.code == 0 and int(r0.pair_nnz_base[0].item()) == 0
