@@ -355,7 +355,7 @@ static void prof_mark(Ctx* c, int i, cudaStream_t st) {
 static inline int64_t align256(int64_t v) { return (v + 255) & ~(int64_t)255; }
 
 struct Layout {   // byte offsets inside the workspace
-    int64_t hdr, info, order, rows1, cells, nnz, pool_off, dense_off, slot_off, refine_list, tau_hist, pool, slots;
+    int64_t hdr, info, order, rows1, cells, nnz, pool_off, dense_off, slot_off, refine_list, tau_hist, scan_tmp, pool, slots;
     int64_t fixed;   // everything before the slots
 };
 
@@ -378,6 +378,7 @@ static Layout make_layout(int64_t P, int64_t nnz_cap, bool dense, int64_t max_sl
     L.slot_off = take(max_slots * 8);
     L.refine_list = take((int64_t)kNumRefine * (P + kListPad) * 4);
     L.tau_hist = take((int64_t)kTauBins * 8);
+    L.scan_tmp = take((P / kScanChunk + 2) * 2 * 8);
     L.pool = take(nnz_cap * 8);
     L.slots = o;
     L.fixed = o;
@@ -745,12 +746,9 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     for (int c = 0; c < kNumClasses; ++c) mw.w[c] = ((cmask >> c) & 1) ? max_units(c, fp64, sms) : 0;
     k_slots<<<1, 1024, 0, st>>>((const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), mw, avail,
                                 (int64_t*)(ws + L.slot_off), hdr);
-    k_scan<int32_t><<<1, 1024, 0, st>>>((const int32_t*)(ws + L.rows1), P, out->pair_row_base);
-    g_launches += 2;
-    if (dense) {
-        k_scan<int64_t><<<1, 1024, 0, st>>>((const int64_t*)(ws + L.cells), P, (int64_t*)(ws + L.dense_off));
-        ++g_launches;
-    }
+    ++g_launches;
+    scan_launch<int32_t>((const int32_t*)(ws + L.rows1), P, out->pair_row_base, (int64_t*)(ws + L.scan_tmp), st, &g_launches);
+    if (dense) scan_launch<int64_t>((const int64_t*)(ws + L.cells), P, (int64_t*)(ws + L.dense_off), (int64_t*)(ws + L.scan_tmp), st, &g_launches);
     QP_TRY(cudaGetLastError());
 
     // ---- a1..a7: one persistent kernel per class, forked onto side streams ----------------------------------
@@ -804,7 +802,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     // ---- CSR placement in pair order; it only needs the fp32 pass, so it runs beside the fp64 kernels ------------
     cudaStream_t ps = refine ? cx->st[kNumStreams - 1] : st;
     if (refine) QP_TRY(cudaStreamWaitEvent(ps, cx->fork2, 0));
-    k_scan<int32_t><<<1, 1024, 0, ps>>>((const int32_t*)(ws + L.nnz), P, out->pair_nnz_base);
+    scan_launch<int32_t>((const int32_t*)(ws + L.nnz), P, out->pair_nnz_base, (int64_t*)(ws + L.scan_tmp), ps, &g_launches);
     if (out->nnz_capacity > 0)
         k_copy_pool<<<(int)((P + 3) / 4), 128, 0, ps>>>((const int32_t*)(ws + L.nnz), (const int64_t*)(ws + L.pool_off),
                                                         out->pair_nnz_base, P, (const float2*)(ws + L.pool), out->nnz_capacity,
@@ -819,7 +817,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     }
     prof_mark(cx, 3, st);
     k_finish<<<1, 32, 0, st>>>(hdr, out->status);
-    g_launches += 3;
+    g_launches += 2;
     prof_mark(cx, 4, st);
     QP_TRY(cudaGetLastError());
 #undef QP_TRY
