@@ -457,7 +457,7 @@ def run_e2e(args, fam, pairs, prm, qp, dev, my_cells):
     "memory-budgeted by streaming pair batches") and copies the distance matrix and the WHOLE CSR back to pinned host
     memory; batch b's copies overlap batch b+1's kernels (csrc/qp_host.cu)."""
     import torch
-    hc = qp.HostCall(fam, pairs, prm, device=str(dev))
+    hc = qp.HostCall(fam, pairs, prm, device=str(dev), compact_cols=True)
     hc.run()   # warm-up
     torch.cuda.synchronize()
     steps = max(1, min(args.steps, 3))
@@ -468,7 +468,7 @@ def run_e2e(args, fam, pairs, prm, qp, dev, my_cells):
     wall = time.perf_counter() - t0
     return {"value": my_cells * steps / wall, "unit": UNIT, "h2d_bytes_per_step": hc.h2d_bytes,
             "d2h_bytes_per_step": hc.d2h_bytes, "ms_per_step": 1e3 * wall / steps, "steps": steps,
-            "batches": hc.batches, "nnz": hc.nnz,
+            "batches": hc.batches, "nnz": hc.nnz, "csr_columns": "uint16 (qp_host_output.col_idx16: lossless, QP_MAX_LEN = 65535)",
             "note": "host wall clock around qp_posteriors_host (one C-ABI call per step, pinned host buffers): H2D of the "
                     "inputs, qp_posteriors per pair batch, D2H of distances and the full CSR (two batches in flight: "
                     "copies overlap the next batch's kernels)"}

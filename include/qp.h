@@ -145,10 +145,12 @@ typedef struct {
     int64_t* pair_row_base;  /* [P+1] */
     int64_t* pair_nnz_base;  /* [P+1] */
     int32_t* row_ptr;        /* [sum(n_p+1)] */
-    int32_t* col_idx;        /* [nnz_capacity] */
+    int32_t* col_idx;        /* [nnz_capacity]; not written (may be NULL) when col_idx16 is given */
     float* val;              /* [nnz_capacity] */
     int64_t nnz_capacity;
     float* dist;             /* [k*k] */
+    uint16_t* col_idx16;     /* optional [nnz_capacity]: the columns as 16-bit values instead (lossless, QP_MAX_LEN is
+                                65535): 6 instead of 8 bytes per entry cross PCIe, which is what bounds this call */
     double beta_guess;       /* in */
     int32_t status[4];       /* out: {code, pair index or -1, detail, pairs re-evaluated in fp64} */
     int32_t batches;         /* out */

@@ -2,9 +2,10 @@
 //
 // BASELINE.json configs[3]: "memory-budgeted by streaming pair batches". The caller's data lives in host memory;
 // the pair list is cut into batches that fit the device workspace twice, and two batches are in flight: while batch
-// b's CSR travels back over PCIe on one stream, batch b+1's kernels run on the other, so the wall time of a family
-// is max(compute, copy) instead of their sum. Every step of the computation runs inside qp_posteriors (this file
-// only plans batches, moves buffers and orders streams; it is written against the public C ABI).
+// b's CSR travels back over PCIe on the slot's copy stream, batch b+1's kernels run on the compute stream, so the wall
+// time of a family is max(compute, copy) instead of their sum. Every step of the computation runs inside qp_posteriors (this file
+// only plans batches, moves buffers and orders streams; it is written against the public C ABI; its one kernel
+// narrows the column indices to 16 bits when the caller asks for the compact form).
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -18,6 +19,15 @@ namespace {
 
 inline int64_t al256(int64_t v) { return (v + 255) & ~(int64_t)255; }
 
+// columns as 16-bit values for the trip over PCIe (QP_MAX_LEN = 65535: lossless); the count is read on the device
+__global__ void k_narrow_cols(const int32_t* __restrict__ col, const int64_t* __restrict__ count, uint16_t* __restrict__ col16) {
+    const int64_t n = *count;
+    for (int64_t q = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) * 2; q < n; q += (int64_t)gridDim.x * blockDim.x * 2) {
+        if (q + 1 < n) *(ushort2*)(col16 + q) = make_ushort2((unsigned short)col[q], (unsigned short)col[q + 1]);
+        else col16[q] = (uint16_t)col[q];
+    }
+}
+
 struct Batch {
     int64_t lo, hi;        // pairs [lo, hi)
     int64_t cells, rows;   // sum n*m, sum (n+1)
@@ -30,6 +40,7 @@ struct Slot {              // device buffers of one batch in flight + its stream
     int32_t* pairs = nullptr;
     int64_t *row_base = nullptr, *nnz_base = nullptr;
     int32_t *row_ptr = nullptr, *col = nullptr, *status = nullptr;
+    uint16_t* col16 = nullptr;
     float* val = nullptr;
     char* ws = nullptr;
     int64_t ws_bytes = 0, cap = 0;
@@ -47,8 +58,8 @@ struct SlotPlan {
 // bytes of one slot for batches of at most these sizes
 SlotPlan plan_slot(int64_t max_pairs, int64_t max_rows, int64_t cap, int64_t ws_bytes) {
     SlotPlan p{max_pairs, max_rows, cap, ws_bytes, 0};
-    p.total = al256(max_pairs * 8) + 2 * al256((max_pairs + 1) * 8) + al256(max_rows * 4) + 2 * al256(cap * 4) + 256 +
-              al256(ws_bytes);
+    p.total = al256(max_pairs * 8) + 2 * al256((max_pairs + 1) * 8) + al256(max_rows * 4) + 2 * al256(cap * 4) + al256(cap * 2) +
+              256 + al256(ws_bytes);
     return p;
 }
 
@@ -105,7 +116,7 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
                                   qp_host_output* out, void* cuda_stream) {
     if (!out || !params || !h_offsets || k < 0 || P < 0 || (P > 0 && (!h_seqs || !h_pairs || !d_workspace))) return QP_ERR_INVALID_ARG;
     if (!out->pair_row_base || !out->pair_nnz_base || (P > 0 && (!out->row_ptr || !out->dist))) return QP_ERR_INVALID_ARG;
-    if (out->nnz_capacity < 0 || (out->nnz_capacity > 0 && (!out->col_idx || !out->val))) return QP_ERR_INVALID_ARG;
+    if (out->nnz_capacity < 0 || (out->nnz_capacity > 0 && ((!out->col_idx && !out->col_idx16) || !out->val))) return QP_ERR_INVALID_ARG;
     if (((uintptr_t)d_workspace & 255) != 0) return QP_ERR_INVALID_ARG;
     out->h2d_bytes = out->d2h_bytes = 0;
     out->batches = 0;
@@ -138,7 +149,7 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
     const int64_t seq_bytes = h_offsets[k] - h_offsets[0];
     const int64_t common = al256(seq_bytes) + al256((int64_t)(k + 1) * 8) + al256((int64_t)k * k * 4);
     qp_params prm = *params;
-    prm.flags = (prm.flags & ~QP_FLAG_SYNC_STATUS) | QP_FLAG_NO_POLLERS;   // several calls in flight: see qp.h
+    prm.flags &= ~QP_FLAG_SYNC_STATUS;   // the batches' kernels run one call after the other on one stream
 
     std::vector<Batch> batches;
     SlotPlan sp{0, 0, 0, 0, 0};
@@ -158,6 +169,27 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
             }
         }
         if (b.hi > b.lo) batches.push_back(b);
+        // taper the end: nothing overlaps the copy of the LAST batch, so the last batch is cut into 1/2, 1/4, 1/4
+        if (batches.size() >= 2 && batches.back().cells > 400000000 && batches.back().hi - batches.back().lo >= 8) {
+            const Batch last = batches.back();
+            batches.pop_back();
+            const double cut[2] = {0.5 * (double)last.cells, 0.75 * (double)last.cells};
+            Batch t{last.lo, last.lo, 0, 0};
+            int64_t acc = 0;
+            int ci = 0;
+            for (int64_t p = last.lo; p < last.hi; ++p) {
+                t.cells += cells[p];
+                t.rows += out->pair_row_base[p + 1] - out->pair_row_base[p];
+                t.hi = p + 1;
+                acc += cells[p];
+                if (ci < 2 && (double)acc >= cut[ci]) {
+                    batches.push_back(t);
+                    t = Batch{p + 1, p + 1, 0, 0};
+                    ++ci;
+                }
+            }
+            if (t.hi > t.lo) batches.push_back(t);
+        }
         int64_t max_pairs = 0, max_rows = 0, max_cells = 0;
         for (const Batch& q : batches) {
             max_pairs = std::max(max_pairs, q.hi - q.lo);
@@ -199,6 +231,8 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
     int64_t* d_offs = (int64_t*)(w + al256(seq_bytes));
     float* d_dist = (float*)(w + al256(seq_bytes) + al256((int64_t)(k + 1) * 8));
     Slot sl[2];
+    cudaStream_t comp = nullptr;   // every batch's kernels, in order: two calls with their persistent kernels side by side
+                                   // would starve each other's short tail kernels; a slot's own stream carries its copies
     int rc = QP_OK;
     int64_t* h_small = nullptr;   // pinned: per slot [1] nnz + [4] status
     auto cleanup = [&]() {
@@ -207,6 +241,10 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
             if (s.sized) cudaEventDestroy(s.sized);
             if (s.done) cudaEventDestroy(s.done);
             if (s.st) cudaStreamDestroy(s.st);
+        }
+        if (comp) {
+            cudaStreamSynchronize(comp);
+            cudaStreamDestroy(comp);
         }
         if (h_small) cudaFreeHost(h_small);
         (void)cudaGetLastError();
@@ -219,6 +257,7 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         }                           \
     } while (0)
     QP_H(cudaMallocHost((void**)&h_small, 2 * 64));
+    QP_H(cudaStreamCreateWithFlags(&comp, cudaStreamNonBlocking));
     for (int q = 0; q < 2; ++q) {
         Slot& s = sl[q];
         QP_H(cudaStreamCreateWithFlags(&s.st, cudaStreamNonBlocking));
@@ -238,6 +277,8 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         o += al256(sp.cap * 4);
         s.val = (float*)o;
         o += al256(sp.cap * 4);
+        s.col16 = (uint16_t*)o;
+        o += al256(sp.cap * 2);
         s.status = (int32_t*)o;
         o += 256;
         s.ws = o;
@@ -261,13 +302,15 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
     cudaMemsetAsync(d_dist, 0, (size_t)k * k * 4, main);
     cudaEventRecord(up, main);
     out->h2d_bytes += seq_bytes + (int64_t)(k + 1) * 8;
-    for (Slot& s : sl) cudaStreamWaitEvent(s.st, up, 0);
+    cudaStreamWaitEvent(comp, up, 0);
 
-    // enqueue one batch on a slot: pairs up, the stage, sizes and status down
+    // enqueue one batch: pairs up, the stage, sizes and status down -- all on the compute stream, behind the copy that
+    // last read the slot's buffers
     auto enqueue = [&](Slot& s, const Batch& b) -> int {
         s.cur = b;
         const int64_t nb = b.hi - b.lo;
-        cudaMemcpyAsync(s.pairs, h_pairs + 2 * b.lo, (size_t)nb * 8, cudaMemcpyHostToDevice, s.st);
+        cudaStreamWaitEvent(comp, s.done, 0);
+        cudaMemcpyAsync(s.pairs, h_pairs + 2 * b.lo, (size_t)nb * 8, cudaMemcpyHostToDevice, comp);
         out->h2d_bytes += nb * 8;
         qp_output o;
         o.pair_row_base = s.row_base;
@@ -280,14 +323,16 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         o.dense_P = nullptr;
         o.logZ = nullptr;
         o.status = s.status;
-        const int r = qp_posteriors(d_seqs, d_offs, k, s.pairs, nb, &prm, s.ws, (size_t)s.ws_bytes, &o, s.st);
+        const int r = qp_posteriors(d_seqs, d_offs, k, s.pairs, nb, &prm, s.ws, (size_t)s.ws_bytes, &o, comp);
         if (r != QP_OK) return r;
-        cudaMemcpyAsync(s.h_last, s.nnz_base + nb, 8, cudaMemcpyDeviceToHost, s.st);
-        cudaMemcpyAsync(s.h_status, s.status, 16, cudaMemcpyDeviceToHost, s.st);
-        // row pointers do not depend on the CSR size: straight to their place in the caller's array
+        if (out->col_idx16) k_narrow_cols<<<1184, 256, 0, comp>>>(s.col, s.nnz_base + nb, s.col16);
+        cudaMemcpyAsync(s.h_last, s.nnz_base + nb, 8, cudaMemcpyDeviceToHost, comp);
+        cudaMemcpyAsync(s.h_status, s.status, 16, cudaMemcpyDeviceToHost, comp);
+        cudaEventRecord(s.sized, comp);
+        // what does not depend on the CSR size goes down on the slot's copy stream right away
+        cudaStreamWaitEvent(s.st, s.sized, 0);
         cudaMemcpyAsync(out->row_ptr + out->pair_row_base[b.lo], s.row_ptr, (size_t)b.rows * 4, cudaMemcpyDeviceToHost, s.st);
         cudaMemcpyAsync(out->pair_nnz_base + b.lo + 1, s.nnz_base + 1, (size_t)nb * 8, cudaMemcpyDeviceToHost, s.st);
-        cudaEventRecord(s.sized, s.st);
         out->d2h_bytes += 24 + b.rows * 4 + nb * 8;
         return cudaGetLastError() == cudaSuccess ? QP_OK : QP_ERR_CUDA;
     };
@@ -300,6 +345,21 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
     bool host_overflow = false;
     std::vector<int> inflight;   // slots in enqueue order
     int next_slot = 0;
+    struct Fixup {
+        int64_t lo, hi, base;
+        int slot;
+    };
+    std::vector<Fixup> fixups;   // pair_nnz_base ranges waiting for their copy to land
+    auto apply_fixups = [&](int slot) {   // after the slot's `done` event has completed
+        for (size_t u = 0; u < fixups.size();) {
+            if (fixups[u].slot != slot) {
+                ++u;
+                continue;
+            }
+            for (int64_t p = fixups[u].lo + 1; p <= fixups[u].hi; ++p) out->pair_nnz_base[p] += fixups[u].base;
+            fixups.erase(fixups.begin() + u);
+        }
+    };
     auto collect = [&](int q) -> int {   // sizes known -> CSR down -> fix the prefix; returns QP_OK, an error, or 1 = "split"
         Slot& s = sl[q];
         if (cudaEventSynchronize(s.sized) != cudaSuccess) return QP_ERR_CUDA;
@@ -318,22 +378,22 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         if (nnz_running + nz > out->nnz_capacity) {
             host_overflow = true;
         } else {
-            cudaMemcpyAsync(out->col_idx + nnz_running, s.col, (size_t)nz * 4, cudaMemcpyDeviceToHost, s.st);
+            if (out->col_idx16) cudaMemcpyAsync(out->col_idx16 + nnz_running, s.col16, (size_t)nz * 2, cudaMemcpyDeviceToHost, s.st);
+            else cudaMemcpyAsync(out->col_idx + nnz_running, s.col, (size_t)nz * 4, cudaMemcpyDeviceToHost, s.st);
             cudaMemcpyAsync(out->val + nnz_running, s.val, (size_t)nz * 4, cudaMemcpyDeviceToHost, s.st);
-            out->d2h_bytes += nz * 8;
+            out->d2h_bytes += nz * (out->col_idx16 ? 6 : 8);
         }
         cudaEventRecord(s.done, s.st);
-        // the batch's pair_nnz_base arrived as local offsets (copied before `sized`): make them global
-        for (int64_t p = b.lo + 1; p <= b.hi; ++p) out->pair_nnz_base[p] += nnz_running;
+        s.out_nnz0 = nnz_running;   // the batch's pair_nnz_base arrives as local offsets: made global once `done` has passed
         nnz_running += nz;
         ++out->batches;
+        fixups.push_back({b.lo, b.hi, s.out_nnz0, q});
         return QP_OK;
     };
     while (rc == QP_OK && (!work.empty() || !inflight.empty())) {
         // keep two batches in flight
         while (rc == QP_OK && !work.empty() && inflight.size() < 2) {
-            Slot& s = sl[next_slot];
-            cudaEventSynchronize(s.done);            // the slot's previous CSR has left the device
+            Slot& s = sl[next_slot];   // (its kernels wait on the device for the slot's previous copy: enqueue)
             rc = enqueue(s, work.back());
             work.pop_back();
             inflight.push_back(next_slot);
@@ -345,6 +405,7 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         if (r == 1) {
             // denser than beta_guess: everything enqueued after this batch is abandoned (its results are simply
             // computed again), the batch goes back as two halves
+            cudaStreamSynchronize(comp);
             for (int other : inflight) cudaStreamSynchronize(sl[other].st);
             for (size_t u = inflight.size(); u-- > 1;) work.push_back(sl[inflight[u]].cur);
             const Batch b = sl[q].cur;
@@ -368,7 +429,11 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         rc = r;
         inflight.erase(inflight.begin());
     }
-    for (Slot& s : sl) cudaStreamSynchronize(s.st);
+    cudaStreamSynchronize(comp);
+    for (int q = 0; q < 2; ++q) {
+        cudaStreamSynchronize(sl[q].st);
+        if (rc == QP_OK) apply_fixups(q);
+    }
     if (rc == QP_OK) {
         cudaMemcpyAsync(out->dist, d_dist, (size_t)k * k * 4, cudaMemcpyDeviceToHost, main);
         out->d2h_bytes += (int64_t)k * k * 4;

@@ -70,6 +70,7 @@ class _ConsParams(C.Structure):
 class _HostOutput(C.Structure):
     _fields_ = [("pair_row_base", C.c_void_p), ("pair_nnz_base", C.c_void_p), ("row_ptr", C.c_void_p),
                 ("col_idx", C.c_void_p), ("val", C.c_void_p), ("nnz_capacity", C.c_int64), ("dist", C.c_void_p),
+                ("col_idx16", C.c_void_p),
                 ("beta_guess", C.c_double), ("status", C.c_int32 * 4), ("batches", C.c_int32), ("reserved", C.c_int32),
                 ("h2d_bytes", C.c_int64), ("d2h_bytes", C.c_int64)]
 
@@ -454,7 +455,7 @@ class HostCall:
     Marshalling only: batching, copies and stream ordering happen inside libqp.so (csrc/qp_host.cu)."""
 
     def __init__(self, family, pairs, params, *, device="cuda:0", beta_guess=0.05, nnz_capacity=None, workspace_bytes=None,
-                 precision="fp32", flags=0):
+                 precision="fp32", flags=0, compact_cols=False):
         import torch
         self.torch = torch
         self.dev = torch.device(device)
@@ -471,7 +472,10 @@ class HostCall:
         cap = int(nnz_capacity) if nnz_capacity is not None else int(1.2 * beta_guess * self.cells) + 4096
         e = lambda size, dt: torch.empty(max(int(size), 1), dtype=dt).pin_memory()
         self.pair_row_base, self.pair_nnz_base = e(self.P + 1, torch.int64), e(self.P + 1, torch.int64)
-        self.row_ptr, self.col_idx, self.val = e(rows_total, torch.int32), e(cap, torch.int32), e(cap, torch.float32)
+        # compact_cols: the columns come back as 16-bit values (col_idx16, uint16) instead of int32 (col_idx)
+        self.row_ptr, self.val = e(rows_total, torch.int32), e(cap, torch.float32)
+        self.col_idx = None if compact_cols else e(cap, torch.int32)
+        self.col_idx16 = e(cap, torch.int16).view(torch.uint16) if compact_cols else None   # pinned as int16, read as uint16
         self.dist = torch.empty((self.k, self.k), dtype=torch.float32).pin_memory()
         self.cap, self.beta_guess = cap, float(beta_guess)
         need = C.c_size_t(0)
@@ -488,7 +492,9 @@ class HostCall:
         torch = self.torch
         o = self.out
         o.pair_row_base, o.pair_nnz_base, o.row_ptr = self.pair_row_base.data_ptr(), self.pair_nnz_base.data_ptr(), self.row_ptr.data_ptr()
-        o.col_idx, o.val, o.nnz_capacity, o.dist = self.col_idx.data_ptr(), self.val.data_ptr(), self.cap, self.dist.data_ptr()
+        o.col_idx = self.col_idx.data_ptr() if self.col_idx is not None else None
+        o.col_idx16 = self.col_idx16.data_ptr() if self.col_idx16 is not None else None
+        o.val, o.nnz_capacity, o.dist = self.val.data_ptr(), self.cap, self.dist.data_ptr()
         o.beta_guess = self.beta_guess
         st = stream if stream is not None else torch.cuda.current_stream(self.dev)
         with torch.cuda.device(self.dev):

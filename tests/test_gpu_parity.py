@@ -351,6 +351,10 @@ def test_host_call_matches_single_call(default_params):
     dense = qp.HostCall(fam, pairs, default_params, beta_guess=0.004, nnz_capacity=nz + 16)
     same(dense.run())
     assert dense.batches > hc.batches                          # overflowing batches were split
+    compact = qp.HostCall(fam, pairs, default_params, compact_cols=True).run()      # columns as uint16: 6 B / entry
+    assert compact.code == 0 and compact.nnz == nz and compact.col_idx is None
+    assert torch.equal(compact.col_idx16[:nz].to(torch.int32), want["col"]) and torch.equal(compact.val[:nz], want["val"])
+    assert compact.d2h_bytes < hc.d2h_bytes - nz
     tight = qp.HostCall(fam, pairs, default_params, nnz_capacity=nz // 2)
     tight.run(check=False)
     assert tight.code == qp.ERR["NNZ_CAPACITY"] and int(tight.pair_nnz_base[len(pairs)].item()) == nz
