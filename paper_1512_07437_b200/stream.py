@@ -3,8 +3,10 @@
 BASELINE.json configs[3]: "memory-budgeted by streaming pair batches". The caller's data lives in HOST memory
 (pinned): sequences, offsets and the pair list go host -> device, the k x k distance matrix and the whole CSR
 (pair_row_base, pair_nnz_base, row_ptr, col_idx, val) come back device -> host, batch by batch. Two batches are in
-flight: while batch b's CSR travels back over PCIe on one stream, batch b+1's kernels run on the other, so the wall
-time of a family is max(compute, copy) instead of their sum. Every step of the computation still runs inside
+flight: while batch b's CSR travels back over PCIe on its slot's copy stream, batch b+1's kernels run on the compute
+stream, so the wall time of a family is max(compute, copy) instead of their sum. (The C library has the same driver
+as one call: qp_posteriors_host / qp.HostCall; this class is the generator variant that hands every batch out as soon
+as it is in host memory.) Every step of the computation still runs inside
 qp_posteriors (CUDA); this module only moves buffers and orders streams.
 
     s = HostStreamer(family, pairs, params)          # allocates device workspaces + pinned staging once
@@ -63,8 +65,7 @@ class HostStreamer:
         max_rows = max(self.rows) if nb else 1
         max_pairs = max(bounds[b + 1] - bounds[b] for b in range(nb)) if nb else 1
         self.cap = int(beta_guess * max_cells) + 4096
-        # no sync inside the call (status is read with the CSR sizes); two calls are in flight: no pollers (qp.h)
-        self.cp = qp.CParams(params, precision=precision, flags=qp.FLAG_NO_POLLERS)
+        self.cp = qp.CParams(params, precision=precision, flags=0)   # no sync inside the call: status is read with the CSR sizes
         i64, i32, f32 = torch.int64, torch.int32, torch.float32
         self.h_seqs = torch.from_numpy(np.ascontiguousarray(family.seqs)).pin_memory()
         self.h_offs = torch.from_numpy(np.ascontiguousarray(family.offsets, dtype=np.int64)).pin_memory()
@@ -72,6 +73,7 @@ class HostStreamer:
         self.dist = torch.empty((family.k, family.k), dtype=f32).pin_memory()
         self.d_dist = torch.zeros((family.k, family.k), dtype=f32, device=self.dev)
         self.max_pairs, self.max_rows = max_pairs, max_rows
+        self.comp = torch.cuda.Stream(self.dev)     # every batch's kernels, in order
         self.slots = []
         for _ in range(2):   # two batches in flight
             sl = dict(
@@ -105,20 +107,25 @@ class HostStreamer:
         sl["h_val"] = torch.empty(cap, dtype=torch.float32).pin_memory()
 
     def _enqueue(self, b, d_seqs, d_offs):
-        """H2D of the batch's pairs, the call, D2H of the small arrays (sizes, status); all on the slot's stream."""
+        """H2D of the batch's pairs, the call, D2H of the sizes and the status on the ONE compute stream (two calls with
+        their persistent kernels side by side starve each other's short tail kernels); the other small arrays on the
+        slot's copy stream."""
         torch = self.torch
         s = self.slots[b % 2]
         lo, hi = self.bounds[b], self.bounds[b + 1]
-        with torch.cuda.stream(s["stream"]):
+        self.comp.wait_event(s["done"])            # the slot's previous CSR has left the device
+        with torch.cuda.stream(self.comp):
             s["d_pairs"][: hi - lo].copy_(self.h_pairs[lo:hi], non_blocking=True)
             r = qp.posteriors(d_seqs, d_offs, self.fam.k, s["d_pairs"][: hi - lo], self.cp, s["ws"], nnz_capacity=s["cap"],
-                              h_rows_total=self.rows[b], stream=s["stream"], check=True, reuse=s["res"])
+                              h_rows_total=self.rows[b], stream=self.comp, check=True, reuse=s["res"])
             res = s["res"]
             s["h_nb"][: hi - lo + 1].copy_(res.pair_nnz_base[: hi - lo + 1], non_blocking=True)
-            s["h_rb"][: hi - lo + 1].copy_(res.pair_row_base[: hi - lo + 1], non_blocking=True)
             s["h_status"].copy_(res.status, non_blocking=True)
+            s["sized"].record(self.comp)
+        s["stream"].wait_event(s["sized"])
+        with torch.cuda.stream(s["stream"]):
+            s["h_rb"][: hi - lo + 1].copy_(res.pair_row_base[: hi - lo + 1], non_blocking=True)
             s["h_rp"][: self.rows[b]].copy_(res.row_ptr[: self.rows[b]], non_blocking=True)
-            s["sized"].record(s["stream"])
         self.launches += r.launches
         self.h2d_bytes += 8 * (hi - lo)
 
@@ -158,8 +165,7 @@ class HostStreamer:
         up = torch.cuda.Event()
         up.record(main)
         self.h2d_bytes += self.h_seqs.numel() + 8 * self.h_offs.numel()
-        for sl in self.slots:
-            sl["stream"].wait_event(up)
+        self.comp.wait_event(up)
         if nb:
             self._enqueue(0, d_seqs, d_offs)
         for b in range(nb):
@@ -175,6 +181,7 @@ class HostStreamer:
                 break
             yield HostBatch(lo, hi, s["h_rb"][: hi - lo + 1], s["h_nb"][: hi - lo + 1], s["h_rp"][: self.rows[b]],
                             s["h_col"][:nz], s["h_val"][:nz])
+        main.wait_stream(self.comp)
         for sl in self.slots:
             main.wait_stream(sl["stream"])
         self.dist.copy_(self.d_dist, non_blocking=True)
