@@ -360,6 +360,34 @@ def test_host_call_matches_single_call(default_params):
     assert tight.code == qp.ERR["NNZ_CAPACITY"] and int(tight.pair_nnz_base[len(pairs)].item()) == nz
 
 
+def test_sharded_pair_list_on_the_gpu_matches_one_call(default_params):
+    """SURVEY.md 8(e) on one device: the three shards that multi.ShardedFamily deals to a world of 3 ranks, run one
+    after the other through qp_posteriors, give bit for bit the distances and the per-pair CSR of the unsharded call
+    (the exchange itself -- a sum of matrices with disjoint supports -- is covered by tests/test_multi_gloo.py)."""
+    qp = _qp()
+    import torch
+    from paper_1512_07437_b200 import multi
+    fam = inputs.config_family(1)
+    pairs = inputs.all_pairs(fam.k)
+    ref = qp.run_family(fam, pairs, default_params)
+    rb, nb = ref.pair_row_base.cpu().numpy(), ref.pair_nnz_base.cpu().numpy()
+    col, val = ref.col_idx.cpu().numpy(), ref.val.cpu().numpy()
+    total = torch.zeros_like(ref.dist)
+    seen = np.zeros(len(pairs), dtype=bool)
+    for rank in range(3):
+        sh = multi.ShardedFamily(fam.lengths, pairs, 3, rank)
+        part = qp.run_family(fam, sh.pairs, default_params)
+        total += sh.step(lambda _pairs: part.dist)          # no process group: the exchange is the identity
+        pnb = part.pair_nnz_base.cpu().numpy()
+        pcol, pval = part.col_idx.cpu().numpy(), part.val.cpu().numpy()
+        for q, p in enumerate(sh.mine):
+            assert not seen[p]
+            seen[p] = True
+            assert np.array_equal(pcol[pnb[q]:pnb[q + 1]], col[nb[p]:nb[p + 1]])
+            assert np.array_equal(pval[pnb[q]:pnb[q + 1]], val[nb[p]:nb[p + 1]])
+    assert seen.all() and torch.equal(total, ref.dist)
+
+
 def test_fuzz_random_pairs_models_thresholds():
     """Seeded fuzz: random lengths (1..400, incl. very skewed pairs), random symmetric models with G in {1,2} for
     either automaton, alphabets 4 / 12 / 20 / 31, thresholds 0.001 .. 0.2, both precisions."""
