@@ -66,3 +66,15 @@ def test_kernels_are_sm100a_sass(lib_path):
     import subprocess
     out = subprocess.run(["cuobjdump", "-lelf", lib_path], capture_output=True, text=True).stdout
     assert "sm_100a" in out
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/qp.h is a C header: it compiles with a C99 compiler, no C++ and no CUDA types in the signatures."""
+    import subprocess
+    src = tmp_path / "t.c"
+    src.write_text('#include "qp.h"\nint main(void) { qp_params p; qp_output o; qp_host_output h; qp_csr c; qp_csr_out co;\n'
+                   'qp_consistency_params cp; qp_peaks pk; (void)p; (void)o; (void)h; (void)c; (void)co; (void)cp; (void)pk;\n'
+                   'return QP_OK; }\n')
+    r = subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-I" + os.path.join(ROOT, "include"), "-c",
+                        str(src), "-o", str(tmp_path / "t.o")], capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
