@@ -285,8 +285,9 @@ def roofline_of(cfg, m, clocks, dev=None):
     return {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
             "traffic": ncu_traffic(cfg), "peak_source": peak_src,
             "frac_note": "whole step (schedule + pair kernels + fp64 distance queues + CSR placement) over the HBM peak",
-            "kernel": "qp::pair_kernel<float,GP,C,MODE,W>: the 18 class instances of one call (packed C=2..16, split "
-                      "C8/C12/C16 x W4), launched on side streams; duration = fork..join on the caller's stream",
+            "kernel": "qp::pair_kernel<float,GP,C,MODE,W>: the 22 class instances of one call (packed C=2..16, split "
+                      "C8/C12/C16 x W4, packed two-block C=9..12), launched on side streams; duration = fork..join on the "
+                      "caller's stream",
             "kernel_ms": prof["pair_kernels"], "kernel_achieved": kernel_achieved, "kernel_frac": kernel_achieved / hbm_peak,
             "traffic_note": "dram read+write bytes of those launches from ncu (profiles/traffic.csv), per step",
             "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,

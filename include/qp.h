@@ -283,9 +283,10 @@ int qp_last_launch_count(void);
 void qp_set_profile(int on);
 int qp_get_profile(float ms[4]);
 /* Per scheduling class c (0..14: packed, one warp per pair, stripe width C = c+2; 15..17: split, the warps of a
- * CTA share one long pair): start and stop of its pair kernel in ms after the end of the schedule phase, -1 for
- * classes that did not run. Same preconditions as qp_get_profile. */
-#define QP_NUM_CLASSES 18
+ * CTA share one long pair; 18..21: packed two-block, one warp per pair of 513..768 columns, C = c-18+9): start and
+ * stop of its pair kernel in ms after the end of the schedule phase, -1 for classes that did not run. Same
+ * preconditions as qp_get_profile. */
+#define QP_NUM_CLASSES 22
 int qp_get_profile_classes(float start_ms[QP_NUM_CLASSES], float stop_ms[QP_NUM_CLASSES]);
 
 /*

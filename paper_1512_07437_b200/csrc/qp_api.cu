@@ -40,6 +40,12 @@ QP_DECL_F64_G1(2, kModeDist, 8) QP_DECL_F64_G1(4, kModeDist, 8) QP_DECL_F64_G1(8
 QP_DECL_F32(2, 1) QP_DECL_F32(3, 1) QP_DECL_F32(4, 1) QP_DECL_F32(5, 1) QP_DECL_F32(6, 1) QP_DECL_F32(7, 1) QP_DECL_F32(8, 1)
 QP_DECL_F32(9, 1) QP_DECL_F32(10, 1) QP_DECL_F32(11, 1) QP_DECL_F32(12, 1) QP_DECL_F32(13, 1) QP_DECL_F32(14, 1)
 QP_DECL_F32(15, 1) QP_DECL_F32(16, 1) QP_DECL_F32(8, 4) QP_DECL_F32(12, 4) QP_DECL_F32(16, 4)
+#define QP_DECL_F32_MB(C)                                                                                              \
+    extern template cudaError_t launch_pair<float, 1, C, kModeCsr | kModeMB, 1>(const KArgs<float>&, int, cudaStream_t);  \
+    extern template cudaError_t launch_pair<float, 2, C, kModeCsr | kModeMB, 1>(const KArgs<float>&, int, cudaStream_t);  \
+    extern template cudaError_t launch_pair<float, 1, C, kModeFull | kModeMB, 1>(const KArgs<float>&, int, cudaStream_t); \
+    extern template cudaError_t launch_pair<float, 2, C, kModeFull | kModeMB, 1>(const KArgs<float>&, int, cudaStream_t);
+QP_DECL_F32_MB(9) QP_DECL_F32_MB(10) QP_DECL_F32_MB(11) QP_DECL_F32_MB(12)
 QP_DECL_F64(2, kModeFull, 1) QP_DECL_F64(4, kModeFull, 1) QP_DECL_F64(6, kModeFull, 1) QP_DECL_F64(8, kModeFull, 1)
 QP_DECL_F64(8, kModeFull, 8) QP_DECL_F64(2, kModeDist, 8) QP_DECL_F64(4, kModeDist, 8) QP_DECL_F64(8, kModeDist, 8)
 
@@ -226,7 +232,7 @@ __global__ void k_refine_plan(int which, MaxW64 maxw, int64_t avail, SchedHeader
     RefineQ& rq = h->rq;
     if (which == 0) {
         unsigned long long room = (unsigned long long)avail / 2, used = 0;
-        for (int c = kNumPacked; c < kNumClasses; ++c) {   // slot sizes grow with the class index
+        for (int c = kNumPacked; c < kSplitEnd; ++c) {   // slot sizes grow with the class index
             const unsigned long long sb = (rq.poll_slot_bytes[c] + 255ull) & ~255ull;
             rq.poll_slot_bytes[c] = sb;
             int W = 0;
@@ -284,7 +290,7 @@ static thread_local bool g_tau_hist_valid = false;
 
 // Per host thread and device: side streams so that the per-class kernels overlap their tails, the events that fork
 // and join them, and the profiling events. Created on the first call on a device, kept until qp_shutdown().
-constexpr int kNumRefine = kNumClasses - kNumPacked;          // split fp64 classes of the re-evaluation queues
+constexpr int kNumRefine = kSplitEnd - kNumPacked;            // split fp64 classes of the re-evaluation queues
 constexpr int kNumStreams = kNumClasses + kNumRefine + 1;     // fp32 / QP_FP64 classes | early fp64 queue | CSR placement
 struct Ctx {
     bool ok = false;
@@ -477,6 +483,13 @@ static int launch_class_f32(int gp, bool full, int cls, const KArgs<float>& ka, 
         QP_CASE(0, 2, 1) QP_CASE(1, 3, 1) QP_CASE(2, 4, 1) QP_CASE(3, 5, 1) QP_CASE(4, 6, 1) QP_CASE(5, 7, 1)
         QP_CASE(6, 8, 1) QP_CASE(7, 9, 1) QP_CASE(8, 10, 1) QP_CASE(9, 11, 1) QP_CASE(10, 12, 1) QP_CASE(11, 13, 1)
         QP_CASE(12, 14, 1) QP_CASE(13, 15, 1) QP_CASE(14, 16, 1) QP_CASE(15, 8, 4) QP_CASE(16, 12, 4) QP_CASE(17, 16, 4)
+#define QP_CASE_MB(CLS, C)                                                                                          \
+    case CLS:                                                                                                       \
+        if (full) e = gp == 1 ? launch_pair<float, 1, C, kModeFull | kModeMB, 1>(ka, grid, st) : launch_pair<float, 2, C, kModeFull | kModeMB, 1>(ka, grid, st); \
+        else e = gp == 1 ? launch_pair<float, 1, C, kModeCsr | kModeMB, 1>(ka, grid, st) : launch_pair<float, 2, C, kModeCsr | kModeMB, 1>(ka, grid, st);        \
+        break;
+        QP_CASE_MB(18, 9) QP_CASE_MB(19, 10) QP_CASE_MB(20, 11) QP_CASE_MB(21, 12)
+#undef QP_CASE_MB
     }
 #undef QP_CASE
     ++g_launches;
@@ -761,7 +774,14 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     prof_mark(cx, 1, st);
     QP_TRY(cudaEventRecord(cx->fork, st));
     forked = true;
-    for (int c = kNumClasses - 1; c >= 0; --c) {   // split classes (long pairs) and wide stripes first
+    // launch order: the split classes (the longest pairs: they set the tail) first, then the two-block classes, then
+    // the one-block classes from wide to narrow
+    int launch_order[kNumClasses], nl = 0;
+    for (int c = kSplitEnd - 1; c >= kNumPacked; --c) launch_order[nl++] = c;
+    for (int c = kNumClasses - 1; c >= kSplitEnd; --c) launch_order[nl++] = c;
+    for (int c = kNumPacked - 1; c >= 0; --c) launch_order[nl++] = c;
+    for (int q = 0; q < nl; ++q) {
+        const int c = launch_order[q];
         if (!((cmask >> c) & 1)) continue;
         QP_TRY(cudaStreamWaitEvent(cx->st[c], cx->fork, 0));
         const int grid = class_grid(c, fp64, sms);
@@ -775,7 +795,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     }
     if (pollers) {   // pollers of the fp64 re-evaluation queue, behind the fp32 classes: they fill the room those leave
         ka64->refine_pass = 1;
-        for (int c = kNumClasses - 1; c >= kNumPacked; --c) {
+        for (int c = kSplitEnd - 1; c >= kNumPacked; --c) {
             cudaStream_t es = cx->st[kNumClasses + (c - kNumPacked)];
             QP_TRY(cudaStreamWaitEvent(es, cx->fork, 0));
             r = launch_class_f64(true, params->pf.n_ins, c, *ka64, kPollCtas, es);
@@ -791,7 +811,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
         ++g_launches;
         QP_TRY(cudaEventRecord(cx->fork2, st));
         ka64->refine_pass = 2;
-        for (int c = kNumPacked; c < kNumClasses; ++c) {
+        for (int c = kNumPacked; c < kSplitEnd; ++c) {
             QP_TRY(cudaStreamWaitEvent(cx->st[c], cx->fork2, 0));
             r = launch_class_f64(true, params->pf.n_ins, c, *ka64, class_grid(c, true, sms), cx->st[c]);
             if (r) return fail(r);
@@ -810,7 +830,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     if (refine) {
         QP_TRY(cudaEventRecord(cx->join[kNumStreams - 1], ps));
         QP_TRY(cudaStreamWaitEvent(st, cx->join[kNumStreams - 1], 0));
-        for (int c = kNumPacked; c < kNumClasses; ++c) {
+        for (int c = kNumPacked; c < kSplitEnd; ++c) {
             QP_TRY(cudaStreamWaitEvent(st, cx->join[c], 0));                                               // drainers
             if (pollers) QP_TRY(cudaStreamWaitEvent(st, cx->join[kNumClasses + (c - kNumPacked)], 0));     // pollers
         }

@@ -19,22 +19,30 @@ namespace qp {
 // pipelined anti-diagonal wavefront, block boundaries handed over through shared memory (qp_pair.cuh).
 //   class 0..14  : packed, C = c + 2 = 2..16                (fp64: only C = 2, 4, 6, 8 exist)
 //   class 15..17 : split,  fp32 (C, W) = (8,4) (12,4) (16,4);  fp64 (C, W) = (2,8) (4,8) (8,8)
-constexpr int kNumClasses = 18;
-constexpr int kNumPacked = 15;
+//   class 18..21 : packed TWO-BLOCK, fp32 only, C = c - 18 + 9 = 9..12: a pair of 513..768 columns and moderate size
+//                  on ONE warp, which runs its two 32*C-column blocks one after the other (the boundary column goes
+//                  through the scratch slot). Separate kernel instances (MODE | kModeMB): a run-time block count in
+//                  the one-block kernels costs them registers they do not have (measured: 5-9 % slower).
+constexpr int kNumClasses = 22;
+constexpr int kNumPacked = 15;        // classes below: packed one-block
+constexpr int kSplitEnd = 18;         // classes kNumPacked .. kSplitEnd-1: split; from kSplitEnd on: packed two-block
+constexpr int kModeMB = 4;            // MODE bit of the two-block instances (qp_pair.cuh)
 constexpr int kWarpsPerCta = 4;       // packed classes
 constexpr int kNumBins = 384;         // size bins: 8 per octave of scratch bytes
 constexpr int kSmAssumed = 148;       // used by the host-only workspace query when no device is visible
 
 QP_HD2 int class_C(int c, bool fp64) {
     if (c < kNumPacked) return (fp64 && (c > 6 || (c & 1))) ? 0 : c + 2;
+    if (c >= kSplitEnd) return fp64 ? 0 : c - kSplitEnd + 9;
     return fp64 ? (c == 15 ? 2 : (c == 16 ? 4 : 8)) : (c == 15 ? 8 : (c == 16 ? 12 : 16));
 }
-QP_HD2 int class_W(int c, bool fp64) { return c < kNumPacked ? 1 : (fp64 ? 8 : 4); }
-QP_HD2 int class_index(int C, int W, bool fp64) {
+QP_HD2 int class_W(int c, bool fp64) { return (c < kNumPacked || c >= kSplitEnd) ? 1 : (fp64 ? 8 : 4); }
+QP_HD2 int class_index(int C, int W, bool fp64, bool two_block) {
+    if (two_block) return kSplitEnd + C - 9;
     if (W == 1) return C - 2;
     return fp64 ? (C == 2 ? 15 : (C == 4 ? 16 : 17)) : (C == 8 ? 15 : (C == 12 ? 16 : 17));
 }
-constexpr uint32_t kMaskF32 = 0x3ffff;     // fp32 pass: packed C = 2..16 and the three split classes
+constexpr uint32_t kMaskF32 = 0x3fffff;    // fp32 pass: packed C = 2..16, the three split classes, two-block C = 9..12
 constexpr uint32_t kMaskF64 = 0x20055;     // QP_FP64: packed C = 2, 4, 6, 8, split (8,8)
 constexpr uint32_t kMaskRefine = 0x38000;  // fp64 distance re-evaluation: split classes only (latency matters)
 
@@ -82,10 +90,14 @@ QP_HD2 int64_t slot_bytes(int n, int C, int nb, int real_bytes) {
 
 // choose the class of a pair with n rows and `cols` = m+1 columns among the classes of `mask`:
 //   1. the narrowest packed class whose single block holds all columns (least padding, one warp per pair);
-//   2. else the split class with the shortest pipeline: passes * (rows + 32 * active warps) * (C + per-step overhead
+//   2. else, for pairs of moderate size, the narrowest two-block class that holds the columns: one warp per pair keeps
+//      the efficiency of the packed classes (no idle warp, no ring hand-off: a packed class alone moves 4.8 TB/s of
+//      DRAM traffic, the 4-warp split class for 513..768 columns 2.0); the size limit keeps the time a single warp
+//      spends on one pair (~8 ns per cell) well below the time of a call that contains such pairs;
+//   3. else the split class with the shortest pipeline: passes * (rows + 32 * active warps) * (C + per-step overhead
 //      expressed in cells), a pass = W neighbouring blocks;
-// Returns the class index (-1 if the mask holds no class that can take the pair: packed classes never take more than
-// one block) and the number of 32*C-column blocks.
+// Returns the class index (-1 if the mask holds no class that can take the pair) and the number of 32*C-column blocks.
+constexpr int64_t kTwoBlockMaxCells = 400000;
 QP_HD2 int choose_class(int n, int cols, uint32_t mask, bool fp64, int* nb_out) {
     constexpr int kStepOverhead = 6;
     int best = -1, best_nb = 0;
@@ -98,7 +110,16 @@ QP_HD2 int choose_class(int n, int cols, uint32_t mask, bool fp64, int* nb_out) 
             return c;
         }
     }
-    for (int c = kNumPacked; c < kNumClasses; ++c) {
+    if ((int64_t)n * cols <= kTwoBlockMaxCells)
+        for (int c = kSplitEnd; c < kNumClasses; ++c) {
+            const int C = class_C(c, fp64);
+            if (!((mask >> c) & 1) || C == 0) continue;
+            if (cols <= 64 * C) {
+                *nb_out = 2;
+                return c;
+            }
+        }
+    for (int c = kNumPacked; c < kSplitEnd; ++c) {
         if (!((mask >> c) & 1)) continue;
         const int C = class_C(c, fp64), W = class_W(c, fp64);
         const int nb = (cols + 32 * C - 1) / (32 * C);

@@ -51,10 +51,10 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
     }
     fence_proxy_async();   // ring zeroing (generic proxy) before the first bulk copy lands in it
     __syncthreads();
-    constexpr int cls = class_index(C, W, sizeof(R) == 8);
+    constexpr int cls = class_index(C, W, sizeof(R) == 8, (MODE & kModeMB) != 0);
     const int unit = W == 1 ? blockIdx.x * kWarpsPerCta + warp : blockIdx.x;   // who owns a scratch slot
     SchedHeader* hdr = ka.hdr;
-    if constexpr (MODE == kModeDist) {
+    if constexpr ((MODE & 3) == kModeDist) {
         // consumer of the fp64 re-evaluation queue (split classes only): pull list positions through the class cursor;
         // a poller waits for its position to be filled until every fp32 class CTA has exited
         static_assert(W > 1, "the distance-only kernels are split-class kernels");

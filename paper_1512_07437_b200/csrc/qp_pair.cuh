@@ -20,7 +20,7 @@
 
 namespace qp {
 
-enum : int { kModeCsr = 0, kModeFull = 1, kModeDist = 2 };
+enum : int { kModeCsr = 0, kModeFull = 1, kModeDist = 2 };   // | kModeMB (qp_internal.h): the two-block packed instances
 
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -270,13 +270,15 @@ __device__ __forceinline__ int32_t ld_acquire_gpu(const int32_t* p) {
 // ---------------------------------------------------------------------------------------------------------
 // the pair pipeline
 // ---------------------------------------------------------------------------------------------------------
-template <typename R, int GP, int C, int MODE, int W>
+template <typename R, int GP, int C, int MODEX, int W>
 __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared address of the emission table*/, int p,
                              char* slot, int lane, int warp, FRing& ring, CoopShared<R, GP, W>* cs,
                              uint32_t* hist_s /*this warp's threshold histogram in shared memory*/) {
     using V2 = typename Traits<R>::vec2;
     using Acc = typename Traits<R>::acc_t;
     using SL = Slot<R>;
+    constexpr int MODE = MODEX & 3;                  // what is written
+    constexpr bool kMB = (MODEX & kModeMB) != 0;     // packed class whose pairs have two column blocks
     constexpr int RB = (int)sizeof(R);
     constexpr int GH = 2;
     constexpr bool kCsr = MODE != kModeDist;
@@ -286,8 +288,8 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
 
     const PairInfo pi = ka.info[p];
     const int n = pi.n, m = pi.m;
-    // column blocks (column 0 included); a packed class only takes pairs that fit one block (choose_class)
-    const int nb = kSplit ? (m + 1 + 32 * C - 1) / (32 * C) : 1;
+    // column blocks (column 0 included); a one-block packed class only takes pairs that fit one block (choose_class)
+    const int nb = (kSplit || kMB) ? (m + 1 + 32 * C - 1) / (32 * C) : 1;
     constexpr int kEm = (int)sizeof(V2);
     const uint8_t* __restrict__ xs = ka.seqs + pi.xoff;
     const uint8_t* __restrict__ ys = ka.seqs + pi.yoff;
@@ -341,9 +343,9 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             const int i = t - lane;
             const bool active = (unsigned)i <= (unsigned)n;
             // warp-uniform (FwdModel::prepare): lanes enter their first row while t < 32; scales change on the
-            // renormalisation step and the step after it; lane 0 of a later block of a split pair loses its input
+            // renormalisation step and the step after it; lane 0 of a later block of a multi-block pair loses its input
             // once it is past row n
-            const bool recompute = (t & mask) <= 1 || (kSplit && b > 0 && t > n);
+            const bool recompute = (t & mask) <= 1 || ((kSplit || kMB) && b > 0 && t > n);
             const bool prep = recompute || t < 32;
             FwdEx<R, GH> rh = shfl_up_ex(FB.exh());
             FwdEx<R, GP> rp = shfl_up_ex(FB.exp());
@@ -572,8 +574,8 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             if (enext) eFn = *(const int2*)(lp - stride + dE);
             // warp-uniform (FwdModel::prepare): lanes enter their first row (row n) while t >= n; scales change on the
             // renormalisation step and the step after it (that is also where the recorded forward exponents change);
-            // lane 31 of an earlier block of a split pair loses its input once it is past row 0
-            const bool recompute = (t & mask) >= mask - 1 || (kSplit && !last && t < 32);
+            // lane 31 of an earlier block of a multi-block pair loses its input once it is past row 0
+            const bool recompute = (t & mask) >= mask - 1 || ((kSplit || kMB) && !last && t < 32);
             const bool prep = recompute || t >= n;
             BwdEx<R, GH> rh = shfl_dn_ex(BB.exh());
             BwdEx<R, GP> rp = shfl_dn_ex(BB.exp());
@@ -844,7 +846,39 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
         int32_t* rp = ka.row_ptr + ka.pair_row_base[p];
         float2* pool = ka.pool + poff;   // (value, column bits) per entry: one 8-byte store each
         const int32_t* rowcnt = (const int32_t*)(slot + rowcnt_offset(n, C, nb, RB));
-        // one block per pair here (packed class). Software pipeline over the 32-row chunks: the row counts are
+        if constexpr (kMB) {
+            // two blocks (packed class, wide pair): plain walk, rows 32 at a time, blocks in ascending order
+            int running = 0;
+            for (int i0 = 1; i0 <= n; i0 += 32) {
+                const int i = i0 + lane;
+                const bool valid = i <= n;
+                int c = 0;
+                for (int b = 0; b < nb; ++b) c += valid ? __ldcg(rowcnt + (int64_t)b * (n + 1) + i) : 0;
+                const int ex = warp_excl_scan(c, lane);
+                int d = running + ex;
+                if (valid) rp[i - 1] = d;
+                running += __shfl_sync(kFull, ex + c, 31);
+                if (ok && valid)
+                    for (int b = 0; b < nb; ++b) {
+                        const int cb = __ldcg(rowcnt + (int64_t)b * (n + 1) + i);
+                        const char* buf = slot + (int64_t)b * blk_bytes + (int64_t)(i + 32) * stride;
+                        for (int g = (cb - 1) >> 2; g >= 0; --g) {
+                            const float4 lo = ld_cg_f4(buf + g * 32), hi = ld_cg_f4(buf + g * 32 + 16);
+                            const int q = 4 * g;
+                            if (q + 3 < cb) { pool[d] = make_float2(hi.z, hi.w); ++d; }
+                            if (q + 2 < cb) { pool[d] = make_float2(hi.x, hi.y); ++d; }
+                            if (q + 1 < cb) { pool[d] = make_float2(lo.z, lo.w); ++d; }
+                            pool[d] = make_float2(lo.x, lo.y); ++d;
+                        }
+                    }
+            }
+            if (lane == 0) {
+                rp[n] = running;
+                ka.nnz[p] = nnz;
+                ka.pool_off[p] = (int64_t)poff;
+            }
+        } else {
+        // one block per pair. Software pipeline over the 32-row chunks: the row counts are
         // fetched two chunks ahead and a row's first entry group one chunk ahead, so that a chunk starts with its
         // loads already landed instead of paying two dependent L2 round trips.
         auto cnt_at = [&](int i) -> int { return i <= n ? __ldcg(rowcnt + i) : 0; };
@@ -895,6 +929,7 @@ __device__ void process_pair(const KArgs<R>& ka, const uint32_t tab /*shared add
             rp[n] = running;
             ka.nnz[p] = nnz;
             ka.pool_off[p] = (int64_t)poff;
+        }
         }
     }
 

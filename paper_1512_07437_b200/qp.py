@@ -20,7 +20,7 @@ ERR = {"INVALID_ARG": -1, "BAD_RESIDUE": -2, "EMPTY_SEQUENCE": -3, "BAD_PAIR": -
        "NNZ_CAPACITY": -6, "CUDA": -7, "RANGE": -8}
 QP_FP32, QP_FP64 = 0, 1
 FLAG_SYNC_STATUS, FLAG_NO_REFINE, FLAG_NO_POLLERS = 1, 2, 4
-NUM_CLASSES = 18
+NUM_CLASSES = 22
 
 EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_posteriors_budgeted", "qp_guide_tree", "qp_guide_tree_workspace_bytes", "qp_last_launch_count", "qp_status_string", "qp_version",
            "qp_set_profile", "qp_get_profile", "qp_get_profile_classes", "qp_shutdown",
@@ -169,12 +169,13 @@ def get_profile():
 
 def get_profile_classes():
     """[(class, start_ms, stop_ms)] of the class kernels of the last profiled call (relative to the fork);
-    class = "C<stripe width>" for packed classes, "C<stripe width>xW<warps>" for split ones (fp32 naming)."""
+    class = "C<stripe width>" for packed classes, "C<stripe width>xW<warps>" for split ones, "C<stripe width>x2" for
+    the packed two-block ones (fp32 naming)."""
     a, b = (C.c_float * NUM_CLASSES)(), (C.c_float * NUM_CLASSES)()
     r = _lib.qp_get_profile_classes(a, b)
     if r != QP_OK:
         raise QpError(r)
-    names = ["C%d" % (c + 2) for c in range(15)] + ["C8xW4", "C12xW4", "C16xW4"]
+    names = ["C%d" % (c + 2) for c in range(15)] + ["C8xW4", "C12xW4", "C16xW4"] + ["C%dx2" % C for C in range(9, 13)]
     return [(names[c], round(a[c], 3), round(b[c], 3)) for c in range(NUM_CLASSES) if a[c] >= 0]
 
 

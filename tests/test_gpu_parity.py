@@ -109,7 +109,8 @@ def test_long_skewed_pairs_split_classes(default_params, precision):
     fam = inputs.pack([base, mut[100:800], rng.integers(0, 20, size=20).astype(np.uint8),
                        rng.integers(0, 20, size=1500).astype(np.uint8), rng.choice(20, size=2500, p=q).astype(np.uint8),
                        rng.choice(20, size=45, p=q).astype(np.uint8)])
-    pairs = np.array([[0, 1], [1, 0], [2, 3], [3, 2], [0, 3], [2, 1], [5, 4], [4, 5], [1, 4]], dtype=np.int32)
+    # [3, 1] and [3, 0]: 1500 rows x 701 / 901 columns, too many cells for the two-block packed classes -> split C = 8
+    pairs = np.array([[0, 1], [1, 0], [2, 3], [3, 2], [0, 3], [2, 1], [5, 4], [4, 5], [1, 4], [3, 1], [3, 0]], dtype=np.int32)
     run = orc.Run(default_params, fam, pairs, keep_dense=True)
     res = qp.run_family(fam, pairs, default_params, precision=precision, want_dense=True, want_logZ=True)
     tol = dict(p_atol=1e-7, d_rtol=1e-6, logz_rtol=1e-11) if precision == "fp64" else {}
@@ -210,6 +211,33 @@ def test_g2_partition_function_production_instances_packed(default_params):
     run = orc.Run(prm, fam, pairs, keep_dense=True)
     res = qp.run_family(fam, pairs, prm, precision="fp32")
     _compare(fam, pairs, prm, res, run, dense=False, logZ=False)
+
+
+@pytest.mark.parametrize("g2", [False, True])
+def test_two_block_packed_classes(default_params, g2):
+    """launch_pair<float,GP,C,MODE|kModeMB,1>, C = 9..12: pairs of 513..768 columns and moderate size on ONE warp that
+    runs the two column blocks one after the other. One column count per stripe width (64 C - 20 and the smallest that
+    needs the class), both orientations of the block boundary exercised by related sequences; with the test outputs
+    (kModeFull) and as the production instances (kModeCsr); GP = 1 and GP = 2."""
+    qp = _qp()
+    rng = np.random.default_rng(13)
+    q = inputs.background()
+    prm = inputs.Params(hmm=default_params.hmm, pf=_pf_two_gap_states() if g2 else default_params.pf, threshold=0.01)
+    root = rng.choice(20, size=1010, p=q).astype(np.uint8)
+    seqs = [root[:300].copy(), root[350:610].copy()]
+    for C in range(9, 13):
+        for L in (64 * C - 20, 64 * (C - 1) + 1 if C > 9 else 513):
+            s = root[:L].copy()
+            hit = rng.random(L) < 0.3
+            s[hit] = rng.choice(20, size=int(hit.sum()), p=q)
+            seqs.append(s)
+    fam = inputs.pack(seqs)
+    pairs = np.array([[j % 2, 2 + j] for j in range(8)], dtype=np.int32)
+    run = orc.Run(prm, fam, pairs, keep_dense=True)
+    full = qp.run_family(fam, pairs, prm, precision="fp32", want_dense=True, want_logZ=True)
+    _compare(fam, pairs, prm, full, run)
+    prod = qp.run_family(fam, pairs, prm, precision="fp32")
+    _compare(fam, pairs, prm, prod, run, dense=False, logZ=False)
 
 
 def test_nucleotide_mode_alphabet_4():
