@@ -136,7 +136,7 @@ def workload_name(cfg, fam, pairs):
 
 
 # warp instructions per cell of the pair kernels, everything included (ramp steps, padding columns, per-step and
-# per-pair code, CSR emission): smsp__inst_executed.sum of the 18 fp32 class kernels of one configs[2] step / its cells =
+# per-pair code, CSR emission): smsp__inst_executed.sum of the 22 fp32 class kernels of one configs[2] step / its cells =
 # 5.51e9 / 1.824e9 (profiles/r02_ncu_full_cfg2.md; the hot loop alone: 2.52, profiles/r01_hotloop_c10.md). The issue
 # bound of the kernels is this count x cells / the measured warp-instruction issue rate (qp_measure_peaks)
 WARP_INSTR_PER_CELL = 3.02
