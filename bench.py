@@ -176,7 +176,7 @@ def measure(cfg, steps, warmup, dev, prm, rank=0, world=1, shard=False, sample_c
     d_seqs = torch.from_numpy(np.ascontiguousarray(fam.seqs)).to(dev)
     d_offs = torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev)
     d_pairs = torch.from_numpy(pairs).to(dev)
-    cp_async = qp.CParams(prm, flags=0)
+    cp_async = qp.CParams(prm, flags=QP_FLAGS)
     cap = int(0.05 * my_cells) + 4096
     dist = torch.zeros((fam.k, fam.k), dtype=torch.float32, device=dev)
 
@@ -258,6 +258,7 @@ def measure(cfg, steps, warmup, dev, prm, rank=0, world=1, shard=False, sample_c
 
 
 _ALU = {}
+QP_FLAGS = 0   # --qp-flags
 
 
 def alu_peaks(dev):
@@ -488,9 +489,13 @@ def main():
     ap.add_argument("--no-configs", action="store_true", help="skip the configs[2] / configs[4] block of the default run")
     ap.add_argument("--stage3", type=int, default=None, metavar="CFG",
                     help="only the stage II + III measurement (qp_guide_tree + qp_consistency) on configs[CFG]; prints its block")
+    ap.add_argument("--qp-flags", type=int, default=0,
+                    help="extra qp_params.flags of the device-timed calls, for A/B runs (4 = QP_FLAG_NO_POLLERS, 2 = QP_FLAG_NO_REFINE)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()
+    global QP_FLAGS
+    QP_FLAGS = args.qp_flags
     if args.stage3 is not None:
         import torch
         from paper_1512_07437_b200 import inputs
