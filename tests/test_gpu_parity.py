@@ -489,3 +489,48 @@ def test_memory_limited_mode_raises_threshold(default_params):
     # one pass is not enough: the capacity error comes back with the threshold that was tried last
     r1 = qp.posteriors(*args, budget_passes=1, check=False, **kw)
     assert r1.code == qp.ERR["NNZ_CAPACITY"] and r1.passes == 1 and int(r1.pair_nnz_base[-1].item()) == nnz_full
+
+
+def test_call_can_be_captured_into_a_cuda_graph(default_params):
+    """qp_posteriors only enqueues work (flags = 0: no host synchronisation, no allocation): the whole call, side streams
+    included, can be captured into a CUDA graph and replayed; the replay writes bit for bit what the plain call wrote."""
+    import torch
+    qp = _qp()
+    dev = torch.device("cuda:0")
+    fam = inputs.config_family(0)
+    pairs = inputs.all_pairs(fam.k)
+    L = fam.lengths
+    n, m = L[pairs[:, 0]].astype(np.int64), L[pairs[:, 1]].astype(np.int64)
+    cells, rows = int((n * m).sum()), int((n + 1).sum())
+    d_seqs = torch.from_numpy(np.ascontiguousarray(fam.seqs)).to(dev)
+    d_offs = torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev)
+    d_pairs = torch.from_numpy(pairs).to(dev)
+    cp = qp.CParams(default_params, flags=0)
+    cap = int(0.2 * cells) + 1024
+    ws = torch.empty(qp.workspace_bytes(fam.offsets, fam.k, pairs, cp, cap), dtype=torch.uint8, device=dev)
+    kw = dict(nnz_capacity=cap, h_rows_total=rows, check=False)
+    ref = qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp, ws, **kw)
+    torch.cuda.synchronize()
+    assert int(ref.status[0].item()) == 0
+    want = [t.clone() for t in (ref.dist, ref.pair_nnz_base, ref.row_ptr, ref.col_idx, ref.val)]
+    out = qp.alloc_outputs(dev, len(pairs), rows, cap, fam.k)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):   # warm-up on the capture stream (creates the library's side streams before the capture)
+        qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp, ws, reuse=out, stream=s, **kw)
+    torch.cuda.current_stream().wait_stream(s)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=s):
+        qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp, ws, reuse=out, stream=s, **kw)
+    for _ in range(2):
+        for t in (out.dist, out.val, out.col_idx, out.row_ptr, out.pair_nnz_base, out.status):
+            t.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert out.status.tolist()[0] == 0 and out.status.tolist()[3] == int(ref.status[3].item())
+        nnz = int(want[1][-1].item())
+        got = (out.dist, out.pair_nnz_base, out.row_ptr, out.col_idx, out.val)
+        for a, b, name in zip(got, want, ("dist", "pair_nnz_base", "row_ptr", "col_idx", "val")):
+            k = nnz if name in ("col_idx", "val") else b.numel()
+            assert torch.equal(a[:k] if a.dim() == 1 else a, b[:k] if b.dim() == 1 else b), name
