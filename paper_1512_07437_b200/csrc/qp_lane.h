@@ -429,13 +429,16 @@ template <typename R, int G, int C> struct BwdModel {
 // ---------------------------------------------------------------------------------------------------------
 // combine + MEA quantisation
 // ---------------------------------------------------------------------------------------------------------
-// P_model * sqrt(1/2) = (F*B) * c with c = 2^(eF+eB-eZ) * sqrt(1/2)/Zm. The product F*B of two mantissas cannot
-// overflow (each stays below 2^57 between renormalisations) and 0 * c is 0, so no NaN can arise. It can underflow
-// before it is scaled back only if E is large and positive; a probability never needs that (maxF*maxB <= Z/r with
-// r the smallest ratio of B inside one lane stripe), so E > kMaxE is reported as a range
-// error by the caller instead of being computed inexactly.
+// P_model * sqrt(1/2) = (F*B) * c with c = 2^E * sqrt(1/2)/Zm, E = eF + eB - eZ. The product F*B of two mantissas
+// cannot overflow (each stays below 2^57 between renormalisations) and 0 * c is 0, so no NaN can arise. A large positive
+// E means that every cell of the lane's stripe has a tiny F*B (F peaks at one end of the stripe, B at the other: long
+// gaps through a wide stripe, e.g. 1029 x 489 unrelated residues in the C = 16 class). F*B = P * Zm * 2^-E is still a
+// normal number of full precision while P >= 2^(E - 126) (fp32) and flushes to zero below, so up to kMaxE = 96 every
+// posterior above 2^-30 is exact and the rest is zero to working precision; beyond kMaxE the caller reports a range
+// error instead of computing inexactly. (Round 1 had kMaxE = 64 for fp32: a random-model fuzz with rows >> columns
+// tripped it on posteriors that are perfectly representable.)
 template <typename R> struct PScale {
-    static constexpr int kMaxE = sizeof(R) == 4 ? 64 : 512;
+    static constexpr int kMaxE = sizeof(R) == 4 ? 96 : 512;
     R c;
     QP_HD bool set(int E, R invZr) {
         const bool bad = E > kMaxE;

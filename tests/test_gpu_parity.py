@@ -534,3 +534,27 @@ def test_call_can_be_captured_into_a_cuda_graph(default_params):
         for a, b, name in zip(got, want, ("dist", "pair_nnz_base", "row_ptr", "col_idx", "val")):
             k = nnz if name in ("col_idx", "val") else b.numel()
             assert torch.equal(a[:k] if a.dim() == 1 else a, b[:k] if b.dim() == 1 else b), name
+
+
+def test_rows_much_longer_than_columns_in_a_wide_stripe(default_params):
+    """Unrelated sequences of 1029 / 1285 rows against 489 columns (class C = 16) under a random two-insert-state model:
+    the path has to cross every 16-column stripe through long gaps, F peaks at one end of a stripe and B at the other,
+    and the posterior scale exponent of qp_lane.h (PScale) reaches 65..96. Round 1 reported QP_ERR_RANGE here although
+    every posterior is representable; now the call succeeds and matches the oracle in both precisions."""
+    qp = _qp()
+    rng = np.random.default_rng(6)
+    A = int(rng.choice([4, 12, 20, 31]))
+    gh, gp = int(rng.integers(1, 3)), int(rng.integers(1, 3))
+    prm = inputs.Params(hmm=inputs.random_model(rng, gh, A), pf=inputs.random_model(rng, gp, A),
+                        threshold=float(rng.choice([0.001, 0.01, 0.05, 0.2])))
+    lens = [int(v) for v in rng.integers(1, 1300, size=7)] + [1, 2, 33]
+    assert (A, gh, gp) == (12, 2, 2) and lens[2] == 489 and lens[3] == 1029 and lens[6] == 1285
+    fam = inputs.pack([rng.integers(0, A, size=n).astype(np.uint8) for n in lens])
+    pairs = np.array([[3, 2], [6, 2], [2, 3], [2, 6]], dtype=np.int32)
+    run = orc.Run(prm, fam, pairs, keep_dense=True)
+    for precision in ("fp32", "fp64"):
+        res = qp.run_family(fam, pairs, prm, precision=precision, want_dense=True, want_logZ=True)
+        tol = dict(p_atol=1e-7, d_rtol=1e-6, logz_rtol=1e-11) if precision == "fp64" else dict(logz_rtol=5e-6)
+        _compare(fam, pairs, prm, res, run, **tol)
+    res = qp.run_family(fam, pairs, prm)   # production instances
+    _compare(fam, pairs, prm, res, run, dense=False, logZ=False)
