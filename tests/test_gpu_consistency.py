@@ -273,3 +273,51 @@ def test_error_paths_and_empty_input(default_params):
     none = np.zeros((0, 2), np.int32)
     r0 = qp.consistency(d_offs, fam.k, torch.from_numpy(none).to(dev), csr, d_td, **dict(kw, h_pairs=none, nnz=0))
     assert r0.code == 0 and int(r0.pair_nnz_base[0].item()) == 0
+
+
+def test_fuzz_random_distance_matrices_selection_functions_and_amplification(default_params):
+    """Seeded fuzz: ragged families (lengths 1..260, 4..14 sequences, some pairs missing, either orientation), distance
+    matrices that are NOT tree distances (random symmetric integers), random T, f in {max, min, sum}, h in [1, 5],
+    relaxation caps 1..11, thresholds 0.0005 .. 0.05 -- element by element against the oracle."""
+    import torch
+    qp = _qp()
+    dev = torch.device("cuda:0")
+    total = 0
+    for seed in range(1, 13):
+        rng = np.random.default_rng(5000 + seed)
+        q = inputs.background()
+        k = int(rng.integers(4, 15))
+        root = rng.choice(20, size=260, p=q).astype(np.uint8)
+        seqs = []
+        for _ in range(k):
+            L = int(np.exp(rng.uniform(np.log(1), np.log(260))))
+            s = root[:L].copy()
+            hit = rng.random(L) < rng.uniform(0.05, 0.5)
+            s[hit] = rng.choice(20, size=int(hit.sum()), p=q)
+            seqs.append(s)
+        fam = inputs.pack(seqs)
+        pairs = inputs.all_pairs(fam.k)
+        pairs = pairs[rng.random(len(pairs)) < rng.uniform(0.6, 1.0)]
+        if len(pairs) == 0:
+            continue
+        flip = rng.random(len(pairs)) < 0.5
+        pairs[flip] = pairs[flip][:, ::-1]
+        pairs = np.ascontiguousarray(pairs)
+        prm = inputs.Params(hmm=default_params.hmm, pf=default_params.pf, threshold=float(rng.choice([0.0005, 0.01, 0.05])))
+        S, _ = _oracle_stage1(fam, pairs, prm)
+        td = rng.integers(1, 30, size=(k, k))
+        td = np.minimum(td, td.T)
+        np.fill_diagonal(td, 1)
+        T, f = int(rng.integers(0, 40)), str(rng.choice(["max", "min", "sum"]))
+        h, mr = float(rng.uniform(1.0, 5.0)), int(rng.integers(1, 12))
+        fsel = {"max": oc.SEL_MAX, "min": oc.SEL_MIN, "sum": oc.SEL_SUM}[f]
+        ref, cnt = oc.transform(S, fam.k, td, T=T, f=fsel, h=h, max_relax=mr, tau=prm.threshold)
+        d_offs = torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev)
+        d_pairs = torch.from_numpy(pairs).to(dev)
+        d_td = torch.from_numpy(np.ascontiguousarray(td, dtype=np.int32)).to(dev)
+        csr, nnz = _upload(S, pairs, fam, dev)
+        res = qp.consistency(d_offs, fam.k, d_pairs, csr, d_td, h_offsets=fam.offsets, h_pairs=pairs, nnz=nnz, T=T, f=f, h=h,
+                             max_relax=mr, threshold=prm.threshold)
+        _compare(res, ref, cnt, pairs, fam, prm.threshold)
+        total += sum(cnt.values())
+    assert total > 500

@@ -558,3 +558,66 @@ def test_rows_much_longer_than_columns_in_a_wide_stripe(default_params):
         _compare(fam, pairs, prm, res, run, **tol)
     res = qp.run_family(fam, pairs, prm)   # production instances
     _compare(fam, pairs, prm, res, run, dense=False, logZ=False)
+
+
+@pytest.mark.parametrize("seed", [14, 15, 18, 19])
+def test_fuzz_skewed_length_regimes(seed):
+    """Seeded fuzz over length regimes the configs do not reach: a few very short sequences against 1 500..3 200 residues
+    (every split class, several passes), and log-uniform lengths 2..2 500; random models (G in {1, 2} per automaton,
+    alphabets 4..31), random thresholds; test instances and production instances, both precisions."""
+    qp = _qp()
+    rng = np.random.default_rng(seed)
+    A = int(rng.choice([4, 12, 20, 31]))
+    gh, gp = int(rng.integers(1, 3)), int(rng.integers(1, 3))
+    prm = inputs.Params(hmm=inputs.random_model(rng, gh, A), pf=inputs.random_model(rng, gp, A),
+                        threshold=float(rng.choice([0.001, 0.01, 0.05, 0.2])))
+    if seed % 4 == 2:
+        lens = [int(v) for v in rng.integers(1, 60, size=4)] + [int(v) for v in rng.integers(1500, 3200, size=3)] + [513, 769]
+    else:
+        lens = [int(v) for v in np.exp(rng.uniform(np.log(2), np.log(2500), size=9))]
+    fam = inputs.pack([rng.integers(0, A, size=n).astype(np.uint8) for n in lens])
+    pairs = inputs.all_pairs(fam.k)
+    pairs = pairs[rng.permutation(len(pairs))[:24]]
+    flip = rng.random(len(pairs)) < 0.5
+    pairs[flip] = pairs[flip][:, ::-1]
+    run = orc.Run(prm, fam, pairs, keep_dense=True)
+    for precision in ("fp32", "fp64"):
+        tol = dict(p_atol=1e-7, d_rtol=1e-6, logz_rtol=1e-11) if precision == "fp64" else dict(logz_rtol=5e-6)
+        res = qp.run_family(fam, pairs, prm, precision=precision, want_dense=True, want_logZ=True)
+        _compare(fam, pairs, prm, res, run, **tol)
+        res = qp.run_family(fam, pairs, prm, precision=precision)
+        _compare(fam, pairs, prm, res, run, dense=False, logZ=False, **tol)
+
+
+@pytest.mark.parametrize("seed", [2, 5, 7])
+def test_fuzz_identical_and_near_identical_sequences(seed):
+    """Identical sequences and copies with 1 % / 8 % substitutions and a short deletion, lengths 1..2 600 (log-uniform),
+    protein and nucleotide models: every pair goes through the fp64 distance queue (all three fp64 classes); distances
+    to relative 1e-5 against the oracle, posteriors to 1e-4."""
+    qp = _qp()
+    rng = np.random.default_rng(1000 + seed)
+    nuc = seed % 5 == 0
+    prm = inputs.nucleotide_params() if nuc else inputs.default_params()
+    A = 4 if nuc else 20
+    seqs = []
+    for _ in range(4):
+        n = int(np.exp(rng.uniform(np.log(1), np.log(2600))))
+        base = rng.integers(0, A, size=max(n, 1)).astype(np.uint8)
+        seqs.append(base)
+        for rate in (0.0, 0.01, 0.08):
+            s = base.copy()
+            mut = rng.random(len(s)) < rate
+            s[mut] = rng.integers(0, A, size=int(mut.sum()))
+            if len(s) > 10 and rate > 0:
+                cut = int(rng.integers(0, len(s) - 3))
+                s = np.concatenate([s[:cut], s[cut + int(rng.integers(1, 3)):]])
+            seqs.append(s.astype(np.uint8))
+    fam = inputs.pack(seqs)
+    pairs = np.array([(4 * g + a, 4 * g + b) if (a + b + seed) % 2 else (4 * g + b, 4 * g + a)
+                      for g in range(4) for a in range(4) for b in range(a + 1, 4)], dtype=np.int32)
+    run = orc.Run(prm, fam, pairs, keep_dense=True)
+    res = qp.run_family(fam, pairs, prm, want_dense=True, want_logZ=True, beta_guess=0.3)
+    _compare(fam, pairs, prm, res, run)
+    assert int(res.status[3].item()) == len(pairs)          # every pair was re-evaluated in fp64
+    res = qp.run_family(fam, pairs, prm, beta_guess=0.3)
+    _compare(fam, pairs, prm, res, run, dense=False, logZ=False)
