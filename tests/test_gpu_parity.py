@@ -621,3 +621,35 @@ def test_fuzz_identical_and_near_identical_sequences(seed):
     assert int(res.status[3].item()) == len(pairs)          # every pair was re-evaluated in fp64
     res = qp.run_family(fam, pairs, prm, beta_guess=0.3)
     _compare(fam, pairs, prm, res, run, dense=False, logZ=False)
+
+
+def test_maximum_sequence_length(default_params):
+    """QP_MAX_LEN = 65 535 residues as rows and as columns (128 column blocks of the widest split class, 16 passes),
+    against a medium and a short sequence, plus a 40 000-residue near copy (the fp64 distance queue at that length).
+    fp32 at the usual tolerances; the fp64 mode at 1e-6 on P: at |ln Z| ~ 2e5 the ORACLE's log-space fp64 values have an
+    absolute rounding error of 3e-11 per operation, which 65 535 rows accumulate to ~1e-7."""
+    qp = _qp()
+    rng = np.random.default_rng(77)
+    q = inputs.background()
+    big = rng.choice(20, size=65535, p=q).astype(np.uint8)
+    mid = big[30000:30300].copy()
+    hit = rng.random(300) < 0.3
+    mid[hit] = rng.choice(20, size=int(hit.sum()), p=q)
+    small = big[100:120].copy()
+    near = big[:40000].copy()
+    hit = rng.random(40000) < 0.02
+    near[hit] = rng.choice(20, size=int(hit.sum()), p=q)
+    fam = inputs.pack([big, mid, small, near])
+    pairs = np.array([[0, 1], [1, 0], [0, 2], [2, 0], [3, 1], [1, 3]], dtype=np.int32)
+    run = orc.Run(default_params, fam, pairs, keep_dense=True)
+    res = qp.run_family(fam, pairs, default_params, want_dense=True, want_logZ=True, beta_guess=0.02)
+    _compare(fam, pairs, default_params, res, run, logz_rtol=5e-6)
+    res = qp.run_family(fam, pairs, default_params, beta_guess=0.02)
+    _compare(fam, pairs, default_params, res, run, dense=False, logZ=False)
+    res = qp.run_family(fam, pairs, default_params, precision="fp64", beta_guess=0.02)
+    _compare(fam, pairs, default_params, res, run, dense=False, logZ=False, p_atol=1e-6, d_rtol=1e-6)
+    # one residue more is refused
+    over = inputs.pack([np.zeros(65536, np.uint8), small])
+    with pytest.raises(qp.QpError) as ei:
+        qp.run_family(over, np.array([[0, 1]], dtype=np.int32), default_params)
+    assert ei.value.code == qp.ERR["EMPTY_SEQUENCE"]
