@@ -20,8 +20,10 @@ namespace {
 inline int64_t al256(int64_t v) { return (v + 255) & ~(int64_t)255; }
 
 // columns as 16-bit values for the trip over PCIe (QP_MAX_LEN = 65535: lossless); the count is read on the device
-__global__ void k_narrow_cols(const int32_t* __restrict__ col, const int64_t* __restrict__ count, uint16_t* __restrict__ col16) {
-    const int64_t n = *count;
+// (a batch whose CSR did not fit reports the size it NEEDS there: never walk past the slot's capacity)
+__global__ void k_narrow_cols(const int32_t* __restrict__ col, const int64_t* __restrict__ count, int64_t cap,
+                              uint16_t* __restrict__ col16) {
+    const int64_t n = *count < cap ? *count : cap;
     for (int64_t q = (blockIdx.x * (int64_t)blockDim.x + threadIdx.x) * 2; q < n; q += (int64_t)gridDim.x * blockDim.x * 2) {
         if (q + 1 < n) *(ushort2*)(col16 + q) = make_ushort2((unsigned short)col[q], (unsigned short)col[q + 1]);
         else col16[q] = (uint16_t)col[q];
@@ -328,7 +330,7 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         o.status = s.status;
         const int r = qp_posteriors(d_seqs, d_offs, k, s.pairs, nb, &prm, s.ws, (size_t)s.ws_bytes, &o, comp);
         if (r != QP_OK) return r;
-        if (out->col_idx16) k_narrow_cols<<<1184, 256, 0, comp>>>(s.col, s.nnz_base + nb, s.col16);
+        if (out->col_idx16) k_narrow_cols<<<1184, 256, 0, comp>>>(s.col, s.nnz_base + nb, s.cap, s.col16);
         cudaMemcpyAsync(s.h_last, s.nnz_base + nb, 8, cudaMemcpyDeviceToHost, comp);
         cudaMemcpyAsync(s.h_status, s.status, 16, cudaMemcpyDeviceToHost, comp);
         cudaEventRecord(s.sized, comp);

@@ -379,6 +379,12 @@ def test_host_call_matches_single_call(default_params):
     dense = qp.HostCall(fam, pairs, default_params, beta_guess=0.004, nnz_capacity=nz + 16)
     same(dense.run())
     assert dense.batches > hc.batches                          # overflowing batches were split
+    # the same with 16-bit columns: the narrowing kernel of an overflowing batch must stop at the slot's capacity (it
+    # once walked on to the size the batch NEEDED and overwrote the slot's status word and workspace)
+    dense16 = qp.HostCall(fam, pairs, default_params, beta_guess=0.004, nnz_capacity=nz + 16, compact_cols=True).run()
+    assert dense16.code == 0 and dense16.nnz == nz and dense16.batches > hc.batches
+    assert torch.equal(dense16.col_idx16[:nz].to(torch.int32), want["col"]) and torch.equal(dense16.val[:nz], want["val"])
+    assert torch.equal(dense16.dist, want["dist"]) and torch.equal(dense16.pair_nnz_base, want["nb"])
     compact = qp.HostCall(fam, pairs, default_params, compact_cols=True).run()      # columns as uint16: 6 B / entry
     assert compact.code == 0 and compact.nnz == nz and compact.col_idx is None
     assert torch.equal(compact.col_idx16[:nz].to(torch.int32), want["col"]) and torch.equal(compact.val[:nz], want["val"])
