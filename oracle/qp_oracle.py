@@ -230,5 +230,8 @@ class Run:
 
     def __del__(self):
         if getattr(self, "_h", None):
-            lib().qpo_result_free(self._h)
+            try:
+                lib().qpo_result_free(self._h)
+            except TypeError:   # interpreter shutdown: the module globals are already gone, the process frees the memory
+                pass
             self._h = None
