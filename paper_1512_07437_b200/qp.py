@@ -6,6 +6,7 @@ libqp.so has not been built (python -m paper_1512_07437_b200.build), and calling
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes as C
 import os
 from dataclasses import dataclass
@@ -274,21 +275,25 @@ def posteriors(d_seqs, d_offsets, k, d_pairs, cparams: CParams, workspace, *, nn
     P = int(d_pairs.shape[0])
     i64, i32, f32 = torch.int64, torch.int32, torch.float32
     o = _Output()
-    t = dict(
-        pair_row_base=reuse.pair_row_base, pair_nnz_base=reuse.pair_nnz_base, row_ptr=reuse.row_ptr,
-        col_idx=reuse.col_idx, val=reuse.val, dist=reuse.dist, dense_P=reuse.dense_P, logZ=reuse.logZ,
-        status=reuse.status,
-    ) if reuse is not None else dict(
-        pair_row_base=torch.empty(P + 1, dtype=i64, device=dev),
-        pair_nnz_base=torch.empty(P + 1, dtype=i64, device=dev),
-        row_ptr=torch.empty(max(int(h_rows_total), 1), dtype=i32, device=dev),
-        col_idx=torch.empty(max(int(nnz_capacity), 1), dtype=i32, device=dev),
-        val=torch.empty(max(int(nnz_capacity), 1), dtype=f32, device=dev),
-        dist=dist if dist is not None else torch.zeros((k, k), dtype=f32, device=dev),
-        dense_P=torch.empty(int(want_dense_cells), dtype=f32, device=dev) if want_dense_cells else None,
-        logZ=torch.empty((P, 4), dtype=torch.float64, device=dev) if want_logZ else None,
-        status=torch.zeros(4, dtype=i32, device=dev),
-    )
+    if reuse is not None:
+        t = dict(pair_row_base=reuse.pair_row_base, pair_nnz_base=reuse.pair_nnz_base, row_ptr=reuse.row_ptr,
+                 col_idx=reuse.col_idx, val=reuse.val, dist=reuse.dist, dense_P=reuse.dense_P, logZ=reuse.logZ,
+                 status=reuse.status)
+    else:
+        # fresh outputs are created (and zero-filled) on the stream the call runs on: torch would otherwise fill them
+        # on its current stream, unordered with the kernels that write them
+        with torch.cuda.stream(stream) if stream is not None else contextlib.nullcontext():
+            t = dict(
+                pair_row_base=torch.empty(P + 1, dtype=i64, device=dev),
+                pair_nnz_base=torch.empty(P + 1, dtype=i64, device=dev),
+                row_ptr=torch.empty(max(int(h_rows_total), 1), dtype=i32, device=dev),
+                col_idx=torch.empty(max(int(nnz_capacity), 1), dtype=i32, device=dev),
+                val=torch.empty(max(int(nnz_capacity), 1), dtype=f32, device=dev),
+                dist=dist if dist is not None else torch.zeros((k, k), dtype=f32, device=dev),
+                dense_P=torch.empty(int(want_dense_cells), dtype=f32, device=dev) if want_dense_cells else None,
+                logZ=torch.empty((P, 4), dtype=torch.float64, device=dev) if want_logZ else None,
+                status=torch.zeros(4, dtype=i32, device=dev),
+            )
     for name, v in t.items():
         setattr(o, name, v.data_ptr() if v is not None else None)
     o.nnz_capacity = int(nnz_capacity)

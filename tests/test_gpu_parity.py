@@ -659,3 +659,62 @@ def test_maximum_sequence_length(default_params):
     with pytest.raises(qp.QpError) as ei:
         qp.run_family(over, np.array([[0, 1]], dtype=np.int32), default_params)
     assert ei.value.code == qp.ERR["EMPTY_SEQUENCE"]
+
+
+def test_concurrent_callers_threads_and_interleaved_streams(default_params):
+    """The library keeps its side streams and events per host thread and device: four host threads calling at the same
+    time, and one thread interleaving calls on two streams (separate workspaces, no synchronisation in between), all get
+    bit for bit the results of calls made one after the other."""
+    import threading
+    import torch
+    qp = _qp()
+    dev = torch.device("cuda:0")
+    fams = [inputs.config_family(1), inputs.config_family(0), inputs.random_family(np.random.default_rng(3), 30, 50, 400)]
+    refs = []
+    for fam in fams:
+        pairs = inputs.all_pairs(fam.k)
+        r = qp.run_family(fam, pairs, default_params)
+        nz = int(r.pair_nnz_base[-1].item())
+        refs.append((pairs, r.dist.clone(), r.val[:nz].clone(), r.col_idx[:nz].clone(), r.pair_nnz_base.clone()))
+
+    def same(r, ref):
+        nz = int(ref[4][-1].item())
+        return (int(r.status[0].item()) == 0 and torch.equal(r.dist, ref[1]) and torch.equal(r.val[:nz], ref[2]) and
+                torch.equal(r.col_idx[:nz], ref[3]) and torch.equal(r.pair_nnz_base, ref[4]))
+
+    outs = [[] for _ in range(4)]
+
+    def worker(i):
+        try:
+            for _ in range(4):
+                outs[i].append(same(qp.run_family(fams[i % 3], refs[i % 3][0], default_params), refs[i % 3]))
+        except Exception as e:   # noqa: BLE001 -- reported through the assertion below
+            outs[i].append(repr(e))
+
+    threads = [threading.Thread(target=worker, args=(i,)) for i in range(4)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert all(o == [True] * 4 for o in outs), outs
+
+    def setup(fam, pairs):
+        L = fam.lengths
+        n, m = L[pairs[:, 0]].astype(np.int64), L[pairs[:, 1]].astype(np.int64)
+        cp = qp.CParams(default_params, flags=0)
+        cap = int(0.1 * int((n * m).sum())) + 4096
+        ws = torch.empty(qp.workspace_bytes(fam.offsets, fam.k, pairs, cp, cap), dtype=torch.uint8, device=dev)
+        args = (torch.from_numpy(np.ascontiguousarray(fam.seqs)).to(dev),
+                torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev), fam.k,
+                torch.from_numpy(pairs).to(dev), cp, ws)
+        return args, dict(nnz_capacity=cap, h_rows_total=int((n + 1).sum()), check=False)
+
+    (a_args, a_kw), (b_args, b_kw) = setup(fams[0], refs[0][0]), setup(fams[2], refs[2][0])
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    for _ in range(4):
+        ra = qp.posteriors(*a_args, stream=s1, **a_kw)
+        rb = qp.posteriors(*b_args, stream=s2, **b_kw)
+        ra = qp.posteriors(*a_args, stream=s1, reuse=ra, **a_kw)
+        torch.cuda.synchronize()
+        assert same(ra, refs[0]) and same(rb, refs[2])
