@@ -430,12 +430,15 @@ def consistency(d_offsets, k, d_pairs, csr, treedist, *, h_offsets, h_pairs, nnz
     ws = workspace if workspace is not None else torch.empty(max(int(need.value), 256), dtype=torch.uint8, device=dev)
     i64, i32, f32 = torch.int64, torch.int32, torch.float32
     rows_total = int(csr.row_ptr.numel())
-    out = Result(pair_row_base=csr.pair_row_base, pair_nnz_base=torch.empty(P + 1, dtype=i64, device=dev),
-                 row_ptr=torch.empty(max(rows_total, 1), dtype=i32, device=dev),
-                 col_idx=torch.empty(max(int(nnz), 1), dtype=i32, device=dev),
-                 val=torch.empty(max(int(nnz), 1), dtype=f32, device=dev), dist=None, dense_P=None, dense_off=None,
-                 logZ=None, status=torch.zeros(4, dtype=i32, device=dev), code=0, launches=9)
-    out.relaxations = torch.zeros(max(P, 1), dtype=i32, device=dev)
+    # the zero-filled outputs are created, and the status is read back, on the stream the call runs on
+    on_stream = (lambda: torch.cuda.stream(stream)) if stream is not None else contextlib.nullcontext
+    with on_stream():
+        out = Result(pair_row_base=csr.pair_row_base, pair_nnz_base=torch.empty(P + 1, dtype=i64, device=dev),
+                     row_ptr=torch.empty(max(rows_total, 1), dtype=i32, device=dev),
+                     col_idx=torch.empty(max(int(nnz), 1), dtype=i32, device=dev),
+                     val=torch.empty(max(int(nnz), 1), dtype=f32, device=dev), dist=None, dense_P=None, dense_off=None,
+                     logZ=None, status=torch.zeros(4, dtype=i32, device=dev), code=0, launches=9)
+        out.relaxations = torch.zeros(max(P, 1), dtype=i32, device=dev)
     ci = _Csr(csr.pair_row_base.data_ptr(), csr.pair_nnz_base.data_ptr(), csr.row_ptr.data_ptr(), csr.col_idx.data_ptr(),
               csr.val.data_ptr())
     co = _CsrOut(out.pair_nnz_base.data_ptr(), out.row_ptr.data_ptr(), out.col_idx.data_ptr(), out.val.data_ptr(), int(nnz),
@@ -448,7 +451,8 @@ def consistency(d_offsets, k, d_pairs, csr, treedist, *, h_offsets, h_pairs, nnz
                                    C.c_void_p(st.cuda_stream))
     out._ws = ws
     if code == QP_OK and check:
-        code = int(out.status[0].item())      # synchronises
+        with on_stream():
+            code = int(out.status[0].item())      # synchronises
     out.code = int(code)
     if check and code != QP_OK:
         raise QpError(code)
