@@ -227,11 +227,18 @@ struct MaxW64 {
 //   its pairs). What was taken is recorded in poll_bytes; the fp32 slots start behind it.
 // which = 1, after the fp32 classes have joined: the drainers' slots reuse the fp32 slot region; one slot for every
 //   class with pairs left (a misfit is an error), then the rest of the region class by class.
-__global__ void k_refine_plan(int which, MaxW64 maxw, int64_t avail, SchedHeader* h) {
+__global__ void k_refine_plan(int which, MaxW64 maxw, int64_t avail, const PairInfo* __restrict__ info,
+                              const int32_t* __restrict__ order, SchedHeader* h) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     RefineQ& rq = h->rq;
     if (which == 0) {
-        unsigned long long room = (unsigned long long)avail / 2, used = 0;
+        // the pollers never take what the fp32 classes need at the least (one slot per class, sized for its largest
+        // pair -- the first of its list): a workspace of exactly the minimum that qp_workspace_bytes reports must do
+        long long fp32_min = 0;
+        for (int c = 0; c < kNumClasses; ++c)
+            if (h->cls_count[c] > 0) fp32_min += (long long)bin_ub(info[order[h->cls_start[c]]].bin);
+        const long long spare = (long long)avail - fp32_min;
+        unsigned long long room = (unsigned long long)min((long long)avail / 2, max(spare, 0ll)), used = 0;
         for (int c = kNumPacked; c < kSplitEnd; ++c) {   // slot sizes grow with the class index
             const unsigned long long sb = (rq.poll_slot_bytes[c] + 255ull) & ~255ull;
             rq.poll_slot_bytes[c] = sb;
@@ -752,7 +759,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     MaxW64 mw64;
     for (int c = 0; c < kNumClasses; ++c) mw64.w[c] = ((kMaskRefine >> c) & 1) ? max_units(c, true, sms) : 0;
     if (pollers) {   // the pollers' slots come off the head of the slot region
-        k_refine_plan<<<1, 32, 0, st>>>(0, mw64, avail, hdr);
+        k_refine_plan<<<1, 32, 0, st>>>(0, mw64, avail, (const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), hdr);
         ++g_launches;
     }
     MaxW mw;
@@ -807,7 +814,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
 
     // ---- drainers: what the pollers have not taken when the fp32 classes have finished ----------------------------
     if (refine) {
-        k_refine_plan<<<1, 32, 0, st>>>(1, mw64, avail, hdr);
+        k_refine_plan<<<1, 32, 0, st>>>(1, mw64, avail, (const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), hdr);
         ++g_launches;
         QP_TRY(cudaEventRecord(cx->fork2, st));
         ka64->refine_pass = 2;

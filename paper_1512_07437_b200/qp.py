@@ -211,6 +211,19 @@ class CParams:
         return C.byref(self.s)
 
 
+def min_workspace_bytes(h_offsets, k, h_pairs, cparams: CParams, nnz_capacity: int, want_dense=False) -> int:
+    """The smallest workspace qp_posteriors accepts for this call (one scratch slot per class): the size that
+    qp_workspace_bytes reports back when the budget it is given is too small."""
+    h_offsets = np.ascontiguousarray(h_offsets, dtype=np.int64)
+    h_pairs = np.ascontiguousarray(h_pairs, dtype=np.int32).reshape(-1, 2)
+    out = C.c_size_t(0)
+    r = _lib.qp_workspace_bytes(h_offsets.ctypes.data, int(k), h_pairs.ctypes.data, len(h_pairs), cparams.ref,
+                                int(nnz_capacity), int(bool(want_dense)), 1, C.byref(out))
+    if r not in (QP_OK, ERR["WORKSPACE_TOO_SMALL"]):
+        raise QpError(r)
+    return int(out.value)
+
+
 def workspace_bytes(h_offsets, k, h_pairs, cparams: CParams, nnz_capacity: int, want_dense=False, budget=0) -> int:
     """qp_workspace_bytes: host-only query (numpy int64 offsets [k+1], int32 pairs [P,2])."""
     h_offsets = np.ascontiguousarray(h_offsets, dtype=np.int64)

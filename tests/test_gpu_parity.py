@@ -718,3 +718,40 @@ def test_concurrent_callers_threads_and_interleaved_streams(default_params):
         ra = qp.posteriors(*a_args, stream=s1, reuse=ra, **a_kw)
         torch.cuda.synchronize()
         assert same(ra, refs[0]) and same(rb, refs[2])
+
+
+@pytest.mark.parametrize("kind", ["random", "log_uniform", "near_identical"])
+def test_minimum_workspace_is_enough(default_params, kind):
+    """A workspace of EXACTLY the minimum that qp_workspace_bytes reports (one scratch slot per class) runs the call and
+    gives bit for bit the results of a full-size workspace. (The slots of the fp64 pollers once came off the top
+    regardless and left the fp32 classes short: QP_ERR_WORKSPACE_TOO_SMALL at the advertised minimum.)"""
+    import torch
+    qp = _qp()
+    dev = torch.device("cuda:0")
+    rng = np.random.default_rng({"random": 708, "log_uniform": 705, "near_identical": 702}[kind])
+    if kind == "random":
+        fam = inputs.random_family(rng, 12, 1, 300)
+    elif kind == "log_uniform":
+        fam = inputs.pack([rng.integers(0, 20, size=int(n)).astype(np.uint8)
+                           for n in np.exp(rng.uniform(np.log(2), np.log(2500), size=8))])
+    else:
+        base = rng.integers(0, 20, size=900).astype(np.uint8)
+        fam = inputs.pack([base] + [np.where(rng.random(900) < 0.03, rng.integers(0, 20, size=900), base).astype(np.uint8)
+                                    for _ in range(6)])
+    pairs = inputs.all_pairs(fam.k)
+    ref = qp.run_family(fam, pairs, default_params, beta_guess=0.3)
+    nz = int(ref.pair_nnz_base[-1].item())
+    cp = qp.CParams(default_params)
+    full = qp.workspace_bytes(fam.offsets, fam.k, pairs, cp, nz + 8)
+    least = qp.min_workspace_bytes(fam.offsets, fam.k, pairs, cp, nz + 8)
+    assert least < full
+    L = fam.lengths
+    args = (torch.from_numpy(np.ascontiguousarray(fam.seqs)).to(dev),
+            torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev), fam.k, torch.from_numpy(pairs).to(dev), cp)
+    for wsb in (least, (least + full) // 2):
+        ws = torch.empty(wsb, dtype=torch.uint8, device=dev)
+        res = qp.posteriors(*args, ws, nnz_capacity=nz + 8, h_rows_total=int((L[pairs[:, 0]] + 1).sum()), check=False)
+        assert res.code == 0, (wsb, res.status.tolist())
+        assert torch.equal(res.dist, ref.dist) and torch.equal(res.pair_nnz_base, ref.pair_nnz_base)
+        assert torch.equal(res.val[:nz], ref.val[:nz]) and torch.equal(res.col_idx[:nz], ref.col_idx[:nz])
+        assert int(res.status[3].item()) == int(ref.status[3].item())
