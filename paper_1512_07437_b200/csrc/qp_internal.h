@@ -98,6 +98,7 @@ QP_HD2 int64_t slot_bytes(int n, int C, int nb, int real_bytes) {
 //      expressed in cells), a pass = W neighbouring blocks;
 // Returns the class index (-1 if the mask holds no class that can take the pair) and the number of 32*C-column blocks.
 constexpr int64_t kTwoBlockMaxCells = 400000;
+constexpr int kMultiBlockMaxRows = 256;
 QP_HD2 int choose_class(int n, int cols, uint32_t mask, bool fp64, int* nb_out) {
     constexpr int kStepOverhead = 6;
     int best = -1, best_nb = 0;
@@ -119,6 +120,16 @@ QP_HD2 int choose_class(int n, int cols, uint32_t mask, bool fp64, int* nb_out) 
                 return c;
             }
         }
+    // 2b. short rows against many columns (at most kMultiBlockMaxRows rows): the ramp of a split pass (32 steps per
+    //     active warp) would outweigh the rows; one warp runs the column blocks of the widest multi-block class one
+    //     after the other instead (n + 32 steps per block)
+    if (n <= kMultiBlockMaxRows && (int64_t)n * cols <= kTwoBlockMaxCells && ((mask >> (kNumClasses - 1)) & 1)) {
+        const int C = class_C(kNumClasses - 1, fp64);
+        if (C > 0) {
+            *nb_out = (cols + 32 * C - 1) / (32 * C);
+            return kNumClasses - 1;
+        }
+    }
     for (int c = kNumPacked; c < kSplitEnd; ++c) {
         if (!((mask >> c) & 1)) continue;
         const int C = class_C(c, fp64), W = class_W(c, fp64);

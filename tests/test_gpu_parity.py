@@ -645,8 +645,10 @@ def test_maximum_sequence_length(default_params):
     near = big[:40000].copy()
     hit = rng.random(40000) < 0.02
     near[hit] = rng.choice(20, size=int(hit.sum()), p=q)
-    fam = inputs.pack([big, mid, small, near])
-    pairs = np.array([[0, 1], [1, 0], [0, 2], [2, 0], [3, 1], [1, 3]], dtype=np.int32)
+    tiny = big[5000:5005].copy()
+    fam = inputs.pack([big, mid, small, near, tiny])
+    # [4, 0]: 5 rows against 65 535 columns = 171 column blocks run by ONE warp (short rows: the multi-block class)
+    pairs = np.array([[0, 1], [1, 0], [0, 2], [2, 0], [3, 1], [1, 3], [4, 0], [0, 4], [4, 3]], dtype=np.int32)
     run = orc.Run(default_params, fam, pairs, keep_dense=True)
     res = qp.run_family(fam, pairs, default_params, want_dense=True, want_logZ=True, beta_guess=0.02)
     _compare(fam, pairs, default_params, res, run, logz_rtol=5e-6)
