@@ -18,6 +18,9 @@ INC = os.path.join(os.path.dirname(HERE), "include")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libqp.so")
 
+# -lineinfo stays in the default build: it adds line tables to the ELF (no code change: same SASS, same registers) and is
+# what lets `ncu --import-source on` map the profiles under profiles/ back to csrc/ (the driver's build() contract asks
+# for it as well)
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + INC, "-I" + CSRC] + os.environ.get("QP_EXTRA_NVCC_FLAGS", "").split()
 
