@@ -139,7 +139,10 @@ int qp_posteriors(const uint8_t* d_seqs, const int64_t* d_offsets, int32_t k, co
  *                                  nnz / cells (<= 0: 0.05) sizes the per-batch device CSR; the call fills status,
  *                                  h2d_bytes / d2h_bytes (bytes it copied) and batches
  * Returns QP_OK or an error of qp_posteriors; QP_ERR_NNZ_CAPACITY if out->nnz_capacity is too small (pair_nnz_base[P] =
- * entries required). params->flags: QP_FLAG_NO_REFINE is honoured, the others are set by the call.
+ * entries required). A batch denser than beta_guess is split in two and taken again; a SINGLE pair whose entries do not
+ * fit the per-batch device CSR ends the call with QP_ERR_NNZ_CAPACITY and status[1] = that pair (raise beta_guess).
+ * params->flags: QP_FLAG_NO_REFINE is honoured, the others are set by the call (it runs its batches with
+ * QP_FLAG_NO_POLLERS).
  */
 typedef struct {
     int64_t* pair_row_base;  /* [P+1] */
