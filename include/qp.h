@@ -41,7 +41,8 @@ enum {
     QP_ERR_WORKSPACE_TOO_SMALL = -5,/* workspace cannot hold the fixed arrays + one scratch slot per class     */
     QP_ERR_NNZ_CAPACITY = -6,       /* CSR needs more than nnz_capacity entries; pair_nnz_base[P] = required   */
     QP_ERR_CUDA = -7,               /* a CUDA runtime call failed                                              */
-    QP_ERR_RANGE = -8               /* model weights outside the dynamic range the kernels renormalise for     */
+    QP_ERR_RANGE = -8,              /* model weights outside the dynamic range the kernels renormalise for     */
+    QP_ERR_STATIC_LIMIT = -9        /* qp_guide_tree_static: k > QP_GUIDE_TREE_STATIC_MAX_K (built-in scratch)   */
 };
 
 enum { QP_FP32 = 0, QP_FP64 = 1 };
@@ -209,6 +210,34 @@ int qp_last_tau_curve(double* tau, int64_t* count, int max_bins);
 size_t qp_guide_tree_workspace_bytes(int32_t k);
 int qp_guide_tree(const float* d_dist, int32_t k, int32_t* d_merge, float* d_height, int32_t* d_leaves,
                   int32_t* d_parent, int32_t* d_treedist, void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * qp_guide_tree without a workspace argument and without any allocation, for callers that cannot allocate device
+ * memory: a plug-in inside a host application that owns the whole device heap and hands out only input and output
+ * buffers; a step inside a latency-critical loop, where cudaMalloc / cudaFree may block on the driver and synchronise
+ * the device; a process held to a fixed memory reservation on a shared GPU, where a late allocation can fail even
+ * though the inputs fit. Same arguments, same kernels and bit-identical outputs as qp_guide_tree, minus d_workspace:
+ * the scratch of the merge loop is an array built into libqp.so.
+ *   limit      k <= QP_GUIDE_TREE_STATIC_MAX_K (1024: BASELINE.json's largest family has 1000 sequences). Larger k
+ *              returns QP_ERR_STATIC_LIMIT and launches nothing; use qp_guide_tree with your own workspace.
+ *   cost       the array (QP_GUIDE_TREE_STATIC_BYTES, about 4 MiB) is part of the library image: every GPU on which
+ *              libqp.so's kernels are loaded holds it until the process exits, whether or not this call is used.
+ *   first call the first call on each device looks up the array's device address (one cudaGetSymbolAddress with that
+ *              device current; result kept for the life of the process). Make that first call outside any stream
+ *              capture, with the device you mean to use current.
+ *   sharing    every call on a device uses the SAME array. Calls on one stream run in order and are fine. Two calls
+ *              that can overlap on the GPU (different streams, different host threads without ordering) race on it
+ *              and give wrong trees: order them yourself (one stream, or events). Nothing has to be cleared between
+ *              calls -- the merge kernel rewrites every scratch word it later reads -- so a call never sees what the
+ *              previous one left, whatever its k was.
+ * The call runs no cudaMalloc, cudaFree or allocating library routine; it enqueues two kernels on the stream and
+ * returns without synchronising. Other errors: QP_ERR_INVALID_ARG (NULL pointer, k < 1), QP_ERR_CUDA (no current
+ * device, address lookup or launch failed).
+ */
+#define QP_GUIDE_TREE_STATIC_MAX_K 1024
+#define QP_GUIDE_TREE_STATIC_BYTES (QP_GUIDE_TREE_STATIC_MAX_K * (QP_GUIDE_TREE_STATIC_MAX_K * 4 + 8 + 4 + 1))
+int qp_guide_tree_static(const float* d_dist, int32_t k, int32_t* d_merge, float* d_height, int32_t* d_leaves,
+                         int32_t* d_parent, int32_t* d_treedist, void* cuda_stream);
 
 /*
  * Stage III: selective consistency transformation of the sparse posterior matrices.

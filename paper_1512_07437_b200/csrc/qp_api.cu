@@ -611,6 +611,7 @@ extern "C" const char* qp_status_string(int s) {
         case QP_ERR_NNZ_CAPACITY: return "nnz capacity exceeded";
         case QP_ERR_CUDA: return "CUDA runtime error";
         case QP_ERR_RANGE: return "model weights outside the supported dynamic range";
+        case QP_ERR_STATIC_LIMIT: return "more sequences than the built-in scratch of qp_guide_tree_static holds (1024)";
         default: return "unknown status";
     }
 }

@@ -197,3 +197,79 @@ extern "C" int qp_guide_tree(const float* d_dist, int32_t k, int32_t* d_merge, f
     }
     return cudaGetLastError() == cudaSuccess ? QP_OK : QP_ERR_CUDA;
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// qp_guide_tree_static: the same two kernels for callers that have no device memory to hand over as a workspace.
+//
+// Who that is: code that runs where cudaMalloc / cudaFree may not be called or would be harmful -- a plug-in inside
+// a host program that owns all device memory and gives the plug-in only its input and output buffers; a step of a
+// latency-critical loop, where an allocation may block on the driver and synchronise the whole device; a process
+// sharing its GPU under a fixed memory reservation, where an allocation made late can fail although the inputs fit.
+// qp_guide_tree asks such a caller for a workspace it cannot create. Here the scratch of the merge loop (working
+// matrix, nearest-neighbour cache, slot tables) lives in the array below, which is part of the library image: the
+// driver places it when the module is loaded on a device and keeps it until the process exits (about 4 MiB on every
+// GPU that loads libqp.so), and the call itself runs no cudaMalloc, cudaFree or allocating library routine.
+//
+// In host code the name g_tree_scratch is only a handle for the symbol, not a device address (passing it to a kernel
+// makes the kernel fault, or quietly use unrelated memory on systems where the GPU can read host memory). The device
+// address is looked up once per device with cudaGetSymbolAddress, with that device current, and kept in a table.
+// ---------------------------------------------------------------------------------------------------------------------
+#include <mutex>
+
+namespace qp {
+
+constexpr int kStaticMaxK = QP_GUIDE_TREE_STATIC_MAX_K;
+constexpr size_t kStaticW = (size_t)kStaticMaxK * kStaticMaxK * 4;   // working matrix, already a multiple of 256
+constexpr size_t kStaticNn = (size_t)kStaticMaxK * 8;
+constexpr size_t kStaticNode = (size_t)kStaticMaxK * 4;
+constexpr size_t kStaticAlive = (size_t)kStaticMaxK;
+constexpr size_t kStaticBytes = kStaticW + kStaticNn + kStaticNode + kStaticAlive;
+static_assert(kStaticW % 256 == 0 && kStaticNn % 256 == 0 && kStaticNode % 256 == 0, "sub-arrays stay 256-byte aligned");
+
+static __device__ __align__(256) unsigned char g_tree_scratch[kStaticBytes];
+
+constexpr int kMaxDevices = 64;
+static unsigned char* g_tree_scratch_addr[kMaxDevices];   // device address of g_tree_scratch on device d, 0 = not looked up
+static std::mutex g_tree_scratch_mutex;
+
+// Device address of the scratch array on the CURRENT device; looked up on the first call per device.
+static int static_scratch(unsigned char** out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDevices) return QP_ERR_CUDA;
+    std::lock_guard<std::mutex> lock(g_tree_scratch_mutex);
+    if (!g_tree_scratch_addr[dev]) {
+        void* p = nullptr;
+        if (cudaGetSymbolAddress(&p, g_tree_scratch) != cudaSuccess || !p) {
+            (void)cudaGetLastError();
+            return QP_ERR_CUDA;
+        }
+        g_tree_scratch_addr[dev] = (unsigned char*)p;
+    }
+    *out = g_tree_scratch_addr[dev];
+    return QP_OK;
+}
+
+}  // namespace qp
+
+extern "C" int qp_guide_tree_static(const float* d_dist, int32_t k, int32_t* d_merge, float* d_height,
+                                    int32_t* d_leaves, int32_t* d_parent, int32_t* d_treedist, void* cuda_stream) {
+    if (k < 1 || !d_dist || !d_leaves || !d_parent || (k > 1 && (!d_merge || !d_height))) return QP_ERR_INVALID_ARG;
+    if (k > kStaticMaxK) return QP_ERR_STATIC_LIMIT;   // the built-in scratch holds QP_GUIDE_TREE_STATIC_MAX_K sequences
+    unsigned char* p = nullptr;
+    const int rc = static_scratch(&p);
+    if (rc != QP_OK) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // Nothing has to be cleared between calls: k_wpgma writes W[0 .. k*k), nn, node and alive [0 .. k) before it reads
+    // any of them, so what the previous call (of any k) left behind is never seen.
+    TreeWs w;
+    w.W = (float*)p;
+    w.nn = (unsigned long long*)(p + kStaticW);
+    w.node = (int32_t*)(p + kStaticW + kStaticNn);
+    w.alive = (uint8_t*)(p + kStaticW + kStaticNn + kStaticNode);
+    k_wpgma<<<1, kTreeThreads, 0, st>>>(d_dist, k, w, d_merge, d_height, d_leaves, d_parent);
+    if (d_treedist) {
+        const size_t n = (size_t)k * k;
+        k_treedist<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_leaves, d_parent, k, d_treedist);
+    }
+    return cudaGetLastError() == cudaSuccess ? QP_OK : QP_ERR_CUDA;
+}

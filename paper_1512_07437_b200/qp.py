@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libqp.so")
 
 QP_OK = 0
 ERR = {"INVALID_ARG": -1, "BAD_RESIDUE": -2, "EMPTY_SEQUENCE": -3, "BAD_PAIR": -4, "WORKSPACE_TOO_SMALL": -5,
-       "NNZ_CAPACITY": -6, "CUDA": -7, "RANGE": -8}
+       "NNZ_CAPACITY": -6, "CUDA": -7, "RANGE": -8, "STATIC_LIMIT": -9}
+GUIDE_TREE_STATIC_MAX_K = 1024
 QP_FP32, QP_FP64 = 0, 1
 FLAG_SYNC_STATUS, FLAG_NO_REFINE, FLAG_NO_POLLERS = 1, 2, 4
 NUM_CLASSES = 22
@@ -26,7 +27,7 @@ NUM_CLASSES = 22
 EXPORTS = ["qp_workspace_bytes", "qp_posteriors", "qp_posteriors_budgeted", "qp_guide_tree", "qp_guide_tree_workspace_bytes", "qp_last_launch_count", "qp_status_string", "qp_version",
            "qp_set_profile", "qp_get_profile", "qp_get_profile_classes", "qp_shutdown",
            "qp_consistency", "qp_consistency_workspace_bytes", "qp_consistency_passes", "qp_last_tau_curve", "qp_measure_peaks",
-           "qp_posteriors_host", "qp_posteriors_host_workspace_bytes"]
+           "qp_posteriors_host", "qp_posteriors_host_workspace_bytes", "qp_guide_tree_static"]
 
 
 class QpError(RuntimeError):
@@ -102,6 +103,9 @@ def _load():
     L.qp_guide_tree.restype = C.c_int
     L.qp_guide_tree.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                 C.c_void_p, C.c_size_t, C.c_void_p]
+    L.qp_guide_tree_static.restype = C.c_int
+    L.qp_guide_tree_static.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                       C.c_void_p]
     L.qp_last_launch_count.restype = C.c_int
     L.qp_status_string.restype = C.c_char_p
     L.qp_status_string.argtypes = [C.c_int]
@@ -392,6 +396,32 @@ def guide_tree(dist, want_treedist=True, stream=None, workspace=None) -> GuideTr
         raise QpError(code)
     t._ws = ws   # keep the workspace alive until the stream has run
     return t
+
+
+def guide_tree_static(out: GuideTree, dist, stream=None) -> GuideTree:
+    """qp_guide_tree_static: the guide tree of `dist` written into the tensors of `out`, with the merge loop's scratch in
+    the array built into libqp.so instead of a workspace. For callers that cannot allocate device memory at the point of
+    the call (all device memory owned by a host application, a loop that must not block in the driver, a fixed memory
+    reservation on a shared GPU) -- which is why this wrapper creates no tensor either: `dist` (k x k float32,
+    contiguous, CUDA) and every tensor of `out` (shapes of GuideTree for the same k; treedist may be None) are made by
+    the caller beforehand. k <= GUIDE_TREE_STATIC_MAX_K, else QpError(STATIC_LIMIT). All calls on a device share the one
+    scratch array: keep them on one stream, or order them, or they race. The first call per device resolves the array's
+    address; make it outside stream capture. Enqueued on the stream, not synchronised."""
+    import torch
+    assert dist.is_cuda and dist.dtype == torch.float32 and dist.dim() == 2 and dist.shape[0] == dist.shape[1]
+    assert dist.is_contiguous(), "no copy is made here: pass a contiguous matrix"
+    k, dev = int(dist.shape[0]), dist.device
+    assert out.leaves.numel() == 2 * k - 1 and out.parent.numel() == 2 * k - 1 and out.merge.numel() == 2 * max(k - 1, 0)
+    assert out.height.numel() == max(k - 1, 0) and (out.treedist is None or out.treedist.numel() == k * k)
+    st = stream if stream is not None else torch.cuda.current_stream(dev)
+    with torch.cuda.device(dev):
+        code = _lib.qp_guide_tree_static(dist.data_ptr(), k, out.merge.data_ptr(), out.height.data_ptr(),
+                                         out.leaves.data_ptr(), out.parent.data_ptr(),
+                                         out.treedist.data_ptr() if out.treedist is not None else None,
+                                         C.c_void_p(st.cuda_stream))
+    if code != QP_OK:
+        raise QpError(code)
+    return out
 
 
 def last_tau_curve(max_bins: int = 128):
