@@ -222,12 +222,12 @@ struct MaxW64 {
 };
 // Slot plan of the fp64 re-evaluation queue (RefineQ in qp_internal.h).
 // which = 0, schedule time, before k_slots: the pollers' slots come off the head of the slot region, at most half of
-//   it: up to kPollCtas slots per class that can receive pairs, each sized for the largest pair of the class; classes
+//   it: up to poll_max (poll_ctas(sms)) slots per class that can receive pairs, each sized for the largest pair of the class; classes
 //   are served in ascending slot size and a class that does not fit gets fewer pollers or none (the drainers take
 //   its pairs). What was taken is recorded in poll_bytes; the fp32 slots start behind it.
 // which = 1, after the fp32 classes have joined: the drainers' slots reuse the fp32 slot region; one slot for every
 //   class with pairs left (a misfit is an error), then the rest of the region class by class.
-__global__ void k_refine_plan(int which, MaxW64 maxw, int64_t avail, const PairInfo* __restrict__ info,
+__global__ void k_refine_plan(int which, MaxW64 maxw, int poll_max, int64_t avail, const PairInfo* __restrict__ info,
                               const int32_t* __restrict__ order, SchedHeader* h) {
     if (threadIdx.x != 0 || blockIdx.x != 0) return;
     RefineQ& rq = h->rq;
@@ -243,7 +243,7 @@ __global__ void k_refine_plan(int which, MaxW64 maxw, int64_t avail, const PairI
             const unsigned long long sb = (rq.poll_slot_bytes[c] + 255ull) & ~255ull;
             rq.poll_slot_bytes[c] = sb;
             int W = 0;
-            if (rq.possible[c] > 0 && sb > 0) W = (int)min((long long)min(rq.possible[c], kPollCtas), (long long)((room - used) / sb));
+            if (rq.possible[c] > 0 && sb > 0) W = (int)min((long long)min(rq.possible[c], poll_max), (long long)((room - used) / sb));
             rq.Wpoll[c] = W;
             rq.poll_slot0[c] = used;
             used += (unsigned long long)W * sb;
@@ -672,7 +672,7 @@ extern "C" int qp_workspace_bytes(const int64_t* h_offsets, int32_t k, const int
         if ((kMaskRefine >> c) & 1) ref_full += sz64[c] * (uint64_t)std::min<int64_t>(cnt64[c], max_units(c, true, sms));
     full = std::max(full, std::min<uint64_t>(ref_full, 4ull << 30));
     // the pollers run beside the fp32 classes in a region of their own (at most half of the slot region, k_refine_plan):
-    // kPollCtas slots per class that can receive pairs
+    // at most kPollCtas slots per class that can receive pairs (this query does not touch the device: the upper bound)
     uint64_t poll_full = 0;
     for (int c = 0; c < kNumClasses; ++c)
         if ((kMaskRefine >> c) & 1) poll_full += sz64[c] * (uint64_t)std::min<int64_t>(cnt64[c], kPollCtas);
@@ -760,7 +760,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
     MaxW64 mw64;
     for (int c = 0; c < kNumClasses; ++c) mw64.w[c] = ((kMaskRefine >> c) & 1) ? max_units(c, true, sms) : 0;
     if (pollers) {   // the pollers' slots come off the head of the slot region
-        k_refine_plan<<<1, 32, 0, st>>>(0, mw64, avail, (const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), hdr);
+        k_refine_plan<<<1, 32, 0, st>>>(0, mw64, poll_ctas(sms), avail, (const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), hdr);
         ++g_launches;
     }
     MaxW mw;
@@ -806,7 +806,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
         for (int c = kSplitEnd - 1; c >= kNumPacked; --c) {
             cudaStream_t es = cx->st[kNumClasses + (c - kNumPacked)];
             QP_TRY(cudaStreamWaitEvent(es, cx->fork, 0));
-            r = launch_class_f64(true, params->pf.n_ins, c, *ka64, kPollCtas, es);
+            r = launch_class_f64(true, params->pf.n_ins, c, *ka64, poll_ctas(sms), es);
             if (r) return fail(r);
             QP_TRY(cudaEventRecord(cx->join[kNumClasses + (c - kNumPacked)], es));
         }
@@ -815,7 +815,7 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
 
     // ---- drainers: what the pollers have not taken when the fp32 classes have finished ----------------------------
     if (refine) {
-        k_refine_plan<<<1, 32, 0, st>>>(1, mw64, avail, (const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), hdr);
+        k_refine_plan<<<1, 32, 0, st>>>(1, mw64, poll_ctas(sms), avail, (const PairInfo*)(ws + L.info), (const int32_t*)(ws + L.order), hdr);
         ++g_launches;
         QP_TRY(cudaEventRecord(cx->fork2, st));
         ka64->refine_pass = 2;

@@ -163,13 +163,16 @@ QP_HD2 uint64_t bin_ub(int b) {
 // pair kernels append the pairs whose fp32 distance is below the limit; two sets of fp64 kernels consume the lists
 // through one cursor per class:
 //   pollers  a few CTAs per class, launched with the fp32 classes (after them, so they take SM room only when the fp32
-//            kernels leave some): they wait for entries to appear, and leave when every fp32 CTA has finished and the
-//            list is drained. Their scratch slots are reserved at schedule time, sized for the largest pair the class
-//            could receive.
+//            kernels leave some): they wait for entries to appear, claim a position only when its entry is visible,
+//            and leave when every fp32 CTA has finished and the list is drained -- or after kPollIdleMax empty polls in
+//            a row, so that no number of calls in flight can keep every SM busy with waiting CTAs (qp_kernel.cuh).
+//            Their scratch slots are reserved at schedule time, sized for the largest pair the class could receive.
 //   drainers full-width kernels launched after the fp32 classes have joined, for what is left; slots from the fp32
 //            slot region, sized for the largest pair actually queued.
-constexpr int kPollCtas = 32;         // pollers per class: 3 x 32 CTAs can never fill the 148 SMs, so the fp32 kernels
-                                      // always find room whatever order the hardware places CTAs in
+constexpr int kPollCtas = 32;         // most pollers per class; poll_ctas() scales it to the device
+constexpr int kPollIdleMax = 8192;    // empty polls in a row (2 us apart, ~20 ms) after which a poller leaves
+// pollers per class on a device of `sms` SMs: the three fp64 classes together never ask for more than 2/3 of them
+__host__ __device__ constexpr int poll_ctas(int sms) { return sms * 2 / 9 < 1 ? 1 : (sms * 2 / 9 < kPollCtas ? sms * 2 / 9 : kPollCtas); }
 constexpr int kListPad = 1024;        // every consumer CTA may pull one index past the end of the list
 struct RefineQ {
     int32_t count[kNumClasses];                   // pairs queued, per fp64 class

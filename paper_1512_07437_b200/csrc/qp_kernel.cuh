@@ -55,8 +55,15 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
     const int unit = W == 1 ? blockIdx.x * kWarpsPerCta + warp : blockIdx.x;   // who owns a scratch slot
     SchedHeader* hdr = ka.hdr;
     if constexpr ((MODE & 3) == kModeDist) {
-        // consumer of the fp64 re-evaluation queue (split classes only): pull list positions through the class cursor;
-        // a poller waits for its position to be filled until every fp32 class CTA has exited
+        // consumer of the fp64 re-evaluation queue (split classes only). Drainers (launched after the fp32 classes have
+        // joined: every entry is visible) take list positions with an atomicAdd on the class cursor. Pollers run beside
+        // the fp32 kernels that fill the list and must never be what keeps those kernels off the SMs, so a poller
+        //   - claims a position only once its entry is visible (compare-and-swap on the cursor): it can leave at any
+        //     time without owing the list anything, the drainers take whatever is left;
+        //   - leaves when every fp32 class warp has exited and the list is drained, OR after kPollIdleMax polls in a
+        //     row that found nothing (~20 ms). The second rule makes the call's progress independent of which CTAs
+        //     the hardware makes resident first: however many calls, streams or processes share the device, and
+        //     however few SMs the context has, waiting CTAs go away by themselves.
         static_assert(W > 1, "the distance-only kernels are split-class kernels");
         RefineQ& q = hdr->rq;
         const bool poll = ka.refine_pass == 1;
@@ -66,16 +73,29 @@ pair_kernel(const __grid_constant__ KArgs<R> ka) {
         const int32_t* list = refine_list_of(ka, cls);
         for (;;) {
             if (threadIdx.x == 0) {
-                const int pos = atomicAdd(&q.cursor[cls], 1);
-                int v;
-                for (;;) {
-                    v = ld_acquire_gpu(list + pos);
-                    if (v >= 0) break;
-                    if (ld_acquire_gpu(&hdr->producers_done) >= ka.producers_total) {   // nothing more will be queued
+                int v = -1;
+                if (!poll) {
+                    v = ld_acquire_gpu(list + atomicAdd(&q.cursor[cls], 1));
+                } else {
+                    for (int idle = 0;;) {
+                        const int pos = ld_acquire_gpu(&q.cursor[cls]);
                         v = ld_acquire_gpu(list + pos);
-                        break;
+                        if (v >= 0) {
+                            if (atomicCAS(&q.cursor[cls], pos, pos + 1) == pos) break;   // ours
+                            idle = 0;                                                    // another consumer took it
+                            continue;
+                        }
+                        if (ld_acquire_gpu(&hdr->producers_done) >= ka.producers_total) {   // nothing more will be queued
+                            if (ld_acquire_gpu(list + ld_acquire_gpu(&q.cursor[cls])) >= 0) continue;   // a late entry
+                            v = -1;
+                            break;
+                        }
+                        if (++idle > kPollIdleMax) {   // give the SM back; the drainers finish the list
+                            v = -1;
+                            break;
+                        }
+                        __nanosleep(2000);
                     }
-                    __nanosleep(2000);
                 }
                 cs->next = v;
             }

@@ -722,6 +722,45 @@ def test_concurrent_callers_threads_and_interleaved_streams(default_params):
         assert same(ra, refs[0]) and same(rb, refs[2])
 
 
+@pytest.mark.timeout(600, method="thread")
+def test_large_calls_in_flight_with_pollers_finish_and_agree(default_params):
+    """Three configs[2]-sized calls (19 900 pairs each, every one wide enough to fill the GPU by itself), WITH the fp64
+    pollers, enqueued back to back on three streams without any synchronisation in between, ten rounds: every call
+    finishes and returns bit for bit what it returns alone. The pollers of one call wait for that call's fp32 kernels;
+    with several calls in flight their CTAs could once have covered the SMs before those kernels were resident. They now
+    claim only visible queue entries and leave after a bounded number of empty polls (csrc/qp_kernel.cuh), so progress
+    does not depend on which CTAs the hardware places first."""
+    import torch
+    qp = _qp()
+    dev = torch.device("cuda:0")
+    fam = inputs.config_family(2)
+    pairs = inputs.all_pairs(fam.k)
+    ref = qp.run_family(fam, pairs, default_params)
+    nz = int(ref.pair_nnz_base[-1].item())
+    assert int(ref.status[3].item()) > 0, "the family must send pairs through the fp64 queue for this test to mean anything"
+    L = fam.lengths
+    n, m = L[pairs[:, 0]].astype(np.int64), L[pairs[:, 1]].astype(np.int64)
+    cp = qp.CParams(default_params, flags=0)   # pollers on (no QP_FLAG_NO_POLLERS), no synchronisation inside the call
+    cap = nz + 4096
+    d_seqs = torch.from_numpy(np.ascontiguousarray(fam.seqs)).to(dev)
+    d_offs = torch.from_numpy(np.ascontiguousarray(fam.offsets, dtype=np.int64)).to(dev)
+    d_pairs = torch.from_numpy(pairs).to(dev)
+    wsb = qp.workspace_bytes(fam.offsets, fam.k, pairs, cp, cap)
+    wss = [torch.empty(wsb, dtype=torch.uint8, device=dev) for _ in range(3)]
+    streams = [torch.cuda.Stream() for _ in range(3)]
+    kw = dict(nnz_capacity=cap, h_rows_total=int((n + 1).sum()), check=False)
+    res = [None] * 3
+    torch.cuda.synchronize()
+    for _ in range(10):
+        for q in range(3):
+            res[q] = qp.posteriors(d_seqs, d_offs, fam.k, d_pairs, cp, wss[q], stream=streams[q], reuse=res[q], **kw)
+        torch.cuda.synchronize()
+        for r in res:
+            assert int(r.status[0].item()) == 0 and int(r.status[3].item()) == int(ref.status[3].item())
+            assert torch.equal(r.dist, ref.dist) and torch.equal(r.pair_nnz_base, ref.pair_nnz_base)
+            assert torch.equal(r.val[:nz], ref.val[:nz]) and torch.equal(r.col_idx[:nz], ref.col_idx[:nz])
+
+
 @pytest.mark.parametrize("kind", ["random", "log_uniform", "near_identical"])
 def test_minimum_workspace_is_enough(default_params, kind):
     """A workspace of EXACTLY the minimum that qp_workspace_bytes reports (one scratch slot per class) runs the call and
