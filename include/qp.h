@@ -50,10 +50,14 @@ enum { QP_FP32 = 0, QP_FP64 = 1 };
 enum {
     QP_FLAG_SYNC_STATUS = 1,        /* synchronise the stream at the end and return the device status          */
     QP_FLAG_NO_REFINE = 2,          /* QP_FP32 only: skip the fp64 re-evaluation of near-identical pairs        */
-    QP_FLAG_NO_POLLERS = 4          /* QP_FP32 only: do not start the fp64 re-evaluation beside the fp32 kernels, only
-                                       after them. For callers that keep several calls in flight on different streams
-                                       (qp_posteriors_host): the waiting kernels of one call would sit in front of the
-                                       next call's kernels in the hardware queues they share                      */
+    QP_FLAG_NO_POLLERS = 4          /* QP_FP32 only: run the fp64 re-evaluation only AFTER the fp32 kernels (drainers), not
+                                       also beside them (pollers). Pollers are kernels that wait, on the device, for the
+                                       fp32 kernels of the same call to queue pairs. They never block progress: a poller
+                                       claims only entries that are already visible and leaves after ~20 ms without
+                                       work, whatever else shares the device. But with several calls in flight on
+                                       different streams the waiting kernels of one call sit in front of the next call's
+                                       kernels in the hardware queues they share and cost throughput: such callers
+                                       (qp_posteriors_host does) should set this flag                               */
 };
 
 /*
@@ -96,7 +100,7 @@ typedef struct {
     float* dense_P;          /* optional: concatenated dense n_p*m_p row-major matrices, pair order (tests)    */
     double* logZ;            /* optional [P][4]: ln Z of hmm fwd, hmm bwd, pf fwd, pf bwd                        */
     int32_t* status;         /* [4] device status word: {code, pair index or -1, detail, pairs whose distance was
-                                re-evaluated in fp64 (predicted near-identical pairs + those found by the fp32 pass)} */
+                                re-evaluated in fp64 (those whose fp32 distance came out below refine_below)}       */
 } qp_output;
 
 /*
@@ -306,25 +310,28 @@ int qp_last_launch_count(void);
  * Phase timing for bench.py's roofline line. qp_set_profile(1) makes later qp_posteriors calls on this thread
  * record CUDA events on the caller's stream at the phase boundaries (no synchronisation is added). After the
  * caller has synchronised the stream, qp_get_profile fills ms[0..3] with the device time of the last call:
- *   ms[0] schedule (a0, with the near-identical pair prediction), ms[1] pair kernels (a1-a7, all stripe classes, fork
- *   to join; the early fp64 distance queue runs beside them), ms[2] what is left after their join: the late fp64
- *   distance queue (pairs the prediction missed) and the CSR placement (scan + copy) beside it, the early queue's
- *   tail if any, ms[3] status word.
+ *   ms[0] schedule (a0), ms[1] pair kernels (a1-a7, all classes, fork to join; the pollers of the fp64 distance queue
+ *   run beside them), ms[2] what is left after their join: the drainers of the fp64 distance queue (pairs the pollers
+ *   had not taken) and the CSR placement (scan + copy) beside them, the pollers' tail if any, ms[3] status word.
  * Returns QP_OK, or QP_ERR_INVALID_ARG if no profiled call has completed.
  */
 void qp_set_profile(int on);
 int qp_get_profile(float ms[4]);
-/* Per scheduling class c (0..14: packed, one warp per pair, stripe width C = c+2; 15..17: split, the warps of a
- * CTA share one long pair; 18..21: packed two-block, one warp per pair of 513..768 columns, C = c-18+9): start and
- * stop of its pair kernel in ms after the end of the schedule phase, -1 for classes that did not run. Same
- * preconditions as qp_get_profile. */
+/* Per scheduling class c: start and stop of its pair kernel in ms after the end of the schedule phase, -1 for classes
+ * that did not run. Same preconditions as qp_get_profile.
+ *   0..14   packed: one warp per pair, stripe width C = c + 2, at most 32 C columns (one column block)
+ *   15..17  split: the 4 warps of a CTA share one long pair (C = 8, 12, 16)
+ *   18..21  packed multi-block: one warp per pair, C = c - 18 + 9, the column blocks of 32 C columns one after the other.
+ *           Takes pairs of 513..768 columns (two or three blocks) and, in class 21, every pair of at most 256 rows and
+ *           4e5 cells whatever its width (up to ~170 blocks): a split pass would spend more on its ramp than on the rows */
 #define QP_NUM_CLASSES 22
 int qp_get_profile_classes(float start_ms[QP_NUM_CLASSES], float stop_ms[QP_NUM_CLASSES]);
 
 /*
  * Releases what the library keeps per host thread and device between calls: the side streams and events that fork
  * and join the per-class kernels (created lazily by the first qp_posteriors call of a thread on a device). Call it
- * from the thread that made the calls, after its streams have been synchronised. Later calls re-create them.
+ * from the thread that made the calls, after its streams have been synchronised. Later calls re-create them. A thread
+ * that exits without calling it releases them on its way out (the work it enqueued should have been synchronised).
  */
 void qp_shutdown(void);
 

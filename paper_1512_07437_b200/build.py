@@ -32,8 +32,20 @@ def _newer(target, deps):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def _flags_changed() -> bool:
+    """The flags are part of the rebuild key: objects built with other flags (QP_EXTRA_NVCC_FLAGS) are stale."""
+    stamp = os.path.join(OBJ, "nvcc_flags.txt")
+    want = " ".join(NVCC_FLAGS)
+    have = open(stamp).read() if os.path.exists(stamp) else None
+    if have != want:
+        with open(stamp, "w") as f:
+            f.write(want)
+    return have is not None and have != want
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
+    force = _flags_changed() or force
     srcs = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
     hdrs = glob.glob(os.path.join(CSRC, "*.h")) + glob.glob(os.path.join(CSRC, "*.cuh")) + \
         glob.glob(os.path.join(INC, "*.h"))

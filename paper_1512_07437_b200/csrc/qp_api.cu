@@ -315,7 +315,11 @@ static thread_local Ctx* g_ctx = nullptr;     // context of the last call on thi
 static void ctx_destroy(Ctx* c) {
     if (!c) return;
     int cur = -1;
-    cudaGetDevice(&cur);
+    if (cudaGetDevice(&cur) != cudaSuccess) {   // no usable runtime (e.g. process teardown): only the host object goes
+        (void)cudaGetLastError();
+        delete c;
+        return;
+    }
     if (c->dev >= 0) cudaSetDevice(c->dev);
     if (c->ok) {
         for (int q = 0; q < kNumStreams; ++q) {
@@ -331,6 +335,21 @@ static void ctx_destroy(Ctx* c) {
     (void)cudaGetLastError();
     delete c;
 }
+
+// A host thread that exits without qp_shutdown() must not leak its 26 streams and ~75 events per device: the first
+// context a thread creates arms this owner, whose destructor runs at thread exit and releases what is left.
+struct CtxOwner {
+    bool armed = false;
+    ~CtxOwner() {
+        if (!armed) return;
+        for (int d = 0; d < kMaxDevices; ++d) {
+            ctx_destroy(g_ctxs[d]);
+            g_ctxs[d] = nullptr;
+        }
+        g_ctx = nullptr;
+    }
+};
+static thread_local CtxOwner g_ctx_owner;
 
 static Ctx* ctx_get() {
     int dev;
@@ -353,6 +372,7 @@ static Ctx* ctx_get() {
     }
     c->ok = true;
     g_ctxs[dev] = c;
+    g_ctx_owner.armed = true;
     return g_ctx = c;
 }
 
@@ -821,7 +841,8 @@ static int run_posteriors(Ctx* cx, const uint8_t* d_seqs, const int64_t* d_offse
         ka64->refine_pass = 2;
         for (int c = kNumPacked; c < kSplitEnd; ++c) {
             QP_TRY(cudaStreamWaitEvent(cx->st[c], cx->fork2, 0));
-            r = launch_class_f64(true, params->pf.n_ins, c, *ka64, class_grid(c, true, sms), cx->st[c]);
+            // every drainer CTA pulls exactly one index past the end of its list (pollers pull none): the pad bounds the grid
+            r = launch_class_f64(true, params->pf.n_ins, c, *ka64, std::min(class_grid(c, true, sms), kListPad), cx->st[c]);
             if (r) return fail(r);
             QP_TRY(cudaEventRecord(cx->join[c], cx->st[c]));
         }

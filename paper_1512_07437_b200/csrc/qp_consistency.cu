@@ -8,7 +8,9 @@
 //     S'_xy = ( 2 h_xy S_xy + sum_{z in sel(x,y)} S_xz S_zy ) / ( 2 h_xy + |sel(x,y)| )   on the pattern of S_xy,
 //     h_xy = 1 + (h - 1) min(|sel|, R) / R,   values below tau dropped.
 //
-// Design (HBM / L2 bound: ~1 multiply-add per 5 bytes read):
+// Design (measured: INSTRUCTION-bound, not bandwidth-bound -- ~350 warp instructions per (row, z) for ~4.5 useful
+// multiply-adds at 15 of 32 lanes, DRAM at 2 % of peak, profiles/r02_stage3.md; the algorithmic ratio is ~1 multiply-add
+// per 5 bytes read):
 //   k_cs_index      pair lookup table pair_of[k][k] -> (pair, orientation); per-pair column counts
 //   k_cs_transpose  per pair: an interleaved (value, column) copy of the matrix and its transpose (value, row), so
 //                   that EVERY oriented matrix S_ab (rows = residues of a) is a row-compressed list of 8-byte entries
@@ -143,14 +145,14 @@ __global__ void __launch_bounds__(kCsThreads) k_cs_transpose(CsArgs a) {
     }
     // S_xz is a factor of some relaxation only if f(d_xz, .) <= T is possible: for max and sum that needs d_xz <= T
     // (distances are >= 0). Copies of the other pairs are never read.
-    if (a.f != QP_SEL_MIN && a.treedist[(int64_t)x * a.k + y] > a.T) return;
     const int32_t* rp = a.row_ptr + a.row_base[p];
     const int64_t base = a.nnz_base[p];
     const int cnt = rp[n];
-    if (base + cnt > a.nnz) {
+    if (base + cnt > a.nnz) {   // checked for EVERY pair, copied or not: the later kernels index tmp / ent with base + e
         if (threadIdx.x == 0) cs_status(a.hdr, QP_ERR_NNZ_CAPACITY, (int)p);
         return;
     }
+    if (a.f != QP_SEL_MIN && a.treedist[(int64_t)x * a.k + y] > a.T) return;
     const int32_t* col = a.col_idx + base;
     const float* val = a.val + base;
     float2* e0 = a.ent + base;             // direct, interleaved
@@ -333,7 +335,21 @@ __global__ void __launch_bounds__(kCsThreads) k_cs_relax(CsArgs a) {
     }
     // ---- amplify, normalise, threshold; kept entries are packed at the start of their row ------------
     const int r = rtot;
-    if (!touched) {   // nothing selected: S' = S, the placement copies the input entries themselves
+    if (!touched) {   // nothing selected: S' = S cut at the threshold
+        // a stage-III threshold above the one the input was cut at drops entries here too (include/qp.h: "values below
+        // `threshold` are dropped", whatever |sel| is); only when every entry passes -- the usual case, the same tau in
+        // both stages -- does the placement copy the input entries themselves
+        int below = 0;
+        for (int e = tid; e < cnt; e += kCsThreads) below |= valxy[e] < a.tau;
+        below = __syncthreads_or(below);
+        if (below) {   // CTA-uniform: zero accumulators, then the general path with r = 0 gives v = (2 S + 0) / 2 = S exactly
+            if (cached) for (int e = tid; e < cnt; e += kCsThreads) acc_s[e] = 0.f;
+            else for (int e = tid; e < cnt; e += kCsThreads) tmp[e].x = 0.f;
+            touched = true;
+            __syncthreads();
+        }
+    }
+    if (!touched) {
         for (int i = tid; i <= n; i += kCsThreads) orp[i] = rp[i];
         if (tid == 0) {
             a.nnz_pair[p] = -cnt - 1;                          // negative: "copy from the input"

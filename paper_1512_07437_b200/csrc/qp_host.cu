@@ -262,6 +262,14 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         }                           \
     } while (0)
     QP_H(cudaMallocHost((void**)&h_small, 2 * 64));
+    for (int q = 0; q < 16; ++q) h_small[q] = 0;
+    // every copy, event and wait below goes through ck(): a failure is remembered and ends the call with QP_ERR_CUDA
+    // instead of letting collect() read sizes and status words that never arrived
+    bool cuda_bad = false;
+    auto ck = [&](cudaError_t e) {
+        if (e != cudaSuccess) cuda_bad = true;
+    };
+    constexpr int32_t kNotArrived = INT32_MIN;   // h_status[0] before the batch's status word has landed
     QP_H(cudaStreamCreateWithFlags(&comp, cudaStreamNonBlocking));
     for (int q = 0; q < 2; ++q) {
         Slot& s = sl[q];
@@ -296,26 +304,29 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
     // ---- inputs host -> device, once ---------------------------------------------------------------------------------
     cudaEvent_t up;
     QP_H(cudaEventCreateWithFlags(&up, cudaEventDisableTiming));
-    cudaMemcpyAsync(d_seqs, h_seqs + h_offsets[0], (size_t)seq_bytes, cudaMemcpyHostToDevice, main);
+    ck(cudaMemcpyAsync(d_seqs, h_seqs + h_offsets[0], (size_t)seq_bytes, cudaMemcpyHostToDevice, main));
+    std::vector<int64_t> shifted;   // lives until the end of the call
     if (h_offsets[0] == 0) {
-        cudaMemcpyAsync(d_offs, h_offsets, (size_t)(k + 1) * 8, cudaMemcpyHostToDevice, main);
-    } else {   // the device copy of the sequences starts at 0
-        std::vector<int64_t> sh(k + 1);
-        for (int q = 0; q <= k; ++q) sh[q] = h_offsets[q] - h_offsets[0];
-        cudaMemcpy(d_offs, sh.data(), (size_t)(k + 1) * 8, cudaMemcpyHostToDevice);
+        ck(cudaMemcpyAsync(d_offs, h_offsets, (size_t)(k + 1) * 8, cudaMemcpyHostToDevice, main));
+    } else {   // the device copy of the sequences starts at 0; the copy is ordered on `main` like the others (earlier
+               // work of the caller on that stream may still be using the workspace)
+        shifted.resize(k + 1);
+        for (int q = 0; q <= k; ++q) shifted[q] = h_offsets[q] - h_offsets[0];
+        ck(cudaMemcpyAsync(d_offs, shifted.data(), (size_t)(k + 1) * 8, cudaMemcpyHostToDevice, main));
     }
-    cudaMemsetAsync(d_dist, 0, (size_t)k * k * 4, main);
-    cudaEventRecord(up, main);
+    ck(cudaMemsetAsync(d_dist, 0, (size_t)k * k * 4, main));
+    ck(cudaEventRecord(up, main));
     out->h2d_bytes += seq_bytes + (int64_t)(k + 1) * 8;
-    cudaStreamWaitEvent(comp, up, 0);
+    ck(cudaStreamWaitEvent(comp, up, 0));
 
     // enqueue one batch: pairs up, the stage, sizes and status down -- all on the compute stream, behind the copy that
     // last read the slot's buffers
     auto enqueue = [&](Slot& s, const Batch& b) -> int {
         s.cur = b;
         const int64_t nb = b.hi - b.lo;
-        cudaStreamWaitEvent(comp, s.done, 0);
-        cudaMemcpyAsync(s.pairs, h_pairs + 2 * b.lo, (size_t)nb * 8, cudaMemcpyHostToDevice, comp);
+        s.h_status[0] = kNotArrived;   // the slot's previous batch has been collected: nothing is in flight into it
+        ck(cudaStreamWaitEvent(comp, s.done, 0));
+        ck(cudaMemcpyAsync(s.pairs, h_pairs + 2 * b.lo, (size_t)nb * 8, cudaMemcpyHostToDevice, comp));
         out->h2d_bytes += nb * 8;
         qp_output o;
         o.pair_row_base = s.row_base;
@@ -331,15 +342,15 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         const int r = qp_posteriors(d_seqs, d_offs, k, s.pairs, nb, &prm, s.ws, (size_t)s.ws_bytes, &o, comp);
         if (r != QP_OK) return r;
         if (out->col_idx16) k_narrow_cols<<<1184, 256, 0, comp>>>(s.col, s.nnz_base + nb, s.cap, s.col16);
-        cudaMemcpyAsync(s.h_last, s.nnz_base + nb, 8, cudaMemcpyDeviceToHost, comp);
-        cudaMemcpyAsync(s.h_status, s.status, 16, cudaMemcpyDeviceToHost, comp);
-        cudaEventRecord(s.sized, comp);
+        ck(cudaMemcpyAsync(s.h_last, s.nnz_base + nb, 8, cudaMemcpyDeviceToHost, comp));
+        ck(cudaMemcpyAsync(s.h_status, s.status, 16, cudaMemcpyDeviceToHost, comp));
+        ck(cudaEventRecord(s.sized, comp));
         // what does not depend on the CSR size goes down on the slot's copy stream right away
-        cudaStreamWaitEvent(s.st, s.sized, 0);
-        cudaMemcpyAsync(out->row_ptr + out->pair_row_base[b.lo], s.row_ptr, (size_t)b.rows * 4, cudaMemcpyDeviceToHost, s.st);
-        cudaMemcpyAsync(out->pair_nnz_base + b.lo + 1, s.nnz_base + 1, (size_t)nb * 8, cudaMemcpyDeviceToHost, s.st);
+        ck(cudaStreamWaitEvent(s.st, s.sized, 0));
+        ck(cudaMemcpyAsync(out->row_ptr + out->pair_row_base[b.lo], s.row_ptr, (size_t)b.rows * 4, cudaMemcpyDeviceToHost, s.st));
+        ck(cudaMemcpyAsync(out->pair_nnz_base + b.lo + 1, s.nnz_base + 1, (size_t)nb * 8, cudaMemcpyDeviceToHost, s.st));
         out->d2h_bytes += 24 + b.rows * 4 + nb * 8;
-        return cudaGetLastError() == cudaSuccess ? QP_OK : QP_ERR_CUDA;
+        return cudaGetLastError() == cudaSuccess && !cuda_bad ? QP_OK : QP_ERR_CUDA;
     };
 
     // ---- the pipeline ---------------------------------------------------------------------------------------------------
@@ -367,8 +378,9 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
     };
     auto collect = [&](int q) -> int {   // sizes known -> CSR down -> fix the prefix; returns QP_OK, an error, or 1 = "split"
         Slot& s = sl[q];
-        if (cudaEventSynchronize(s.sized) != cudaSuccess) return QP_ERR_CUDA;
+        if (cudaEventSynchronize(s.sized) != cudaSuccess || cuda_bad) return QP_ERR_CUDA;
         const int code = s.h_status[0];
+        if (code == kNotArrived) return QP_ERR_CUDA;   // the status word of this batch never landed
         const Batch b = s.cur;
         const int64_t nb = b.hi - b.lo;
         if (code == QP_ERR_NNZ_CAPACITY && nb > 1) return 1;
@@ -383,12 +395,13 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         if (nnz_running + nz > out->nnz_capacity) {
             host_overflow = true;
         } else {
-            if (out->col_idx16) cudaMemcpyAsync(out->col_idx16 + nnz_running, s.col16, (size_t)nz * 2, cudaMemcpyDeviceToHost, s.st);
-            else cudaMemcpyAsync(out->col_idx + nnz_running, s.col, (size_t)nz * 4, cudaMemcpyDeviceToHost, s.st);
-            cudaMemcpyAsync(out->val + nnz_running, s.val, (size_t)nz * 4, cudaMemcpyDeviceToHost, s.st);
+            if (out->col_idx16) ck(cudaMemcpyAsync(out->col_idx16 + nnz_running, s.col16, (size_t)nz * 2, cudaMemcpyDeviceToHost, s.st));
+            else ck(cudaMemcpyAsync(out->col_idx + nnz_running, s.col, (size_t)nz * 4, cudaMemcpyDeviceToHost, s.st));
+            ck(cudaMemcpyAsync(out->val + nnz_running, s.val, (size_t)nz * 4, cudaMemcpyDeviceToHost, s.st));
             out->d2h_bytes += nz * (out->col_idx16 ? 6 : 8);
         }
-        cudaEventRecord(s.done, s.st);
+        ck(cudaEventRecord(s.done, s.st));
+        if (cuda_bad) return QP_ERR_CUDA;
         s.out_nnz0 = nnz_running;   // the batch's pair_nnz_base arrives as local offsets: made global once `done` has passed
         nnz_running += nz;
         ++out->batches;
@@ -410,8 +423,8 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
         if (r == 1) {
             // denser than beta_guess: everything enqueued after this batch is abandoned (its results are simply
             // computed again), the batch goes back as two halves
-            cudaStreamSynchronize(comp);
-            for (int other : inflight) cudaStreamSynchronize(sl[other].st);
+            ck(cudaStreamSynchronize(comp));
+            for (int other : inflight) ck(cudaStreamSynchronize(sl[other].st));
             for (size_t u = inflight.size(); u-- > 1;) work.push_back(sl[inflight[u]].cur);
             const Batch b = sl[q].cur;
             int64_t mid = b.lo, acc = 0;
@@ -427,22 +440,24 @@ extern "C" int qp_posteriors_host(const uint8_t* h_seqs, const int64_t* h_offset
             work.push_back(lo_half);
             inflight.clear();
             next_slot = 0;
-            cudaEventRecord(sl[0].done, sl[0].st);
-            cudaEventRecord(sl[1].done, sl[1].st);
+            ck(cudaEventRecord(sl[0].done, sl[0].st));
+            ck(cudaEventRecord(sl[1].done, sl[1].st));
+            if (cuda_bad) rc = QP_ERR_CUDA;
             continue;
         }
         rc = r;
         inflight.erase(inflight.begin());
     }
-    cudaStreamSynchronize(comp);
+    ck(cudaStreamSynchronize(comp));
     for (int q = 0; q < 2; ++q) {
-        cudaStreamSynchronize(sl[q].st);
+        ck(cudaStreamSynchronize(sl[q].st));
+        if (rc == QP_OK && cuda_bad) rc = QP_ERR_CUDA;
         if (rc == QP_OK) apply_fixups(q);
     }
     if (rc == QP_OK) {
-        cudaMemcpyAsync(out->dist, d_dist, (size_t)k * k * 4, cudaMemcpyDeviceToHost, main);
+        ck(cudaMemcpyAsync(out->dist, d_dist, (size_t)k * k * 4, cudaMemcpyDeviceToHost, main));
         out->d2h_bytes += (int64_t)k * k * 4;
-        if (cudaStreamSynchronize(main) != cudaSuccess) rc = QP_ERR_CUDA;
+        if (cudaStreamSynchronize(main) != cudaSuccess || cuda_bad) rc = QP_ERR_CUDA;
     }
     cudaEventDestroy(up);
     cleanup();

@@ -173,7 +173,8 @@ constexpr int kPollCtas = 32;         // most pollers per class; poll_ctas() sca
 constexpr int kPollIdleMax = 8192;    // empty polls in a row (2 us apart, ~20 ms) after which a poller leaves
 // pollers per class on a device of `sms` SMs: the three fp64 classes together never ask for more than 2/3 of them
 __host__ __device__ constexpr int poll_ctas(int sms) { return sms * 2 / 9 < 1 ? 1 : (sms * 2 / 9 < kPollCtas ? sms * 2 / 9 : kPollCtas); }
-constexpr int kListPad = 1024;        // every consumer CTA may pull one index past the end of the list
+constexpr int kListPad = 1024;        // every DRAINER CTA pulls one index past the end of its list: the drainer grid is
+                                      // clamped to this (qp_api.cu); pollers claim only filled positions
 struct RefineQ {
     int32_t count[kNumClasses];                   // pairs queued, per fp64 class
     int32_t cursor[kNumClasses];                  // next list position to consume

@@ -174,13 +174,13 @@ def get_profile():
 
 def get_profile_classes():
     """[(class, start_ms, stop_ms)] of the class kernels of the last profiled call (relative to the fork);
-    class = "C<stripe width>" for packed classes, "C<stripe width>xW<warps>" for split ones, "C<stripe width>x2" for
-    the packed two-block ones (fp32 naming)."""
+    class = "C<stripe width>" for packed classes, "C<stripe width>xW<warps>" for split ones, "C<stripe width>mb" for
+    the packed multi-block ones (one warp, the column blocks one after the other; fp32 naming)."""
     a, b = (C.c_float * NUM_CLASSES)(), (C.c_float * NUM_CLASSES)()
     r = _lib.qp_get_profile_classes(a, b)
     if r != QP_OK:
         raise QpError(r)
-    names = ["C%d" % (c + 2) for c in range(15)] + ["C8xW4", "C12xW4", "C16xW4"] + ["C%dx2" % C for C in range(9, 13)]
+    names = ["C%d" % (c + 2) for c in range(15)] + ["C8xW4", "C12xW4", "C16xW4"] + ["C%dmb" % C for C in range(9, 13)]
     return [(names[c], round(a[c], 3), round(b[c], 3)) for c in range(NUM_CLASSES) if a[c] >= 0]
 
 

@@ -114,7 +114,7 @@ def _check_extra(p, extra, val, rows, col, tau):
     assert (v < tau + BAND).all(), f"pair {p}: {int((v >= tau + BAND).sum())} entries kept that the oracle dropped"
 
 
-def _run_case(fam, pairs, prm, T, f="max", h=3.0, passes=1):
+def _run_case(fam, pairs, prm, T, f="max", h=3.0, passes=1, tau3=None):
     import torch
     qp = _qp()
     dev = torch.device("cuda:0")
@@ -125,11 +125,12 @@ def _run_case(fam, pairs, prm, T, f="max", h=3.0, passes=1):
     csr, nnz = _upload(S, pairs, fam, dev)
     fsel = {"max": oc.SEL_MAX, "min": oc.SEL_MIN, "sum": oc.SEL_SUM}[f]
     worst = 0.0
+    tau3 = prm.threshold if tau3 is None else tau3   # stage III's own threshold (normally stage I's)
     for it in range(passes):
-        ref, cnt = oc.transform(S, fam.k, td, T=T, f=fsel, h=h, max_relax=200, tau=prm.threshold)
+        ref, cnt = oc.transform(S, fam.k, td, T=T, f=fsel, h=h, max_relax=200, tau=tau3)
         res = qp.consistency(d_offs, fam.k, d_pairs, csr, d_td, h_offsets=fam.offsets, h_pairs=pairs, nnz=nnz, T=T, f=f,
-                             h=h, max_relax=200, threshold=prm.threshold)
-        worst = max(worst, _compare(res, ref, cnt, pairs, fam, prm.threshold))
+                             h=h, max_relax=200, threshold=tau3)
+        worst = max(worst, _compare(res, ref, cnt, pairs, fam, tau3))
         if it + 1 < passes:
             # second transformation (k < 50): both sides continue from the ORACLE's first result
             S = {key: oc.from_csr(M.indptr, M.indices, M.data.astype(np.float32).astype(np.float64), *M.shape)
@@ -146,6 +147,18 @@ def test_cfg0_all_pairs(default_params, T, f):
     pairs = inputs.all_pairs(fam.k)
     worst, nrel = _run_case(fam, pairs, default_params, T, f, passes=_qp().consistency_passes(fam.k))
     print(f"cfg0 T={T} f={f}: {nrel} relaxations, worst |dS'| {worst:.2e}")
+
+
+@pytest.mark.parametrize("T", [0, 5, 200])
+def test_threshold_above_stage_one_cuts_unrelaxed_pairs_too(default_params, T):
+    """A stage-III threshold (0.05) above the one the input was cut at (0.01): include/qp.h drops relaxed values below
+    it, and the oracle's relax_pair does so whether or not any z was selected -- so the pairs with |sel| = 0 (all of
+    them at T = 0, some at T = 5) lose their small entries as well instead of being copied through unchanged."""
+    fam = inputs.config_family(0)
+    pairs = inputs.all_pairs(fam.k)
+    worst, nrel = _run_case(fam, pairs, default_params, T, tau3=0.05)
+    assert (nrel == 0) == (T == 0)
+    print(f"cfg0 T={T} tau3=0.05: {nrel} relaxations, worst |dS'| {worst:.2e}")
 
 
 def test_cfg1_all_pairs(default_params):
@@ -269,6 +282,12 @@ def test_error_paths_and_empty_input(default_params):
     with pytest.raises(qp.QpError) as ei:
         qp.consistency(d_offs, fam.k, d_pairs, csr, d_td, workspace=small, **kw)
     assert ei.value.code == qp.ERR["WORKSPACE_TOO_SMALL"]
+    # an entry count smaller than what the matrices hold is caught for every pair, also for the pairs that are too far
+    # apart to be a factor of anything (T = 0: nothing is selected, none of the copies is ever built)
+    for T in (9, 0):
+        with pytest.raises(qp.QpError) as ei:
+            qp.consistency(d_offs, fam.k, d_pairs, csr, d_td, **dict(kw, nnz=nnz - 1, T=T))
+        assert ei.value.code == qp.ERR["NNZ_CAPACITY"]
     # empty pair list
     none = np.zeros((0, 2), np.int32)
     r0 = qp.consistency(d_offs, fam.k, torch.from_numpy(none).to(dev), csr, d_td, **dict(kw, h_pairs=none, nnz=0))
