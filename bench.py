@@ -47,16 +47,21 @@ def peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(cfg):
-    """dram bytes (read + write) of the pair kernels of one step, from the committed ncu captures
-    (profiles/traffic.csv: config,dram_bytes_per_step), or None if this config was not captured."""
+def ncu_census(cfg):
+    """(dram bytes read + written, warp instructions) of the pair kernels of one step of configs[cfg], from the committed
+    ncu capture (profiles/traffic.csv: config,dram_bytes_per_step,warp_instr_per_step; profiles/r03_dram.md names the
+    command), or (None, None) if this config was not captured. A kernel change makes the file stale: re-capture it."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
     if os.path.exists(p):
         for ln in open(p):
             f = ln.strip().split(",")
-            if len(f) == 2 and f[0].isdigit() and int(f[0]) == cfg:
-                return float(f[1])
-    return None
+            if len(f) >= 2 and f[0].isdigit() and int(f[0]) == cfg:
+                return float(f[1]), (float(f[2]) if len(f) > 2 and f[2] else None)
+    return None, None
+
+
+def ncu_traffic(cfg):
+    return ncu_census(cfg)[0]
 
 
 class ClockSampler(threading.Thread):
@@ -282,7 +287,10 @@ def roofline_of(cfg, m, clocks, dev=None):
     mhz = (clocks or {}).get("sm_mhz") or 1965
     alu = alu_peaks(dev) if dev is not None else None
     issue_rate = alu["warp_instr_per_s"] if alu else N_SMS * 4 * mhz * 1e6
-    issue_s = WARP_INSTR_PER_CELL * cells / issue_rate
+    census_instr = ncu_census(cfg)[1]   # this config's own count when it was captured, else the configs[2] census
+    own = bool(census_instr) and m.get("total_cells") == cells   # the census counts the whole config, not a rank's shard
+    instr_per_cell = census_instr / cells if own else WARP_INSTR_PER_CELL
+    issue_s = instr_per_cell * cells / issue_rate
     return {"bound": "hbm", "achieved": achieved, "peak": hbm_peak, "unit": "GB/s", "frac": achieved / hbm_peak,
             "traffic": ncu_traffic(cfg), "peak_source": peak_src,
             "frac_note": "whole step (schedule + pair kernels + fp64 distance queues + CSR placement) over the HBM peak",
@@ -293,7 +301,10 @@ def roofline_of(cfg, m, clocks, dev=None):
             "traffic_note": "dram read+write bytes of those launches from ncu (profiles/traffic.csv), per step",
             "algorithmic_bytes_per_cell": ALGO_BYTES_PER_CELL,
             "phases_ms": {k: round(v, 3) for k, v in prof.items()},
-            "issue": {"warp_instr_per_cell": WARP_INSTR_PER_CELL, "sm_mhz": mhz, "warp_instr_per_s": issue_rate,
+            "issue": {"warp_instr_per_cell": instr_per_cell,
+                      "warp_instr_source": ("ncu census of this config (profiles/traffic.csv)" if own
+                                            else "borrowed: the configs[2] census (profiles/r02_ncu_full_cfg2.md)"),
+                      "sm_mhz": mhz, "warp_instr_per_s": issue_rate,
                       "bound_ms": 1e3 * issue_s, "frac": issue_s / kern_s,
                       "note": "warp instructions per cell (ncu census, profiles/) x cells / the MEASURED issue rate "
                               "(qp_measure_peaks: scalar FFMA lane-ops per second / 32) over the pair-kernel time"},
